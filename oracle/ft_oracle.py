@@ -1,0 +1,150 @@
+"""ctypes front-end of the CPU ORACLE (oracle/ft_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module; the product package never does, and nothing here imports the product's
+CUDA binding.  It takes a `Workload`-like object (duck-typed: the seeded input module is the
+only thing the two sides share) and returns numpy arrays.
+
+The per-band top-k ("retrieving the loudest candidate within each region";
+north_star: per-frequency-sub-band top-k) is the plain definition written out: sort every
+template of a band by (ranking value descending, canonical index ascending), keep the first k.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libft_oracle.so")
+_SRC = os.path.join(_HERE, "ft_oracle.c")
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off (no FMA contraction: the canonical op order is literal)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
+               "-std=c11", "-Wall", "-o", _SO, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+class _Problem(C.Structure):
+    _fields_ = [
+        ("P", C.c_void_p), ("n_sft", C.c_int64), ("n_bins", C.c_int64), ("ld", C.c_int64),
+        ("t_mid", C.c_void_p), ("vel", C.c_void_p), ("w", C.c_void_p), ("wkind", C.c_int32),
+        ("f_min", C.c_double), ("df", C.c_double),
+        ("f0_start", C.c_double), ("df0", C.c_double), ("n_f0", C.c_int64),
+        ("f1_start", C.c_double), ("df1", C.c_double), ("n_f1", C.c_int64),
+        ("t_ref", C.c_double),
+        ("n_sky", C.c_int64), ("sky", C.c_void_p),
+        ("n_ap", C.c_int64), ("a_p", C.c_void_p),
+        ("n_porb", C.c_int64), ("P_orb", C.c_void_p),
+        ("n_tasc", C.c_int64), ("tasc_frac", C.c_void_p),
+        ("rho_th", C.c_double),
+    ]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.fto_track.restype = C.c_int
+        _lib.fto_eval_range.restype = C.c_int
+        _lib.fto_eval_list.restype = C.c_int
+        _lib.fto_num_threads.restype = C.c_int
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().fto_num_threads())
+
+
+class Oracle:
+    """Binds one workload (spectrogram + tables + grid) and evaluates templates on the CPU."""
+
+    def __init__(self, wl, rho_th=None):
+        self.lib = _load()
+        g = wl.grid
+        self._keep = dict(
+            P=np.ascontiguousarray(wl.P, dtype=np.float32),
+            t_mid=np.ascontiguousarray(wl.t_mid, dtype=np.float64),
+            vel=np.ascontiguousarray(wl.vel, dtype=np.float64),
+            w=np.ascontiguousarray(wl.w, dtype=np.float32),
+            sky=np.ascontiguousarray(g.sky, dtype=np.float64),
+            a_p=np.ascontiguousarray(g.a_p, dtype=np.float64),
+            P_orb=np.ascontiguousarray(g.P_orb, dtype=np.float64),
+            tasc=np.ascontiguousarray(g.tasc_frac, dtype=np.float64),
+        )
+        k = self._keep
+        n_sft, n_bins = k["P"].shape
+        assert k["t_mid"].shape == (n_sft,) and k["vel"].shape == (n_sft, 3)
+        wkind = 2 if k["w"].ndim == 2 else 1
+        assert k["w"].shape == ((n_sft, n_bins) if wkind == 2 else (n_sft,))
+        p = lambda a: a.ctypes.data_as(C.c_void_p)
+        self.pb = _Problem(
+            p(k["P"]), n_sft, n_bins, n_bins, p(k["t_mid"]), p(k["vel"]), p(k["w"]), wkind,
+            float(wl.f_min), float(wl.df),
+            float(g.f0_start), float(g.df0), int(g.n_f0),
+            float(g.f1_start), float(g.df1), int(g.n_f1), float(g.t_ref),
+            len(k["sky"]), p(k["sky"]), len(k["a_p"]), p(k["a_p"]),
+            len(k["P_orb"]), p(k["P_orb"]), len(k["tasc"]), p(k["tasc"]),
+            float(wl.rho_th if rho_th is None else rho_th))
+        self.n_sft, self.n_bins = n_sft, n_bins
+        self.dims = (len(k["sky"]), len(k["a_p"]), len(k["P_orb"]), len(k["tasc"]), int(g.n_f1),
+                     int(g.n_f0))
+        self.n_templates = int(np.prod([int(d) for d in self.dims], dtype=object))
+
+    def track(self, idx: int):
+        """bins k[n_sft] (int64), positions x[n_sft] (fp64) of one template; rc != 0 = out of range."""
+        k = np.empty(self.n_sft, dtype=np.int64)
+        x = np.empty(self.n_sft, dtype=np.float64)
+        rc = self.lib.fto_track(C.byref(self.pb), C.c_uint64(int(idx)),
+                                k.ctypes.data_as(C.c_void_p), x.ctypes.data_as(C.c_void_p))
+        return k, x, rc
+
+    def _outs(self, n):
+        return (np.empty(n, np.float64), np.empty(n, np.int32), np.empty(n, np.float64),
+                np.empty(n, np.uint8))
+
+    def eval_range(self, begin: int = 0, end=None):
+        """(power f64, count i32, wcount f64, near_tie u8) for canonical indices [begin, end)."""
+        end = self.n_templates if end is None else end
+        o = self._outs(end - begin)
+        rc = self.lib.fto_eval_range(C.byref(self.pb), C.c_uint64(begin), C.c_uint64(end),
+                                     *[a.ctypes.data_as(C.c_void_p) for a in o])
+        if rc != 0:
+            raise ValueError(f"oracle: a track left the spectrogram (rc={rc})")
+        return o
+
+    def eval_list(self, idx):
+        idx = np.ascontiguousarray(idx, dtype=np.uint64)
+        o = self._outs(idx.size)
+        rc = self.lib.fto_eval_list(C.byref(self.pb), idx.ctypes.data_as(C.c_void_p),
+                                    C.c_int64(idx.size), *[a.ctypes.data_as(C.c_void_p) for a in o])
+        if rc != 0:
+            raise ValueError(f"oracle: a track left the spectrogram (rc={rc})")
+        return o
+
+
+def topk_per_band(values, n_f0: int, bins_per_band: int, k: int, idx_begin: int = 0):
+    """Plain definition of the per-band top-k over a FULL statistic array.
+
+    values[j] is the ranking value of canonical index idx_begin + j (idx_begin a multiple of
+    n_f0).  Band of a template = (idx % n_f0) // bins_per_band.  Returns a list over bands of
+    (idx[k'], value[k']) sorted by (value desc, idx asc), k' = min(k, templates in band)."""
+    values = np.asarray(values)
+    idx = np.arange(values.size, dtype=np.uint64) + np.uint64(idx_begin)
+    band = (idx % np.uint64(n_f0)).astype(np.int64) // bins_per_band
+    n_bands = (n_f0 + bins_per_band - 1) // bins_per_band
+    out = []
+    for b in range(n_bands):
+        sel = np.flatnonzero(band == b)
+        order = np.lexsort((idx[sel], -values[sel].astype(np.float64)))[:k]
+        out.append((idx[sel][order], values[sel][order]))
+    return out

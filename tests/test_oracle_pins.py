@@ -1,0 +1,379 @@
+"""Pins of the CPU oracle (oracle/ft_oracle.c) against what the paper and the mathematics fix.
+
+The paper prints no worked numeric example (PAPER.md has no input/output pair for Eq. 3), so every
+pin is a closed form, an invariant, a special case that reduces to a library routine, an exact /
+50-digit evaluation, or brute force on tiny inputs.  Each test says which mistake it would catch.
+"""
+import math
+from fractions import Fraction
+
+import mpmath
+import numpy as np
+import pytest
+
+from oracle import ft_oracle as fo
+from paper_2411_18370_b200 import workloads as W
+
+
+def _simple_workload(n_sft=64, n_bins=256, df=1.0 / 1800.0, f_lo=100.0, pad=40, n_f0=None, seed=7,
+                     vel=None, grid_kw=None, w=None, P=None, t_mid=None):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    T = 1.0 / df
+    t_mid = (np.arange(n_sft) + 0.5) * T if t_mid is None else t_mid
+    vel = W.earth_velocity(t_mid, 46.45, 0.0) if vel is None else vel
+    P = (-np.log(1.0 - rng.random((n_sft, n_bins)))).astype(np.float32) if P is None else P
+    w = np.full(n_sft, 1.0 / n_sft, np.float32) if w is None else w
+    n_f0 = n_bins - 2 * pad if n_f0 is None else n_f0
+    g = dict(f0_start=f_lo, df0=df, n_f0=n_f0)
+    g.update(grid_kw or {})
+    return W.Workload("t", 99, P, t_mid, vel, w, f_lo - pad * df, df, W.Grid(**g), "both", 1.6,
+                      0.01, 5, T)
+
+
+# ---------------------------------------------------------------- T1: Eq. (13)-(14) noise moments
+def test_noise_mean_and_variance_eq13_eq14(golden):
+    """Catches: a dropped weight, wrong normalisation, gathering the same pixel twice."""
+    wl = W.config2(n_sft=400, n_sky=3)
+    o = fo.Oracle(wl)
+    n_f0 = wl.grid.n_f0
+    power = o.eval_range(0, n_f0)[0]          # one sky point, one f1: disjoint columns -> independent
+    w = wl.w.astype(np.float64)
+    mean_th = golden["noise_mean_per_sum_w_exp1"] * w.sum()
+    var_th = golden["noise_var_per_sum_w2_exp1"] * (w ** 2).sum()
+    se = math.sqrt(var_th / n_f0)
+    assert abs(power.mean() - mean_th) < 4 * se
+    assert abs(power.var() / var_th - 1.0) < 4 * math.sqrt(2.0 / n_f0) + 0.05
+    # chi^2_2 scale of the paper: multiply pixels by 2 -> mu_G = 2 sum w (Eq. 13)
+    wl2 = W.config2(n_sft=400, n_sky=3)
+    wl2.P *= np.float32(2.0)
+    p2 = fo.Oracle(wl2).eval_range(0, n_f0)[0]
+    assert abs(p2.mean() - golden["noise_mean_per_sum_w_chi2"] * w.sum()) < 8 * se
+
+
+# ---------------------------------------------------------------- T2: Eq. (7), (11) binomial count
+def test_hough_count_is_binomial(golden):
+    """Catches: >= instead of >, threshold on the wrong scale, count not integer/in range."""
+    wl = W.config2(n_sft=400, n_sky=3)
+    o = fo.Oracle(wl, rho_th=golden["hough_threshold_exp1"])
+    n_f0, n = wl.grid.n_f0, wl.n_sft
+    _, cnt, wcnt, _ = o.eval_range(0, n_f0)
+    p = golden["hough_p"]
+    assert p == pytest.approx(math.exp(-golden["hough_threshold_chi2"] / 2.0), rel=1e-15)
+    assert cnt.min() >= 0 and cnt.max() <= n
+    assert abs(cnt.mean() - n * p) < 4 * math.sqrt(n * p * (1 - p) / n_f0)
+    assert abs(cnt.var() / (n * p * (1 - p)) - 1.0) < 4 * math.sqrt(2.0 / n_f0) + 0.05
+    # weighted count: mean = p * sum w (Eq. 3 applied to Eq. 7)
+    w = wl.w.astype(np.float64)
+    assert abs(wcnt.mean() - p * w.sum()) < 4 * math.sqrt(p * (1 - p) * (w ** 2).sum() / n_f0)
+    # non-increasing in rho_th; strict '>' : threshold equal to a pixel value excludes it
+    c_lo = fo.Oracle(wl, rho_th=1.0).eval_range(0, n_f0)[1]
+    c_hi = fo.Oracle(wl, rho_th=2.5).eval_range(0, n_f0)[1]
+    assert np.all(c_lo >= cnt) and np.all(cnt >= c_hi)
+
+
+def test_hough_strict_greater_than():
+    P = np.full((8, 64), 1.6, np.float32)   # (float)1.6 == pixel -> not counted (strict >)
+    wl = _simple_workload(n_sft=8, n_bins=64, pad=20, P=P)
+    assert np.all(fo.Oracle(wl, rho_th=1.6).eval_range()[1] == 0)
+    assert np.all(fo.Oracle(wl, rho_th=np.nextafter(np.float32(1.6), np.float32(0))).eval_range()[1] == 8)
+
+
+# ---------------------------------------------------------------- T3: a_p = 0 is the isolated track
+def test_ap_zero_reduces_to_isolated():
+    """PAPER.md:56 'For a_p = 0 the source effectively behaves like an isolated one'."""
+    base = _simple_workload(grid_kw=dict(sky=W.fibonacci_sphere(4)))
+    iso = fo.Oracle(base).eval_range()
+    binw = _simple_workload(grid_kw=dict(sky=W.fibonacci_sphere(4), a_p=np.array([0.0, 3.0]),
+                                         P_orb=np.array([5.0, 9.0]) * 86400.0,
+                                         tasc_frac=np.array([0.0, 0.37])))
+    ob = fo.Oracle(binw)
+    full = ob.eval_range()
+    dims = ob.dims
+    pw = full[0].reshape(dims)
+    ct = full[1].reshape(dims)
+    iso_pw = iso[0].reshape(4, 1, 1, 1, 1, -1)
+    for ip in range(2):
+        for it in range(2):
+            assert np.array_equal(pw[:, 0, ip, it], iso_pw[:, 0, 0, 0])
+            assert np.array_equal(ct[:, 0, ip, it], iso[1].reshape(4, 1, 1, 1, 1, -1)[:, 0, 0, 0])
+    assert not np.array_equal(pw[:, 1, 0, 0], iso_pw[:, 0, 0, 0])  # a_p = 3 does move the track
+
+
+# ---------------------------------------------------------------- T4: straight line = column sum
+def test_zero_velocity_is_weighted_column_sum():
+    """v = 0, a_p = 0, f1 = 0: s(f0_i) = sum_alpha w_alpha P[alpha][pad + i] — a GEMV (w^T P).
+    Catches: transposed spectrogram, off-by-one in the bin origin, weight index mix-up."""
+    n_sft, n_bins, pad = 50, 200, 30
+    rng = np.random.Generator(np.random.PCG64(3))
+    w = rng.random(n_sft).astype(np.float32)
+    wl = _simple_workload(n_sft=n_sft, n_bins=n_bins, pad=pad, vel=np.zeros((n_sft, 3)), w=w)
+    pw, ct, wc, _ = fo.Oracle(wl).eval_range()
+    ref = w.astype(np.float64) @ wl.P.astype(np.float64)
+    assert np.allclose(pw, ref[pad:n_bins - pad], rtol=1e-13, atol=0)
+    assert np.array_equal(ct, (wl.P > np.float32(1.6)).sum(0)[pad:n_bins - pad])
+    refc = w.astype(np.float64) @ (wl.P > np.float32(1.6)).astype(np.float64)
+    assert np.allclose(wc, refc[pad:n_bins - pad], rtol=1e-13)
+    # per-bin weights: same reduction with w[alpha][k]
+    w2 = rng.random((n_sft, n_bins)).astype(np.float32)
+    wl2 = _simple_workload(n_sft=n_sft, n_bins=n_bins, pad=pad, vel=np.zeros((n_sft, 3)), w=w2)
+    pw2 = fo.Oracle(wl2).eval_range()[0]
+    ref2 = (w2.astype(np.float64) * wl2.P.astype(np.float64)).sum(0)
+    assert np.allclose(pw2, ref2[pad:n_bins - pad], rtol=1e-13)
+
+
+# ---------------------------------------------------------------- T5: injected track
+def test_injected_track_recovers_exact_sum():
+    """Eq. (3) on a noiseless spectrogram with amplitude A along lambda*: s = A sum w, count = n_sft,
+    mismatch m(lambda*; lambda*) = 0 (Eq. 24); every other template scores <= that."""
+    n_sft = 80
+    g = dict(sky=W.fibonacci_sphere(5), a_p=np.array([0.0, 2.0, 4.0]),
+             P_orb=np.array([3.0, 4.5]) * 86400.0, tasc_frac=np.array([0.1, 0.6]))
+    rng = np.random.Generator(np.random.PCG64(11))
+    w = (rng.random(n_sft) + 0.5).astype(np.float32)
+    wl = _simple_workload(n_sft=n_sft, n_bins=256, pad=40, grid_kw=g, w=w,
+                          P=np.zeros((n_sft, 256), np.float32))
+    o = fo.Oracle(wl)
+    star = int(wl.grid.ravel(3, 2, 1, 1, 0, 77))
+    k, _, rc = o.track(star)
+    assert rc == 0
+    A = 2.0
+    W.inject(wl.P, k, A)
+    o = fo.Oracle(wl)
+    pw, ct, _, _ = o.eval_range()
+    assert pw[star] == pytest.approx(A * w.astype(np.float64).sum(), rel=1e-14)
+    assert ct[star] == n_sft
+    assert np.all(pw <= pw[star]) and np.all(ct <= n_sft)
+    mu_g = 0.0  # noiseless
+    assert (pw[star] - pw[star]) / (pw[star] - mu_g) == 0.0   # Eq. (24) at the true template
+
+
+# ---------------------------------------------------------------- T6: one-bin resolution, Eq. (27)
+def test_resolution_property_eq27_eqA1_eq28():
+    """delta f0 = 1/T_SFT (Eq. A1) moves every bin by 1 (0 or 2 only across a rounding boundary);
+    delta a_p = 1/(T_SFT f0 Omega) and delta phi_b = 1/(T_SFT f0 a_p Omega) (Eq. 28) move the
+    track by about one bin at most.  Catches: wrong units of a_p/Omega, missing factor f0."""
+    T, f0 = 900.0, 150.0
+    n_sft = 960
+    t_mid = (np.arange(n_sft) + 0.5) * T
+    P_orb, a_p = 10.0 * T * 96, 8.0         # 10 days in units of T_SFT
+    Om = 2 * math.pi / P_orb
+    d_ap = 1.0 / (T * f0 * Om)
+    d_phi = 1.0 / (T * f0 * a_p * Om)       # radians; as a t_asc fraction: d_phi / (2 pi)
+    g = dict(f0_start=f0, df0=1.0 / T, n_f0=3, a_p=np.array([a_p, a_p + d_ap]),
+             P_orb=np.array([P_orb]), tasc_frac=np.array([0.25, 0.25 + d_phi / (2 * math.pi)]))
+    wl = _simple_workload(n_sft=n_sft, n_bins=400, df=1.0 / T, f_lo=f0, pad=150, t_mid=t_mid,
+                          grid_kw=g)
+    o = fo.Oracle(wl)
+    k000 = o.track(int(wl.grid.ravel(0, 0, 0, 0, 0, 0)))[0]
+    k_f0 = o.track(int(wl.grid.ravel(0, 0, 0, 0, 0, 1)))[0]
+    k_ap = o.track(int(wl.grid.ravel(0, 1, 0, 0, 0, 0)))[0]
+    k_ph = o.track(int(wl.grid.ravel(0, 0, 0, 1, 0, 0)))[0]
+    d = k_f0 - k000
+    assert set(np.unique(d)) <= {0, 1, 2} and (d == 1).mean() > 0.99
+    for kk in (k_ap, k_ph):
+        assert 1 <= np.abs(kk - k000).max() <= 2
+    # a 10x finer step than the resolution leaves most of the track unchanged
+    g2 = dict(g, a_p=np.array([a_p, a_p + 0.1 * d_ap]))
+    wl2 = _simple_workload(n_sft=n_sft, n_bins=400, df=1.0 / T, f_lo=f0, pad=150, t_mid=t_mid,
+                           grid_kw=g2)
+    o2 = fo.Oracle(wl2)
+    same = o2.track(int(wl2.grid.ravel(0, 1, 0, 0, 0, 0)))[0] == o2.track(0)[0]
+    assert same.mean() > 0.85
+
+
+# ---------------------------------------------------------------- closed-form binary extremes
+def test_binary_track_extremes_and_period():
+    """At v = 0 the track is f0 [1 - a_p Omega cos(Omega (t - t_asc))] (Eq. 2): its extreme bins are
+    rint((f0 (1 -+ a_p Omega) - f_min)/df) and the bin sequence has period P_orb on a gap-free grid.
+    Catches: sin for cos, wrong sign of the binary term, Omega = P/2pi, t_asc not t_ref + u P."""
+    T = 900.0
+    per = 64                                   # P_orb = 64 T_SFT
+    n_sft = 4 * per
+    t_mid = (np.arange(n_sft) + 0.5) * T
+    P_orb, a_p, f0, u = per * T, 40.0, 150.0, 0.5 / per  # t_asc = t_mid[0]
+    g = dict(f0_start=f0, df0=1.0 / T, n_f0=2, a_p=np.array([a_p]), P_orb=np.array([P_orb]),
+             tasc_frac=np.array([u]))
+    wl = _simple_workload(n_sft=n_sft, n_bins=1200, df=1.0 / T, f_lo=f0, pad=590, t_mid=t_mid,
+                          vel=np.zeros((n_sft, 3)), grid_kw=g)
+    k, x, rc = fo.Oracle(wl).track(0)
+    assert rc == 0
+    Om = 2 * math.pi / P_orb
+    lo = round((f0 * (1 - a_p * Om) - wl.f_min) * T)
+    hi = round((f0 * (1 + a_p * Om) - wl.f_min) * T)
+    assert k[0] == lo == k.min()               # cos(0) = 1 at t = t_asc: minimum frequency
+    assert k[per // 2] == hi == k.max()        # half an orbit later: maximum
+    assert hi - lo > 300                       # the modulation is resolved (not a trivial pass)
+    assert np.array_equal(k[:-per], k[per:])   # period P_orb
+    assert not np.array_equal(k[:-per // 2], k[per // 2:])
+
+
+# ---------------------------------------------------------------- exact-rational track (isolated)
+def _half_even(fr: Fraction) -> int:
+    fl = math.floor(fr)
+    r = fr - fl
+    if r > Fraction(1, 2) or (r == Fraction(1, 2) and fl % 2 == 1):
+        return fl + 1
+    return fl
+
+
+def test_isolated_track_against_exact_rational_arithmetic():
+    """Evaluate Eq. (2) (with f1) in exact rational arithmetic from the same double inputs; the
+    fp64 oracle must give the same bin except within 1e-9 of a tie, and x within 1e-9.
+    Catches: any dropped term, sign, operand or index error in the track."""
+    wl = W.config2(n_sft=120, n_sky=7)
+    o = fo.Oracle(wl)
+    g = wl.grid
+    rng = np.random.Generator(np.random.PCG64(5))
+    c = Fraction(299792458)
+    for idx in rng.integers(0, g.n_templates, 12):
+        i_sky, _, _, _, i_f1, i_f0 = (int(v) for v in g.unravel(idx))
+        k, x, rc = o.track(int(idx))
+        assert rc == 0
+        f0 = Fraction(g.f0_start) + i_f0 * Fraction(g.df0)
+        f1 = Fraction(g.f1_start) + i_f1 * Fraction(g.df1)
+        n = [Fraction(float(v)) for v in g.sky[i_sky]]
+        for a in range(0, wl.n_sft, 7):
+            t = Fraction(float(wl.t_mid[a]))
+            V = sum(Fraction(float(wl.vel[a, j])) * n[j] for j in range(3)) / c
+            xe = ((f0 + f1 * (t - Fraction(g.t_ref))) * (1 + V) - Fraction(wl.f_min)) / Fraction(wl.df)
+            assert abs(float(xe) - x[a]) < 1e-9
+            if abs((xe - math.floor(xe)) - Fraction(1, 2)) > Fraction(1, 10 ** 8):
+                assert _half_even(xe) == k[a]
+
+
+def test_binary_track_against_50_digit_evaluation():
+    """Same as above with the binary term, in 50-digit mpmath (true pi, true cos)."""
+    mpmath.mp.dps = 50
+    wl = W.config3(n_sft=200, n_ap=5, n_porb=4, n_tasc=3, n_inj=0)
+    o = fo.Oracle(wl)
+    g = wl.grid
+    rng = np.random.Generator(np.random.PCG64(6))
+    mpf = mpmath.mpf
+    for idx in rng.integers(0, g.n_templates, 10):
+        i_sky, i_ap, i_po, i_ta, _, i_f0 = (int(v) for v in g.unravel(idx))
+        k, x, rc = o.track(int(idx))
+        assert rc == 0
+        f0 = mpf(g.f0_start) + i_f0 * mpf(g.df0)
+        Om = 2 * mpmath.pi / mpf(float(g.P_orb[i_po]))
+        t_asc = mpf(g.t_ref) + mpf(float(g.tasc_frac[i_ta])) * mpf(float(g.P_orb[i_po]))
+        n = [mpf(float(v)) for v in g.sky[i_sky]]
+        for a in range(0, wl.n_sft, 5):
+            t = mpf(float(wl.t_mid[a]))
+            V = sum(mpf(float(wl.vel[a, j])) * n[j] for j in range(3)) / mpf(299792458)
+            B = mpf(float(g.a_p[i_ap])) * Om * mpmath.cos(Om * (t - t_asc))
+            xe = (f0 * (1 + V - B) - mpf(wl.f_min)) / mpf(wl.df)
+            assert abs(xe - mpf(float(x[a]))) < mpf(10) ** -9
+            if abs((xe - mpmath.floor(xe)) - mpf(1) / 2) > mpf(10) ** -8:
+                assert int(mpmath.nint(xe)) == k[a]
+
+
+# ---------------------------------------------------------------- rounding mode (reading R5)
+def test_round_half_to_even_and_near_tie_flag():
+    n_sft, n_bins = 4, 16
+    P = np.arange(n_sft * n_bins, dtype=np.float32).reshape(n_sft, n_bins)
+    t_mid = np.arange(n_sft) + 0.5
+    for f0, k_expect in ((2.5, 2), (3.5, 4), (4.5, 4), (2.25, 2), (2.75, 3)):
+        wl = W.Workload("r", 99, P, t_mid, np.zeros((n_sft, 3)), np.ones(n_sft, np.float32), 0.0, 1.0,
+                        W.Grid(f0_start=f0, df0=1.0, n_f0=1), "both", 1.6, 1.0, 1, 1.0)
+        o = fo.Oracle(wl)
+        k, x, _ = o.track(0)
+        assert np.all(k == k_expect) and np.all(x == f0)
+        tie = o.eval_range()[3][0]
+        assert tie == (1 if f0 % 1 == 0.5 else 0)
+        assert o.eval_range()[0][0] == P[:, k_expect].astype(np.float64).sum()
+
+
+def test_track_out_of_range_is_an_error():
+    wl = _simple_workload(n_sft=8, n_bins=64, pad=0)    # no Doppler padding: tracks leave the band
+    o = fo.Oracle(wl)
+    with pytest.raises(ValueError):
+        o.eval_range()
+
+
+# ---------------------------------------------------------------- T7: metamorphic
+def test_linearity_and_permutation_invariance():
+    wl = W.config2(n_sft=160, n_sky=4)
+    o = fo.Oracle(wl)
+    pw, ct, wc, _ = o.eval_range(0, 3000)
+    wl2 = W.config2(n_sft=160, n_sky=4)
+    wl2.P *= np.float32(2.0)                       # exact scaling
+    pw2 = fo.Oracle(wl2).eval_range(0, 3000)[0]
+    assert np.array_equal(pw2, 2.0 * pw)
+    perm = np.random.Generator(np.random.PCG64(1)).permutation(wl.n_sft)
+    wl3 = W.config2(n_sft=160, n_sky=4)
+    wl3.P, wl3.t_mid, wl3.vel, wl3.w = wl3.P[perm], wl3.t_mid[perm], wl3.vel[perm], wl3.w[perm]
+    pw3, ct3, wc3, _ = fo.Oracle(wl3).eval_range(0, 3000)
+    assert np.array_equal(ct3, ct)                 # integer counts: exact under SFT reordering
+    assert np.allclose(pw3, pw, rtol=1e-13) and np.allclose(wc3, wc, rtol=1e-13)
+
+
+# ---------------------------------------------------------------- T8: brute force on tiny inputs
+def test_brute_force_python_on_tiny_grid():
+    """Independent nested-loop Python evaluation (index order by explicit loops, Python floats,
+    round() = half-even).  Catches: canonical index order / unravel mistakes, list vs range API."""
+    n_sft = 11
+    g = dict(n_f0=7, f1_start=-2e-9, df1=1e-9, n_f1=2, sky=W.fibonacci_sphere(3),
+             a_p=np.array([0.0, 1.5]), P_orb=np.array([1.0, 2.5]) * 86400.0,
+             tasc_frac=np.array([0.0, 0.4]))
+    wl = _simple_workload(n_sft=n_sft, n_bins=96, pad=40, grid_kw=g, n_f0=7)
+    wl.grid.f0_start, wl.grid.df0 = 100.0, wl.df
+    o = fo.Oracle(wl)
+    pw, ct, wc, _ = o.eval_range()
+    idx = 0
+    for sky in wl.grid.sky:
+        for ap in wl.grid.a_p:
+            for Po in wl.grid.P_orb:
+                for u in wl.grid.tasc_frac:
+                    for j in range(2):
+                        for i in range(7):
+                            f0 = 100.0 + i * wl.df
+                            f1 = -2e-9 + j * 1e-9
+                            Om = 6.283185307179586 / Po
+                            tasc = 0.0 + u * Po
+                            s, c = 0.0, 0
+                            for a in range(n_sft):
+                                t = float(wl.t_mid[a])
+                                V = ((wl.vel[a, 0] * sky[0] + wl.vel[a, 1] * sky[1]) + wl.vel[a, 2] * sky[2]) / 299792458.0
+                                B = (ap * Om) * math.cos(Om * (t - tasc)) if ap != 0.0 else 0.0
+                                x = (((f0 + f1 * (t - 0.0)) * ((1.0 + V) - B)) - wl.f_min) * (1.0 / wl.df)
+                                k = round(x)
+                                p = wl.P[a, k]
+                                s += float(wl.w[a]) * float(p)
+                                c += int(p > np.float32(1.6))
+                            assert pw[idx] == s and ct[idx] == c, idx
+                            idx += 1
+    assert idx == o.n_templates
+    sub = np.array([5, 0, 111, 77, o.n_templates - 1], dtype=np.uint64)
+    lp, lc, lw, _ = o.eval_list(sub)
+    assert np.array_equal(lp, pw[sub.astype(np.int64)]) and np.array_equal(lc, ct[sub.astype(np.int64)])
+    rp = o.eval_range(70, 90)[0]
+    assert np.array_equal(rp, pw[70:90])
+
+
+def test_topk_per_band_is_exhaustive_sort():
+    """Brute force with Python's sorted() on config 1 (T8): (value desc, index asc), k per band."""
+    wl = W.config1()
+    o = fo.Oracle(wl)
+    pw, ct, _, _ = o.eval_range()
+    n_f0, bpb, k = wl.grid.n_f0, 18, 5
+    for vals in (pw, ct):
+        got = fo.topk_per_band(vals, n_f0, bpb, k)
+        assert len(got) == 10
+        for b, (gi, gv) in enumerate(got):
+            members = [(-float(vals[j]), j) for j in range(vals.size) if (j % n_f0) // bpb == b]
+            ref = sorted(members)[:k]
+            assert [j for _, j in ref] == [int(v) for v in gi]
+            assert [-v for v, _ in ref] == [float(v) for v in gv]
+
+
+def test_config1_injection_is_loudest_in_its_band():
+    wl = W.config1()
+    (tidx, amp), = wl.planned_injections
+    star = int(wl.grid.ravel(*tidx))
+    k, _, _ = fo.Oracle(wl).track(star)
+    before = fo.Oracle(wl).eval_range()[0]
+    W.inject(wl.P, k, amp)
+    after = fo.Oracle(wl).eval_range()[0]
+    assert after[star] == pytest.approx(before[star] + amp * float(wl.w.astype(np.float64).sum()), rel=1e-6)  # fp32 pixels
+    top = fo.topk_per_band(after, wl.grid.n_f0, 18, 5)
+    assert int(top[90 // 18][0][0]) == star
