@@ -1,0 +1,423 @@
+// C ABI of libfasttracks_b200 (include/fasttracks_b200.h): handle, validation, launch orchestration.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/fasttracks_b200.h"
+#include "ft_common.cuh"
+#include "ft_select.cuh"
+#include "ft_tile.cuh"
+
+struct ft_ctx {
+  cudaStream_t stream = nullptr;
+  FtDev d{};
+  bool per_bin = false;
+  // library-owned device memory
+  double* t_mid_dev = nullptr;
+  double* vel_dev = nullptr;
+  float* w_dev = nullptr;       // per-SFT weights copy
+  float* Q_dev = nullptr;       // folded per-bin weights
+  double* axes_dev = nullptr;   // sky | a_p | P_orb | tasc
+  // host copies used for validation
+  std::vector<double> t_mid, vel;
+  double vmax = 0.0, dt_min = 0.0, dt_max = 0.0;
+  // bound grid
+  bool bound = false;
+  int stat = 0;
+  double df = 0.0;
+  bool tile_ok = false;
+  FtTilePlan plan{};
+  // options
+  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0;
+  // selection buffers
+  FtSelectDev sel{};
+  uint64_t* final_idx = nullptr;
+  int32_t* final_band = nullptr;
+  uint32_t* final_n = nullptr;   // [0] final_n, [1] overflow
+  FtCandDev* cand = nullptr;
+  FtCandDev* out_dev = nullptr;
+  uint32_t final_cap = 0;
+  size_t out_cap = 0;
+  float* scratch_f = nullptr;
+  int32_t* scratch_i = nullptr;
+  size_t scratch_elems = 0;
+  unsigned long long* near_ties_dev = nullptr;
+  // bookkeeping
+  ft_counters counters{};
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool ev_valid = false;
+  std::string err = "";
+};
+
+namespace {
+
+int fail(ft_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+#define FT_CUDA(c, expr)                                                                     \
+  do {                                                                                       \
+    cudaError_t e__ = (expr);                                                                \
+    if (e__ != cudaSuccess)                                                                  \
+      return fail((c), e__ == cudaErrorMemoryAllocation ? FT_ERR_ALLOC : FT_ERR_CUDA,        \
+                  std::string(#expr) + ": " + cudaGetErrorString(e__));                      \
+  } while (0)
+
+template <typename T>
+void dfree(T*& p) {
+  if (p) cudaFree(p);
+  p = nullptr;
+}
+
+bool finite_all(const double* p, size_t n) {
+  for (size_t i = 0; i < n; ++i)
+    if (!std::isfinite(p[i])) return false;
+  return true;
+}
+
+void free_select(ft_ctx* c) {
+  dfree(c->sel.thr); dfree(c->sel.cnt); dfree(c->sel.key); dfree(c->sel.idx);
+  dfree(c->final_idx); dfree(c->final_band); dfree(c->final_n); dfree(c->cand); dfree(c->out_dev);
+  c->sel = FtSelectDev{};
+  c->final_cap = 0; c->out_cap = 0;
+}
+
+int ensure_select(ft_ctx* c, int32_t n_bands, int32_t k) {
+  uint32_t cap = (uint32_t)((1u << 24) / (uint32_t)n_bands);
+  cap = cap > 65536u ? 65536u : (cap < 4096u ? 4096u : cap);
+  const uint32_t final_cap = (uint32_t)n_bands * 2048u;
+  if (c->sel.n_bands != n_bands || c->sel.cap != cap || c->out_cap < (size_t)n_bands * k) {
+    free_select(c);
+    FT_CUDA(c, cudaMalloc(&c->sel.thr, sizeof(float) * n_bands));
+    FT_CUDA(c, cudaMalloc(&c->sel.cnt, sizeof(uint32_t) * n_bands));
+    FT_CUDA(c, cudaMalloc(&c->sel.key, sizeof(float) * (size_t)n_bands * cap));
+    FT_CUDA(c, cudaMalloc(&c->sel.idx, sizeof(uint64_t) * (size_t)n_bands * cap));
+    c->sel.cap = cap; c->sel.n_bands = n_bands;
+    FT_CUDA(c, cudaMalloc(&c->final_idx, sizeof(uint64_t) * final_cap));
+    FT_CUDA(c, cudaMalloc(&c->final_band, sizeof(int32_t) * final_cap));
+    FT_CUDA(c, cudaMalloc(&c->final_n, sizeof(uint32_t) * 2));
+    FT_CUDA(c, cudaMalloc(&c->cand, sizeof(FtCandDev) * final_cap));
+    FT_CUDA(c, cudaMalloc(&c->out_dev, sizeof(FtCandDev) * (size_t)n_bands * k));
+    c->final_cap = final_cap; c->out_cap = (size_t)n_bands * k;
+  }
+  return FT_OK;
+}
+
+int ensure_scratch(ft_ctx* c, size_t elems, bool need_int) {
+  if (c->scratch_elems < elems) {
+    dfree(c->scratch_f); dfree(c->scratch_i);
+    c->scratch_elems = 0;
+    FT_CUDA(c, cudaMalloc(&c->scratch_f, sizeof(float) * elems));
+    c->scratch_elems = elems;
+  }
+  if (need_int && !c->scratch_i) FT_CUDA(c, cudaMalloc(&c->scratch_i, sizeof(int32_t) * c->scratch_elems));
+  return FT_OK;
+}
+
+void tick(ft_ctx* c) {
+  if (!c->ev0) { cudaEventCreate(&c->ev0); cudaEventCreate(&c->ev1); }
+  cudaEventRecord(c->ev0, c->stream);
+}
+void tock(ft_ctx* c) {
+  cudaEventRecord(c->ev1, c->stream);
+  c->ev_valid = true;
+}
+
+// Statistic over points [pt_begin, pt_end): full write-out (out_* indexed from out_base) and/or
+// fused filter into c->sel.  Chooses the tile or the generic kernel.
+int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out_power, int32_t* out_count,
+             uint64_t out_base, bool filter, int32_t bpb) {
+  const bool use_tile = c->tile_ok && c->opt_kernel != 1;
+  if (use_tile) {
+    int launches = 0;
+    FT_CUDA(c, ft_launch_tile(c->d, c->plan, stat, pt_begin, pt_end, out_power, out_count, out_base,
+                              filter ? &c->sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
+    c->counters.kernel_launches += launches;
+  } else {
+    if (filter) return fail(c, FT_ERR_UNSUPPORTED, "fused filter needs the tile kernel");
+    FT_CUDA(c, ft_launch_generic(c->d, stat, pt_begin, pt_end, out_power, out_count, out_base, c->stream));
+    c->counters.kernel_launches += 1;
+  }
+  return FT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ft_create(ft_ctx** out, const float* P_dev, int64_t n_sft, int64_t n_bins, int64_t ld_bins,
+              const double* t_mid_host, const double* vel_host, const float* w, int wkind,
+              double f_min, double df, void* cuda_stream) {
+  if (!out) return FT_ERR_ARG;
+  *out = nullptr;
+  ft_ctx* c = new (std::nothrow) ft_ctx();
+  if (!c) return FT_ERR_ALLOC;
+  *out = c;  // returned even on error so ft_last_error can be read; caller still calls ft_destroy
+  if (!P_dev || !t_mid_host || !vel_host || !w) return fail(c, FT_ERR_ARG, "ft_create: NULL pointer argument");
+  if (n_sft < 1 || n_bins < 1 || ld_bins < n_bins) return fail(c, FT_ERR_ARG, "ft_create: need n_sft >= 1, 1 <= n_bins <= ld_bins");
+  if (n_sft > (1 << 24)) return fail(c, FT_ERR_ARG, "ft_create: n_sft > 2^24 (integer counts are selected as exact fp32 keys)");
+  if ((ld_bins & 3) || (reinterpret_cast<uintptr_t>(P_dev) & 15)) return fail(c, FT_ERR_ARG, "ft_create: P must be 16-byte aligned with ld_bins a multiple of 4");
+  if (wkind != FT_W_PER_SFT && wkind != FT_W_PER_SFT_BIN) return fail(c, FT_ERR_ARG, "ft_create: bad wkind");
+  if (!(df > 0.0) || !std::isfinite(df) || !std::isfinite(f_min)) return fail(c, FT_ERR_ARG, "ft_create: need finite f_min and df > 0");
+  if (!finite_all(t_mid_host, (size_t)n_sft) || !finite_all(vel_host, (size_t)n_sft * 3)) return fail(c, FT_ERR_ARG, "ft_create: non-finite t_mid / vel");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(c, FT_ERR_CUDA, "ft_create: no CUDA device (this library has no CPU fallback)");
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->t_mid.assign(t_mid_host, t_mid_host + n_sft);
+  c->vel.assign(vel_host, vel_host + 3 * n_sft);
+  for (int64_t a = 0; a < n_sft; ++a) {
+    const double* v = vel_host + 3 * a;
+    c->vmax = std::fmax(c->vmax, std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
+  }
+  FT_CUDA(c, cudaMalloc(&c->t_mid_dev, sizeof(double) * n_sft));
+  FT_CUDA(c, cudaMalloc(&c->vel_dev, sizeof(double) * 3 * n_sft));
+  FT_CUDA(c, cudaMemcpyAsync(c->t_mid_dev, t_mid_host, sizeof(double) * n_sft, cudaMemcpyHostToDevice, c->stream));
+  FT_CUDA(c, cudaMemcpyAsync(c->vel_dev, vel_host, sizeof(double) * 3 * n_sft, cudaMemcpyHostToDevice, c->stream));
+  FT_CUDA(c, cudaMalloc(&c->near_ties_dev, sizeof(unsigned long long)));
+  FT_CUDA(c, cudaMemsetAsync(c->near_ties_dev, 0, sizeof(unsigned long long), c->stream));
+  FtDev& d = c->d;
+  d.P = P_dev; d.n_sft = n_sft; d.n_bins = n_bins; d.ld = ld_bins;
+  d.t_mid = c->t_mid_dev; d.vel = c->vel_dev;
+  d.wkind = wkind; d.f_min = f_min; d.inv_df = 1.0 / df;
+  c->df = df;
+  c->per_bin = (wkind == FT_W_PER_SFT_BIN);
+  if (!c->per_bin) {
+    FT_CUDA(c, cudaMalloc(&c->w_dev, sizeof(float) * n_sft));
+    FT_CUDA(c, cudaMemcpyAsync(c->w_dev, w, sizeof(float) * n_sft, cudaMemcpyHostToDevice, c->stream));
+    d.w = c->w_dev; d.Q = nullptr;
+  } else {
+    if (reinterpret_cast<uintptr_t>(w) & 15) return fail(c, FT_ERR_ARG, "ft_create: per-bin weights must be 16-byte aligned");
+    d.w = w;
+    // fold Q = w*P once (one fp32 rounding per pixel; the fp64 refinement uses w and P unfolded)
+    FT_CUDA(c, cudaMalloc(&c->Q_dev, sizeof(float) * (size_t)n_sft * ld_bins));
+    FT_CUDA(c, ft_launch_fold(P_dev, w, c->Q_dev, n_sft * ld_bins, c->stream));
+    c->counters.kernel_launches += 1;
+    d.Q = c->Q_dev;
+  }
+  FT_CUDA(c, cudaStreamSynchronize(c->stream));  // host tables may be freed by the caller now
+  return FT_OK;
+}
+
+int ft_set_option(ft_ctx* c, int option, int64_t value) {
+  if (!c) return FT_ERR_ARG;
+  switch (option) {
+    case FT_OPT_KERNEL: if (value < 0 || value > 2) return fail(c, FT_ERR_ARG, "FT_OPT_KERNEL: 0..2"); c->opt_kernel = value; break;
+    case FT_OPT_FUSED_TOPK: c->opt_fused = value ? 1 : 0; break;
+    case FT_OPT_POINTS_PER_CTA: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_POINTS_PER_CTA >= 0"); c->opt_ppc = value; break;
+    default: return fail(c, FT_ERR_ARG, "unknown option");
+  }
+  if (c->bound) c->bound = false;  // options change the plan: re-bind with ft_eval
+  return FT_OK;
+}
+
+int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_power_dev, int32_t* out_count_dev) {
+  if (!c || !g) return FT_ERR_ARG;
+  c->bound = false;
+  if (stat < 0 || stat > 2) return fail(c, FT_ERR_ARG, "ft_eval: bad stat");
+  if (!g->sky || !g->a_p || !g->P_orb || !g->tasc_frac) return fail(c, FT_ERR_ARG, "ft_eval: NULL grid axis");
+  if (g->n_f0 < 1 || g->n_f1 < 1 || g->n_sky < 1 || g->n_ap < 1 || g->n_porb < 1 || g->n_tasc < 1) return fail(c, FT_ERR_ARG, "ft_eval: empty grid axis");
+  const double scal[] = {g->f0_start, g->df0, g->f1_start, g->df1, g->t_ref, rho_th};
+  if (!finite_all(scal, 6) || !finite_all(g->sky, 3 * (size_t)g->n_sky) || !finite_all(g->a_p, g->n_ap) ||
+      !finite_all(g->P_orb, g->n_porb) || !finite_all(g->tasc_frac, g->n_tasc))
+    return fail(c, FT_ERR_ARG, "ft_eval: non-finite grid value");
+  if (g->n_f0 > 1 && !(g->df0 > 0.0)) return fail(c, FT_ERR_ARG, "ft_eval: df0 must be > 0");
+  for (int i = 0; i < g->n_porb; ++i) if (!(g->P_orb[i] > 0.0)) return fail(c, FT_ERR_ARG, "ft_eval: P_orb must be > 0");
+  // conservative bound on every track (header: FT_ERR_TRACK_RANGE; reading R9)
+  double ap_max = 0.0, porb_min = g->P_orb[0], n_max = 0.0;
+  for (int i = 0; i < g->n_ap; ++i) ap_max = std::fmax(ap_max, std::fabs(g->a_p[i]));
+  for (int i = 0; i < g->n_porb; ++i) porb_min = std::fmin(porb_min, g->P_orb[i]);
+  for (int64_t i = 0; i < g->n_sky; ++i) {
+    const double* n = g->sky + 3 * i;
+    n_max = std::fmax(n_max, std::sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]));
+  }
+  const double eps = c->vmax * n_max / FT_C_LIGHT + ap_max * FT_TWO_PI / porb_min;
+  double dt_lo = c->t_mid[0] - g->t_ref, dt_hi = dt_lo;
+  for (double t : c->t_mid) { dt_lo = std::fmin(dt_lo, t - g->t_ref); dt_hi = std::fmax(dt_hi, t - g->t_ref); }
+  const double f1a = g->f1_start, f1b = g->f1_start + (double)(g->n_f1 - 1) * g->df1;
+  const double cands[4] = {f1a * dt_lo, f1a * dt_hi, f1b * dt_lo, f1b * dt_hi};
+  double f1dt_lo = cands[0], f1dt_hi = cands[0];
+  for (double v : cands) { f1dt_lo = std::fmin(f1dt_lo, v); f1dt_hi = std::fmax(f1dt_hi, v); }
+  const double fs_lo = g->f0_start + f1dt_lo, fs_hi = g->f0_start + (double)(g->n_f0 - 1) * g->df0 + f1dt_hi;
+  if (!(fs_lo > 0.0) || !(eps < 0.01)) return fail(c, FT_ERR_ARG, "ft_eval: need positive frequencies and |Doppler| < 1e-2");
+  const double x_lo = (fs_lo * (1.0 - eps) - c->d.f_min) / c->df, x_hi = (fs_hi * (1.0 + eps) - c->d.f_min) / c->df;
+  if (x_lo < -0.49 || x_hi > (double)(c->d.n_bins - 1) + 0.49) {
+    char buf[256];
+    std::snprintf(buf, sizeof buf, "ft_eval: tracks may leave the spectrogram: bound [%.2f, %.2f] bins vs [0, %lld)", x_lo, x_hi, (long long)c->d.n_bins);
+    return fail(c, FT_ERR_TRACK_RANGE, buf);
+  }
+  // copy axes
+  const size_t n_ax = 3 * (size_t)g->n_sky + g->n_ap + g->n_porb + g->n_tasc;
+  std::vector<double> ax(n_ax);
+  std::memcpy(ax.data(), g->sky, sizeof(double) * 3 * g->n_sky);
+  size_t o = 3 * (size_t)g->n_sky;
+  std::memcpy(ax.data() + o, g->a_p, sizeof(double) * g->n_ap); o += g->n_ap;
+  std::memcpy(ax.data() + o, g->P_orb, sizeof(double) * g->n_porb); o += g->n_porb;
+  std::memcpy(ax.data() + o, g->tasc_frac, sizeof(double) * g->n_tasc);
+  FT_CUDA(c, cudaStreamSynchronize(c->stream));  // previous work may still read the old axes
+  dfree(c->axes_dev);
+  FT_CUDA(c, cudaMalloc(&c->axes_dev, sizeof(double) * n_ax));
+  FT_CUDA(c, cudaMemcpyAsync(c->axes_dev, ax.data(), sizeof(double) * n_ax, cudaMemcpyHostToDevice, c->stream));
+  FT_CUDA(c, cudaStreamSynchronize(c->stream));
+  FtDev& d = c->d;
+  d.sky = c->axes_dev; d.a_p = d.sky + 3 * g->n_sky; d.P_orb = d.a_p + g->n_ap; d.tasc = d.P_orb + g->n_porb;
+  d.n_f0 = g->n_f0; d.n_sky = g->n_sky; d.n_f1 = g->n_f1; d.n_ap = g->n_ap; d.n_porb = g->n_porb; d.n_tasc = g->n_tasc;
+  d.f0_start = g->f0_start; d.df0 = g->df0; d.f1_start = g->f1_start; d.df1 = g->df1; d.t_ref = g->t_ref;
+  d.rho = (float)rho_th;
+  d.n_points = (uint64_t)g->n_sky * g->n_ap * g->n_porb * g->n_tasc * g->n_f1;
+  c->stat = stat;
+  // tile-kernel eligibility and plan
+  c->tile_ok = false;
+  if (c->opt_kernel != 1) {
+    std::string why;
+    int launches = 0;
+    const cudaError_t e = ft_tile_plan(d, c->df, eps, stat, (int)c->opt_ppc, c->stream, &c->plan, &why, &launches);
+    c->counters.kernel_launches += launches;
+    if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_tile_plan: ") + cudaGetErrorString(e));
+    c->tile_ok = why.empty();
+    if (!c->tile_ok && c->opt_kernel == 2) return fail(c, FT_ERR_UNSUPPORTED, "tile kernel not eligible: " + why);
+  }
+  c->bound = true;
+  if (out_power_dev || out_count_dev) {
+    tick(c);
+    const int rc = run_stat(c, stat, 0, d.n_points, out_power_dev, out_count_dev, 0, false, 1);
+    tock(c);
+    if (rc != FT_OK) return rc;
+  }
+  return FT_OK;
+}
+
+int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_host, int32_t* n_bands_out) {
+  if (!c || !out_host || !n_bands_out) return FT_ERR_ARG;
+  if (!c->bound) return fail(c, FT_ERR_STATE, "ft_topk_per_band: no grid bound (call ft_eval first)");
+  const FtDev& d = c->d;
+  const double ratio = band_width_hz / d.df0;
+  const long long bpb = std::llround(ratio);
+  if (k < 1 || k > 1024 || !(band_width_hz > 0.0) || bpb < 1 || std::fabs(ratio - (double)bpb) > 1e-9 * std::fmax(1.0, ratio))
+    return fail(c, FT_ERR_BAND, "ft_topk_per_band: band_width must be an integer number of f0 steps and 1 <= k <= 1024");
+  const int64_t n_bands64 = (d.n_f0 + bpb - 1) / bpb;
+  if (n_bands64 > (1 << 20)) return fail(c, FT_ERR_BAND, "ft_topk_per_band: too many bands");
+  const int32_t n_bands = (int32_t)n_bands64;
+  *n_bands_out = n_bands;
+  int rc = ensure_select(c, n_bands, k);
+  if (rc != FT_OK) return rc;
+  const bool by_count = (c->stat == FT_STAT_HOUGH);
+  // FT_STAT_BOTH ranks by power and the fp64 refinement supplies the count: select on power alone
+  const int sel_stat = by_count ? FT_STAT_HOUGH : FT_STAT_POWER;
+  const float margin = by_count ? 0.f : 4e-5f;  // fp32 accumulation error bound 1e-5
+  const bool use_tile = c->tile_ok && c->opt_kernel != 1;
+  const bool fused = use_tile && c->opt_fused;
+  // sample / chunk size in points
+  uint64_t chunk_pts;
+  if (fused) {
+    chunk_pts = ft_tile_sample_points(c->plan, d.n_points);
+  } else {
+    const uint64_t max_elems = (uint64_t)1 << 27;  // 512 MB of fp32 scratch per chunk
+    chunk_pts = max_elems / (uint64_t)d.n_f0;
+    if (chunk_pts < 1) chunk_pts = 1;
+  }
+  if (chunk_pts > d.n_points) chunk_pts = d.n_points;
+  rc = ensure_scratch(c, (size_t)chunk_pts * d.n_f0, by_count);
+  if (rc != FT_OK) return rc;
+  uint32_t* overflow = c->final_n + 1;
+  FT_CUDA(c, ft_select_reset(c->sel, c->final_n, overflow, c->stream));
+  c->counters.kernel_launches += 1;
+  tick(c);
+  for (uint64_t pt = 0; pt < d.n_points; pt += chunk_pts) {
+    const uint64_t pe = (pt + chunk_pts < d.n_points) ? pt + chunk_pts : d.n_points;
+    if (fused && pt > 0) {  // phase B: everything after the sample goes through the fused filter
+      rc = run_stat(c, sel_stat, pt, d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb);
+      if (rc != FT_OK) return rc;
+      break;
+    }
+    rc = run_stat(c, sel_stat, pt, pe, by_count ? nullptr : c->scratch_f, by_count ? c->scratch_i : nullptr,
+                  pt * (uint64_t)d.n_f0, false, (int32_t)bpb);
+    if (rc != FT_OK) return rc;
+    const int64_t rows = (int64_t)(pe - pt);
+    if (by_count) {
+      FT_CUDA(c, ft_count_to_key(c->scratch_i, c->scratch_f, rows * d.n_f0, c->stream));
+      c->counters.kernel_launches += 1;
+    }
+    if (pt == 0) {
+      FT_CUDA(c, ft_select_threshold(c->scratch_f, rows, d.n_f0, (int32_t)bpb, (uint32_t)k, margin, c->sel, c->stream));
+      c->counters.kernel_launches += 1;
+    }
+    FT_CUDA(c, ft_select_append_keys(c->scratch_f, rows, d.n_f0, (int32_t)bpb, pt, c->sel, c->stream));
+    c->counters.kernel_launches += 1;
+  }
+  tock(c);
+  FT_CUDA(c, ft_select_trim(c->sel, (uint32_t)k, margin, c->final_idx, c->final_band, c->final_n, c->final_cap, overflow, c->stream));
+  FT_CUDA(c, ft_launch_refine(d, c->final_idx, c->final_n, c->final_cap, c->cand, c->near_ties_dev, c->stream));
+  FT_CUDA(c, ft_select_rank(c->cand, c->final_band, c->final_n, c->final_cap, by_count ? 1 : 0, (uint32_t)k, n_bands, c->out_dev, overflow, c->stream));
+  c->counters.kernel_launches += 3;
+  uint32_t fin[2] = {0, 0};
+  FT_CUDA(c, cudaMemcpyAsync(fin, c->final_n, sizeof fin, cudaMemcpyDeviceToHost, c->stream));
+  std::vector<uint32_t> cnt(n_bands);
+  FT_CUDA(c, cudaMemcpyAsync(cnt.data(), c->sel.cnt, sizeof(uint32_t) * n_bands, cudaMemcpyDeviceToHost, c->stream));
+  static_assert(sizeof(ft_cand) == sizeof(FtCandDev), "ft_cand layout");
+  FT_CUDA(c, cudaMemcpyAsync(out_host, c->out_dev, sizeof(ft_cand) * (size_t)n_bands * k, cudaMemcpyDeviceToHost, c->stream));
+  FT_CUDA(c, cudaStreamSynchronize(c->stream));
+  uint64_t appended = 0;
+  for (uint32_t v : cnt) appended += v;
+  c->counters.appended = appended;
+  c->counters.refined = fin[0];
+  if (fin[1] != 0 || fin[0] > c->final_cap) {
+    char buf[200];
+    std::snprintf(buf, sizeof buf, "ft_topk_per_band: candidate buffers overflowed (%u attempts in one band / %u refined): too many exact ties at the k-th value", fin[1], fin[0]);
+    return fail(c, FT_ERR_STATE, buf);
+  }
+  return FT_OK;
+}
+
+int ft_eval_list(ft_ctx* c, const uint64_t* idx_host, int64_t n, ft_cand* out_host) {
+  if (!c || !idx_host || !out_host || n < 0) return FT_ERR_ARG;
+  if (!c->bound) return fail(c, FT_ERR_STATE, "ft_eval_list: no grid bound");
+  if (n == 0) return FT_OK;
+  const uint64_t n_templates = c->d.n_points * (uint64_t)c->d.n_f0;
+  for (int64_t i = 0; i < n; ++i)
+    if (idx_host[i] >= n_templates) return fail(c, FT_ERR_ARG, "ft_eval_list: index out of range");
+  uint64_t* idx_dev = nullptr;
+  FtCandDev* out_dev = nullptr;
+  FT_CUDA(c, cudaMalloc(&idx_dev, sizeof(uint64_t) * n));
+  cudaError_t e = cudaMalloc(&out_dev, sizeof(FtCandDev) * n);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(idx_dev, idx_host, sizeof(uint64_t) * n, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) e = ft_launch_refine(c->d, idx_dev, nullptr, n, out_dev, c->near_ties_dev, c->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out_host, out_dev, sizeof(ft_cand) * n, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(idx_dev);
+  cudaFree(out_dev);
+  c->counters.kernel_launches += 1;
+  if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_eval_list: ") + cudaGetErrorString(e));
+  return FT_OK;
+}
+
+int ft_get_counters(ft_ctx* c, ft_counters* out) {
+  if (!c || !out) return FT_ERR_ARG;
+  FT_CUDA(c, cudaStreamSynchronize(c->stream));
+  unsigned long long nt = 0;
+  FT_CUDA(c, cudaMemcpy(&nt, c->near_ties_dev, sizeof nt, cudaMemcpyDeviceToHost));
+  c->counters.near_ties = nt;
+  if (c->ev_valid) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->ev0, c->ev1) == cudaSuccess) c->counters.last_kernel_ms = ms;
+  }
+  *out = c->counters;
+  return FT_OK;
+}
+
+const char* ft_last_error(const ft_ctx* c) { return c ? c->err.c_str() : "null handle"; }
+
+void ft_destroy(ft_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  free_select(c);
+  ft_tile_plan_free(&c->plan);
+  dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->axes_dev);
+  dfree(c->scratch_f); dfree(c->scratch_i); dfree(c->near_ties_dev);
+  if (c->ev0) { cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1); }
+  delete c;
+}
+
+}  // extern "C"

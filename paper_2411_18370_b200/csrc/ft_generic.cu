@@ -1,0 +1,152 @@
+// Generic kernel K0 and the fp64 refinement kernel: the canonical track arithmetic evaluated per
+// (template, SFT), gather through L1/L2, fp64 accumulation in ascending SFT order (so the result
+// is the plain definition, Eq. (3) PAPER.md:64 / Eq. (7) :95, to the last bit).  K0 is the path for
+// grids the tile kernel does not take (df0 != df) and the reference the tile kernel is tested
+// against on the device; the refinement kernel re-evaluates the survivors of the fp32 selection.
+#include "ft_common.cuh"
+
+namespace {
+
+constexpr int K0_THREADS = 256;
+
+// CTA = one outer point x 256 consecutive f0.  Per chunk of 256 SFTs the CTA computes the
+// Doppler/binary factor D_alpha and f1*dt once (they do not depend on f0), then every thread walks
+// the chunk for its own f0 with the canonical x -> k -> gather.
+template <int STAT>
+__global__ void __launch_bounds__(K0_THREADS)
+ft_generic_kernel(const __grid_constant__ FtDev d, uint64_t pt_begin, uint32_t n_fblk,
+                  float* __restrict__ out_power, int32_t* __restrict__ out_count, uint64_t out_base) {
+  __shared__ double sD[K0_THREADS];
+  __shared__ double sF1dt[K0_THREADS];
+  __shared__ float sW[K0_THREADS];
+  const uint64_t pt = pt_begin + blockIdx.x / n_fblk;
+  const int64_t i_f0 = (int64_t)(blockIdx.x % n_fblk) * K0_THREADS + threadIdx.x;
+  const FtPoint p = ft_decode_point(d, pt);
+  const bool active = i_f0 < d.n_f0;
+  const double f0 = ft_f0(d, active ? i_f0 : 0);
+  double power = 0.0;
+  int32_t count = 0;
+  for (int64_t a0 = 0; a0 < d.n_sft; a0 += K0_THREADS) {
+    const int64_t a = a0 + threadIdx.x;
+    __syncthreads();
+    if (a < d.n_sft) {
+      const double t = d.t_mid[a];
+      sD[threadIdx.x] = ft_doppler(d, p, a, t);
+      sF1dt[threadIdx.x] = __dmul_rn(p.f1, __dsub_rn(t, d.t_ref));
+      sW[threadIdx.x] = (d.wkind == 1) ? d.w[a] : 0.f;
+    }
+    __syncthreads();
+    const int n = (int)min((int64_t)K0_THREADS, d.n_sft - a0);
+    if (active) {
+#pragma unroll 4
+      for (int c = 0; c < n; ++c) {
+        const double x = ft_track_x(f0, sF1dt[c], sD[c], d.f_min, d.inv_df);
+        const int64_t k = __double2ll_rn(x);
+        const int64_t off = (a0 + c) * d.ld + k;
+        const float pix = __ldg(d.P + off);
+        if (STAT != 1) {
+          const float w = (d.wkind == 1) ? sW[c] : __ldg(d.w + off);
+          power = fma((double)w, (double)pix, power);  // product exact in fp64 -> same as mul, add
+        }
+        if (STAT != 0) count += (pix > d.rho) ? 1 : 0;
+      }
+    }
+  }
+  if (active) {
+    const uint64_t o = pt * (uint64_t)d.n_f0 + (uint64_t)i_f0 - out_base;
+    if (STAT != 1 && out_power) out_power[o] = (float)power;
+    if (STAT != 0 && out_count) out_count[o] = count;
+  }
+}
+
+// One warp per candidate.  Lanes take 32 consecutive SFTs, then the 32 exact products are added
+// in ascending SFT order (every lane redundantly), so the sum has the oracle's rounding sequence.
+__global__ void __launch_bounds__(128)
+ft_refine_kernel(const __grid_constant__ FtDev d, const uint64_t* __restrict__ idx_list,
+                 const uint32_t* __restrict__ n_dev, int64_t n_max, FtCandDev* __restrict__ out,
+                 unsigned long long* __restrict__ near_ties) {
+  const int64_t n = n_dev ? min((int64_t)*n_dev, n_max) : n_max;
+  const int lane = threadIdx.x & 31;
+  const int64_t cand = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (cand >= n) return;
+  const uint64_t idx = idx_list[cand];
+  const uint64_t pt = idx / (uint64_t)d.n_f0;
+  const int64_t i_f0 = (int64_t)(idx % (uint64_t)d.n_f0);
+  const FtPoint p = ft_decode_point(d, pt);
+  const double f0 = ft_f0(d, i_f0);
+  double power = 0.0, wcount = 0.0;
+  int32_t count = 0;
+  unsigned ties = 0;
+  for (int64_t a0 = 0; a0 < d.n_sft; a0 += 32) {
+    const int64_t a = a0 + lane;
+    double prod = 0.0, wc = 0.0;
+    bool hit = false, tie = false;
+    if (a < d.n_sft) {
+      const double t = d.t_mid[a];
+      const double D = ft_doppler(d, p, a, t);
+      const double x = ft_track_x(f0, __dmul_rn(p.f1, __dsub_rn(t, d.t_ref)), D, d.f_min, d.inv_df);
+      tie = ft_near_tie(x);
+      const int64_t k = __double2ll_rn(x);
+      const int64_t off = a * d.ld + k;
+      const float pix = __ldg(d.P + off);
+      const float w = (d.wkind == 1) ? __ldg(d.w + a) : __ldg(d.w + off);
+      prod = __dmul_rn((double)w, (double)pix);
+      hit = pix > d.rho;
+      wc = hit ? (double)w : 0.0;
+    }
+    count += __popc(__ballot_sync(0xffffffffu, hit));
+    ties += __popc(__ballot_sync(0xffffffffu, tie));
+#pragma unroll
+    for (int l = 0; l < 32; ++l) {
+      power = __dadd_rn(power, __shfl_sync(0xffffffffu, prod, l));
+      wcount = __dadd_rn(wcount, __shfl_sync(0xffffffffu, wc, l));
+    }
+  }
+  if (lane == 0) {
+    FtCandDev c;
+    c.power = power; c.wcount = wcount; c.idx = idx; c.count = count; c.band = -1;
+    out[cand] = c;
+    if (ties && near_ties) atomicAdd(near_ties, (unsigned long long)ties);
+  }
+}
+
+__global__ void ft_fold_kernel(const float* __restrict__ P, const float* __restrict__ w,
+                               float* __restrict__ Q, int64_t n) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+    Q[i] = __fmul_rn(w[i], P[i]);
+}
+
+}  // namespace
+
+cudaError_t ft_launch_generic(const FtDev& d, int stat, uint64_t pt_begin, uint64_t pt_end,
+                              float* out_power, int32_t* out_count, uint64_t out_base_idx,
+                              cudaStream_t s) {
+  const uint32_t n_fblk = (uint32_t)((d.n_f0 + K0_THREADS - 1) / K0_THREADS);
+  uint64_t pt = pt_begin;
+  while (pt < pt_end) {  // grid.x is limited to 2^31-1 blocks
+    const uint64_t n_pt = (pt_end - pt < (uint64_t)(0x7fffffffu / n_fblk)) ? pt_end - pt : (uint64_t)(0x7fffffffu / n_fblk);
+    const dim3 grid((unsigned)(n_pt * n_fblk));
+    if (stat == 0) ft_generic_kernel<0><<<grid, K0_THREADS, 0, s>>>(d, pt, n_fblk, out_power, out_count, out_base_idx);
+    else if (stat == 1) ft_generic_kernel<1><<<grid, K0_THREADS, 0, s>>>(d, pt, n_fblk, out_power, out_count, out_base_idx);
+    else ft_generic_kernel<2><<<grid, K0_THREADS, 0, s>>>(d, pt, n_fblk, out_power, out_count, out_base_idx);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    pt += n_pt;
+  }
+  return cudaSuccess;
+}
+
+cudaError_t ft_launch_refine(const FtDev& d, const uint64_t* idx_dev, const uint32_t* n_dev, int64_t n_max,
+                             FtCandDev* out, unsigned long long* near_ties, cudaStream_t s) {
+  if (n_max <= 0) return cudaSuccess;
+  const int64_t warps_per_block = 4;
+  const unsigned grid = (unsigned)((n_max + warps_per_block - 1) / warps_per_block);
+  ft_refine_kernel<<<grid, 128, 0, s>>>(d, idx_dev, n_dev, n_max, out, near_ties);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_launch_fold(const float* P, const float* w, float* Q, int64_t n, cudaStream_t s) {
+  ft_fold_kernel<<<148 * 8, 256, 0, s>>>(P, w, Q, n);
+  return cudaGetLastError();
+}
