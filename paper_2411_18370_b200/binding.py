@@ -1,0 +1,162 @@
+"""Thin ctypes binding of libfasttracks_b200.so (include/fasttracks_b200.h): argument marshalling
+only.  Every step of the path runs in the library's CUDA kernels; there is no CPU fallback and
+this module never imports oracle/.  PyTorch supplies device memory and the stream."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+FT_STAT = {"power": 0, "hough": 1, "both": 2}
+FT_OPT_KERNEL, FT_OPT_FUSED_TOPK, FT_OPT_POINTS_PER_CTA = 0, 1, 2
+SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_eval_list", "ft_set_option",
+           "ft_get_counters", "ft_last_error", "ft_destroy"]
+
+
+class FtGrid(C.Structure):
+    _fields_ = [("f0_start", C.c_double), ("df0", C.c_double), ("n_f0", C.c_int64),
+                ("f1_start", C.c_double), ("df1", C.c_double), ("n_f1", C.c_int32),
+                ("t_ref", C.c_double),
+                ("n_sky", C.c_int64), ("sky", C.c_void_p),
+                ("n_ap", C.c_int32), ("a_p", C.c_void_p),
+                ("n_porb", C.c_int32), ("P_orb", C.c_void_p),
+                ("n_tasc", C.c_int32), ("tasc_frac", C.c_void_p)]
+
+
+class FtCand(C.Structure):
+    _fields_ = [("power", C.c_double), ("wcount", C.c_double), ("idx", C.c_uint64),
+                ("count", C.c_int32), ("band", C.c_int32)]
+
+
+CAND_DTYPE = np.dtype([("power", "<f8"), ("wcount", "<f8"), ("idx", "<u8"), ("count", "<i4"),
+                       ("band", "<i4")])
+
+
+class FtCounters(C.Structure):
+    _fields_ = [("near_ties", C.c_uint64), ("refine_fallbacks", C.c_uint64),
+                ("appended", C.c_uint64), ("refined", C.c_uint64),
+                ("kernel_launches", C.c_uint64), ("last_kernel_ms", C.c_double)]
+
+
+class FtError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"fasttracks_b200 error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path: str | None = None):
+    """dlopen the in-tree shared library (fails loudly if it was not built)."""
+    global _lib
+    if _lib is None:
+        path = path or _build.SO
+        if not os.path.exists(path):
+            raise FileNotFoundError(f"{path} missing: run `python -m paper_2411_18370_b200.build`")
+        lib = C.CDLL(path)
+        lib.ft_create.restype = C.c_int
+        lib.ft_create.argtypes = [C.POINTER(C.c_void_p), C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
+                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double,
+                                  C.c_double, C.c_void_p]
+        lib.ft_eval.restype = C.c_int
+        lib.ft_eval.argtypes = [C.c_void_p, C.POINTER(FtGrid), C.c_int, C.c_double, C.c_void_p, C.c_void_p]
+        lib.ft_topk_per_band.restype = C.c_int
+        lib.ft_topk_per_band.argtypes = [C.c_void_p, C.c_double, C.c_int32, C.c_void_p, C.POINTER(C.c_int32)]
+        lib.ft_eval_list.restype = C.c_int
+        lib.ft_eval_list.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+        lib.ft_set_option.restype = C.c_int
+        lib.ft_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
+        lib.ft_get_counters.restype = C.c_int
+        lib.ft_get_counters.argtypes = [C.c_void_p, C.POINTER(FtCounters)]
+        lib.ft_last_error.restype = C.c_char_p
+        lib.ft_last_error.argtypes = [C.c_void_p]
+        lib.ft_destroy.restype = None
+        lib.ft_destroy.argtypes = [C.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def _hp(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class Context:
+    """ft_create / ft_eval / ft_topk_per_band on torch device tensors."""
+
+    def __init__(self, P_dev, t_mid, vel, w, f_min, df, stream=None):
+        import torch
+        self.lib = load_library()
+        self.h = C.c_void_p()
+        assert P_dev.is_cuda and P_dev.dtype == torch.float32 and P_dev.dim() == 2 and P_dev.is_contiguous()
+        n_sft, ld = P_dev.shape
+        self.n_sft = n_sft
+        t_mid = np.ascontiguousarray(t_mid, dtype=np.float64)
+        vel = np.ascontiguousarray(vel, dtype=np.float64)
+        if isinstance(w, torch.Tensor):  # per-(SFT, bin) weights live on the device
+            assert w.is_cuda and w.dtype == torch.float32 and tuple(w.shape) == (n_sft, ld) and w.is_contiguous()
+            wptr, wkind = C.c_void_p(w.data_ptr()), 2
+        else:
+            w = np.ascontiguousarray(w, dtype=np.float32)
+            assert w.shape == (n_sft,)
+            wptr, wkind = _hp(w), 1
+        self._keep = (P_dev, w)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(P_dev.device)
+        rc = self.lib.ft_create(C.byref(self.h), C.c_void_p(P_dev.data_ptr()), n_sft, ld, ld, _hp(t_mid),
+                                _hp(vel), wptr, wkind, float(f_min), float(df),
+                                C.c_void_p(self.stream.cuda_stream))
+        self._check(rc)
+        self.n_templates = 0
+        self.k = 0
+
+    def _check(self, rc):
+        if rc != 0:
+            msg = self.lib.ft_last_error(self.h).decode() if self.h else "no handle"
+            raise FtError(rc, msg)
+
+    def set_option(self, option: int, value: int):
+        self._check(self.lib.ft_set_option(self.h, option, int(value)))
+
+    def eval(self, grid, stat: str, rho_th: float, out_power=None, out_count=None):
+        """grid: an object with the ft_grid fields (workloads.Grid).  out_*: torch device tensors or None."""
+        ax = [np.ascontiguousarray(a, dtype=np.float64) for a in (grid.sky, grid.a_p, grid.P_orb, grid.tasc_frac)]
+        g = FtGrid(float(grid.f0_start), float(grid.df0), int(grid.n_f0), float(grid.f1_start),
+                   float(grid.df1), int(grid.n_f1), float(grid.t_ref), len(ax[0]), _hp(ax[0]),
+                   len(ax[1]), _hp(ax[1]), len(ax[2]), _hp(ax[2]), len(ax[3]), _hp(ax[3]))
+        self.n_templates = len(ax[0]) * len(ax[1]) * len(ax[2]) * len(ax[3]) * int(grid.n_f1) * int(grid.n_f0)
+        for o in (out_power, out_count):
+            assert o is None or (o.is_cuda and o.numel() == self.n_templates and o.is_contiguous())
+        pp = C.c_void_p(out_power.data_ptr()) if out_power is not None else None
+        pc = C.c_void_p(out_count.data_ptr()) if out_count is not None else None
+        self._check(self.lib.ft_eval(self.h, C.byref(g), FT_STAT[stat], float(rho_th), pp, pc))
+
+    def topk_per_band(self, band_width_hz: float, k: int, n_bands_max: int):
+        out = np.zeros((n_bands_max, k), dtype=CAND_DTYPE)
+        nb = C.c_int32(0)
+        self._check(self.lib.ft_topk_per_band(self.h, float(band_width_hz), int(k), _hp(out), C.byref(nb)))
+        return out.reshape(-1)[: nb.value * k].reshape(nb.value, k)
+
+    def eval_list(self, idx):
+        idx = np.ascontiguousarray(idx, dtype=np.uint64)
+        out = np.zeros(idx.size, dtype=CAND_DTYPE)
+        self._check(self.lib.ft_eval_list(self.h, _hp(idx), idx.size, _hp(out)))
+        return out
+
+    def counters(self) -> dict:
+        c = FtCounters()
+        self._check(self.lib.ft_get_counters(self.h, C.byref(c)))
+        return {f: getattr(c, f) for f, _ in FtCounters._fields_}
+
+    def close(self):
+        if self.h:
+            self.lib.ft_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

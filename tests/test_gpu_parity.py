@@ -1,0 +1,124 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Bar (BASELINE.json north_star (4)): bins / counts bit-exact except templates
+within 1e-9 bin of a rounding tie; power sums to 1e-5 relative; top-k candidate sets identical."""
+import numpy as np
+import pytest
+
+from oracle import ft_oracle as fo
+from paper_2411_18370_b200 import workloads as W
+
+import ft_helpers as H
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [1, 0]  # 1 = generic kernel forced, 0 = auto (tile kernel when eligible)
+
+
+def _small(cfg):
+    """Reduced copies of BASELINE configs 2-4: several f0 tiles, ragged tails, oracle in seconds."""
+    if cfg == 1:
+        return W.config1()
+    if cfg == 2:
+        return W.config2(n_sft=501, n_sky=7, band_hz=0.35)          # 630 f0, ragged n_sft
+    if cfg == 3:
+        return W.config3(n_sft=403, n_ap=3, n_porb=3, n_tasc=2, n_inj=3)
+    if cfg == 4:
+        return W.config4(n_sft=300, n_sky=5, band_hz=0.4, n_lines=6)
+    raise ValueError(cfg)
+
+
+@pytest.fixture(scope="module", params=[1, 2, 3, 4])
+def case(request):
+    wl = H.apply_injections(_small(request.param))
+    o = fo.Oracle(wl)
+    power, count, wcount, tie = o.eval_range()
+    return wl, power, count, tie
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_full_arrays_match_oracle(case, kernel):
+    wl, o_power, o_count, o_tie = case
+    ctx = H.gpu_context(wl, kernel=kernel)
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    flagged = H.assert_full_parity(wl, gp, gc, o_power, o_count, o_tie)
+    assert flagged <= max(2, int(1e-6 * wl.n_evals))
+    # single-statistic launches give the same arrays
+    gp1, _ = H.gpu_full(ctx, wl, stat="power")
+    _, gc1 = H.gpu_full(ctx, wl, stat="hough")
+    assert np.array_equal(gp1, gp) and np.array_equal(gc1, gc)
+    ctx.close()
+
+
+@pytest.mark.parametrize("kernel,fused", [(1, 0), (0, 0), (0, 1)])
+def test_topk_sets_identical(case, kernel, fused):
+    wl, o_power, o_count, o_tie = case
+    bpb = int(round(wl.band_width / wl.grid.df0))
+    n_bands = -(-wl.grid.n_f0 // bpb)
+    ctx = H.gpu_context(wl, kernel=kernel, fused=fused)
+    ctx.eval(wl.grid, "both", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    H.assert_topk_parity(wl, cands, o_power, o_power, o_count, wl.k, bpb)
+    ctx.eval(wl.grid, "hough", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    H.assert_topk_parity(wl, cands, o_count, o_power, o_count, wl.k, bpb, by_count=True)
+    c = ctx.counters()
+    assert c["kernel_launches"] > 0 and c["refined"] >= 1
+    ctx.close()
+
+
+def test_eval_list_is_bit_identical(case):
+    wl, o_power, o_count, _ = case
+    rng = np.random.Generator(np.random.PCG64(5))
+    idx = rng.integers(0, wl.grid.n_templates, 257).astype(np.uint64)
+    ctx = H.gpu_context(wl)
+    ctx.eval(wl.grid, "both", wl.rho_th)
+    out = ctx.eval_list(idx)
+    op, oc, owc, _ = fo.Oracle(wl).eval_list(idx)
+    assert np.array_equal(out["power"], op) and np.array_equal(out["count"], oc)
+    assert np.array_equal(out["wcount"], owc) and np.array_equal(out["idx"], idx)
+    ctx.close()
+
+
+def test_injection_is_rank_one_on_config1():
+    wl = H.apply_injections(W.config1())
+    idx_t, amp = wl.planned_injections[0]
+    inj = int(wl.grid.ravel(*idx_t))
+    bpb = int(round(wl.band_width / wl.grid.df0))
+    ctx = H.gpu_context(wl)
+    ctx.eval(wl.grid, "both", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, 10)
+    assert cands.shape == (10, 5)
+    assert int(cands[idx_t[5] // bpb, 0]["idx"]) == inj
+    ctx.close()
+
+
+def test_errors_and_edge_cases():
+    from paper_2411_18370_b200 import binding as B
+    wl = W.config1()
+    ctx = H.gpu_context(wl)
+    g = wl.grid
+    # a grid whose tracks leave the spectrogram is rejected, not clamped (reading R9)
+    bad = W.Grid(f0_start=g.f0_start + 100 * wl.df, df0=g.df0, n_f0=g.n_f0, sky=g.sky)
+    with pytest.raises(B.FtError) as e:
+        ctx.eval(bad, "power", 1.6)
+    assert e.value.code == -4
+    with pytest.raises(B.FtError) as e:          # no grid bound after the failed eval
+        ctx.topk_per_band(0.01, 5, 10)
+    assert e.value.code == -6
+    ctx.eval(g, "power", 1.6)
+    with pytest.raises(B.FtError) as e:          # band width not an integer number of f0 steps
+        ctx.topk_per_band(0.0101, 5, 32)
+    assert e.value.code == -5
+    # k larger than a band's template count: padded with idx = UINT64_MAX
+    one = W.Grid(f0_start=g.f0_start, df0=g.df0, n_f0=7, sky=g.sky[:1])
+    ctx.eval(one, "power", 1.6)
+    c = ctx.topk_per_band(3 * g.df0, 5, 3)
+    assert c.shape == (3, 5)
+    assert [(c[b]["idx"] != np.uint64(2 ** 64 - 1)).sum() for b in range(3)] == [3, 3, 1]
+    # single template
+    one = W.Grid(f0_start=g.f0_start, df0=g.df0, n_f0=1, sky=g.sky[:1])
+    wl1 = W.Workload("one", 1, wl.P, wl.t_mid, wl.vel, wl.w, wl.f_min, wl.df, one, "both", 1.6, g.df0, 1, wl.T_sft)
+    gp, gc = H.gpu_full(ctx, wl1, stat="both")
+    op, oc, _, _ = fo.Oracle(wl1).eval_range()
+    assert gc[0] == oc[0] and abs(gp[0] - op[0]) <= 1e-5 * op[0]
+    ctx.close()
