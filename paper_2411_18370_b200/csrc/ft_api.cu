@@ -19,7 +19,9 @@ struct ft_ctx {
   double* t_mid_dev = nullptr;
   double* vel_dev = nullptr;
   float* w_dev = nullptr;       // per-SFT weights copy
-  float* Q_dev = nullptr;       // folded per-bin weights
+  float* Q_dev = nullptr;       // folded w*P (tile kernel input)
+  float* H_dev = nullptr;       // hit map (tile kernel input for the number count)
+  float H_rho = 0.f; bool H_valid = false;
   double* axes_dev = nullptr;   // sky | a_p | P_orb | tasc
   // host copies used for validation
   std::vector<double> t_mid, vel;
@@ -132,15 +134,35 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
              uint64_t out_base, bool filter, int32_t bpb) {
   const bool use_tile = c->tile_ok && c->opt_kernel != 1;
   if (use_tile) {
+    // one gather-reduce pass per statistic: power over Q = w*P, number count over the hit map
+    const FtSelectDev* sel = filter ? &c->sel : nullptr;
     int launches = 0;
-    FT_CUDA(c, ft_launch_tile(c->d, c->plan, stat, pt_begin, pt_end, out_power, out_count, out_base,
-                              filter ? &c->sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
-    c->counters.kernel_launches += launches;
+    if (stat != FT_STAT_HOUGH && (out_power || (filter && stat == FT_STAT_POWER))) {
+      FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.Q, pt_begin, pt_end, out_power, nullptr, out_base,
+                                stat == FT_STAT_POWER ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
+      c->counters.kernel_launches += launches;
+    }
+    if (stat != FT_STAT_POWER && (out_count || (filter && stat == FT_STAT_HOUGH))) {
+      FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.H, pt_begin, pt_end, nullptr, out_count, out_base,
+                                stat == FT_STAT_HOUGH ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
+      c->counters.kernel_launches += launches;
+    }
   } else {
     if (filter) return fail(c, FT_ERR_UNSUPPORTED, "fused filter needs the tile kernel");
     FT_CUDA(c, ft_launch_generic(c->d, stat, pt_begin, pt_end, out_power, out_count, out_base, c->stream));
     c->counters.kernel_launches += 1;
   }
+  return FT_OK;
+}
+
+// The tile kernel raises plan.err if a track left its staged strip (a planning bug, never data):
+// surfaced at the next synchronising call instead of silently wrong sums.
+int check_tile_err(ft_ctx* c) {
+  if (!c->plan.err) return FT_OK;
+  int32_t e = 0;
+  FT_CUDA(c, cudaMemcpy(&e, c->plan.err, sizeof e, cudaMemcpyDeviceToHost));
+  if (e != 0) return fail(c, FT_ERR_STATE, e == 1 ? "tile kernel: a track left its staged strip (internal planning error)"
+                                                  : "tile kernel: more than one break in a warp range (internal planning error)");
   return FT_OK;
 }
 
@@ -184,19 +206,20 @@ int ft_create(ft_ctx** out, const float* P_dev, int64_t n_sft, int64_t n_bins, i
   d.wkind = wkind; d.f_min = f_min; d.inv_df = 1.0 / df;
   c->df = df;
   c->per_bin = (wkind == FT_W_PER_SFT_BIN);
+  // fold Q = w*P once (one fp32 rounding per pixel; the fp64 refinement uses w and P unfolded)
+  FT_CUDA(c, cudaMalloc(&c->Q_dev, sizeof(float) * (size_t)n_sft * ld_bins));
   if (!c->per_bin) {
     FT_CUDA(c, cudaMalloc(&c->w_dev, sizeof(float) * n_sft));
     FT_CUDA(c, cudaMemcpyAsync(c->w_dev, w, sizeof(float) * n_sft, cudaMemcpyHostToDevice, c->stream));
-    d.w = c->w_dev; d.Q = nullptr;
+    d.w = c->w_dev;
+    FT_CUDA(c, ft_launch_fold_sft(P_dev, c->w_dev, c->Q_dev, n_sft, ld_bins, c->stream));
   } else {
     if (reinterpret_cast<uintptr_t>(w) & 15) return fail(c, FT_ERR_ARG, "ft_create: per-bin weights must be 16-byte aligned");
     d.w = w;
-    // fold Q = w*P once (one fp32 rounding per pixel; the fp64 refinement uses w and P unfolded)
-    FT_CUDA(c, cudaMalloc(&c->Q_dev, sizeof(float) * (size_t)n_sft * ld_bins));
     FT_CUDA(c, ft_launch_fold(P_dev, w, c->Q_dev, n_sft * ld_bins, c->stream));
-    c->counters.kernel_launches += 1;
-    d.Q = c->Q_dev;
   }
+  c->counters.kernel_launches += 1;
+  d.Q = c->Q_dev; d.H = nullptr;
   FT_CUDA(c, cudaStreamSynchronize(c->stream));  // host tables may be freed by the caller now
   return FT_OK;
 }
@@ -273,12 +296,20 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   if (c->opt_kernel != 1) {
     std::string why;
     int launches = 0;
-    const cudaError_t e = ft_tile_plan(d, c->df, eps, stat, (int)c->opt_ppc, c->stream, &c->plan, &why, &launches);
+    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc};
+    const cudaError_t e = ft_tile_plan(d, hin, c->stream, &c->plan, &why, &launches);
     c->counters.kernel_launches += launches;
     if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_tile_plan: ") + cudaGetErrorString(e));
     c->tile_ok = why.empty();
     if (!c->tile_ok && c->opt_kernel == 2) return fail(c, FT_ERR_UNSUPPORTED, "tile kernel not eligible: " + why);
   }
+  if (c->tile_ok && stat != FT_STAT_POWER && !(c->H_valid && c->H_rho == d.rho)) {
+    if (!c->H_dev) FT_CUDA(c, cudaMalloc(&c->H_dev, sizeof(float) * (size_t)d.n_sft * d.ld));
+    FT_CUDA(c, ft_launch_hitmap(d.P, d.rho, c->H_dev, d.n_sft * d.ld, c->stream));
+    c->counters.kernel_launches += 1;
+    c->H_rho = d.rho; c->H_valid = true;
+  }
+  d.H = c->H_dev;
   c->bound = true;
   if (out_power_dev || out_count_dev) {
     tick(c);
@@ -359,6 +390,7 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
   static_assert(sizeof(ft_cand) == sizeof(FtCandDev), "ft_cand layout");
   FT_CUDA(c, cudaMemcpyAsync(out_host, c->out_dev, sizeof(ft_cand) * (size_t)n_bands * k, cudaMemcpyDeviceToHost, c->stream));
   FT_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (int rc2 = check_tile_err(c)) return rc2;
   uint64_t appended = 0;
   for (uint32_t v : cnt) appended += v;
   c->counters.appended = appended;
@@ -396,6 +428,7 @@ int ft_eval_list(ft_ctx* c, const uint64_t* idx_host, int64_t n, ft_cand* out_ho
 int ft_get_counters(ft_ctx* c, ft_counters* out) {
   if (!c || !out) return FT_ERR_ARG;
   FT_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (int rc2 = check_tile_err(c)) return rc2;
   unsigned long long nt = 0;
   FT_CUDA(c, cudaMemcpy(&nt, c->near_ties_dev, sizeof nt, cudaMemcpyDeviceToHost));
   c->counters.near_ties = nt;
@@ -414,7 +447,7 @@ void ft_destroy(ft_ctx* c) {
   cudaStreamSynchronize(c->stream);
   free_select(c);
   ft_tile_plan_free(&c->plan);
-  dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->axes_dev);
+  dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->H_dev); dfree(c->axes_dev);
   dfree(c->scratch_f); dfree(c->scratch_i); dfree(c->near_ties_dev);
   if (c->ev0) { cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1); }
   delete c;

@@ -11,7 +11,8 @@
 struct FtDev {
   const float* P;       // [n_sft][ld]
   const float* w;       // per-SFT [n_sft] or per-bin [n_sft][ld]
-  const float* Q;       // folded w*P (per-bin weights only), [n_sft][ld]
+  const float* Q;       // folded w*P, one fp32 rounding per pixel, [n_sft][ld] (tile kernel input)
+  const float* H;       // hit map (P > rho) ? 1 : 0 as fp32, [n_sft][ld] (tile kernel input, number count)
   const double* t_mid;  // [n_sft]
   const double* vel;    // [n_sft][3]
   const double* sky;    // [n_sky][3]

@@ -1,9 +1,488 @@
+// Tile kernel K2: the hot path of the track statistics (PAPER.md:53 Eq. 2, :64 Eq. 3, :95 Eq. 7) for
+// product grids whose f0 step equals the spectrogram bin width (Eq. A1 :554, reading R14).
+//
+// One CTA = R outer points (everything of a template but f0) x one f0 tile.  A producer warp streams
+// the spectrogram rows of the tile, one contiguous strip per SFT, into a shared-memory ring with TMA
+// bulk copies (cp.async.bulk + mbarrier complete_tx); the strip bounds are point-independent and
+// come from the plan.  Each consumer warp owns ONE outer point and J consecutive 32-wide f0 chunks.
+// Per block of 32 SFTs every lane computes, for its own SFT, the canonical fp64 track at the first
+// and last f0 of the warp's range: along f0 the bin index is k_i = i + s with at most one break
+// (reading R6: x_i - i drifts by (D-1) per step and 32 J |D-1| < 1), so (s, break position) is the
+// whole track of the warp for that SFT.  The break is located with the canonical arithmetic itself
+// (estimate, verify, bisect), so bins are bit-identical to the plain definition except within 1e-9
+// bin of a rounding tie (counted).  The main loop is then, per SFT, one shuffle (the lane's packed
+// entry) and J x (LDS.32 + FADD): a gather from shared memory, fp32 accumulation in two levels
+// (32-SFT partial sums, then totals).  Weights are folded into the gathered array beforehand
+// (Q = w P, or the 0/1 hit map for the number count), so both statistics are the same kernel.
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
 #include "ft_tile.cuh"
-// placeholder until the tile kernel lands: never eligible
-cudaError_t ft_tile_plan(const FtDev&, double, double, int, int, cudaStream_t, FtTilePlan*, std::string* why, int* launches) {
-  *why = "tile kernel not built yet"; *launches = 0; return cudaSuccess;
+
+namespace {
+
+constexpr int kMaxPitch = 8191;  // packed entry: 13 bits of strip offset
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
-uint64_t ft_tile_sample_points(const FtTilePlan&, uint64_t n_points) { return n_points; }
-cudaError_t ft_launch_tile(const FtDev&, const FtTilePlan&, int, uint64_t, uint64_t, float*, int32_t*, uint64_t,
-                           const FtSelectDev*, int32_t, unsigned long long*, cudaStream_t, int*) { return cudaErrorNotSupported; }
-void ft_tile_plan_free(FtTilePlan* p) { if (p->kst) cudaFree(p->kst); if (p->vrange) cudaFree(p->vrange); *p = FtTilePlan{}; }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+struct FtTileArgs {
+  const float* A;
+  const int32_t* kst;
+  int32_t* err;
+  int32_t tile_w, n_tiles, R, wpp, pitch, copy_floats, rows_per_stage, n_stages;
+  uint64_t pt_begin, pt_end;
+  float* out_f;
+  int32_t* out_i;
+  uint64_t out_base;
+  FtSelectDev sel;
+  int32_t has_sel, bpb;
+  unsigned long long* near_ties;
+};
+
+// Packed per-(warp, SFT) track entry: bits 0-12 strip offset of the warp's first output (floats),
+// bits 13-23 break position relative to the warp's first output (0 = no break in the warp's range),
+// bit 24 set when the shift decreases at the break.  No break <=> entry < 8192.
+__device__ __forceinline__ uint32_t pack_entry(int off, int rel, bool neg) {
+  return (uint32_t)off | ((uint32_t)rel << 13) | (neg ? (1u << 24) : 0u);
+}
+
+template <int J>
+__global__ void __launch_bounds__(512, 1)
+ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileArgs a) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_cw = a.R * a.wpp;
+  const int tile = (int)(blockIdx.x % (unsigned)a.n_tiles);
+  const uint64_t group = blockIdx.x / (unsigned)a.n_tiles;
+  const int64_t n_sft = d.n_sft;
+  const int RPS = a.rows_per_stage, NS = a.n_stages;
+  float* ring = reinterpret_cast<float*>(smem_raw);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NS * RPS * a.pitch * sizeof(float));
+  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + NS);
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < NS; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, n_cw);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int32_t* kst = a.kst + (size_t)tile * n_sft;
+  const int64_t n_iters = (n_sft + RPS - 1) / RPS;
+
+  if (warp == n_cw) {
+    // ---- producer: one elected lane streams the strips (A3) ------------------------------------
+    if (lane == 0) {
+      const int64_t total = n_sft * d.ld;
+      for (int64_t it = 0; it < n_iters; ++it) {
+        const int s = (int)(it % NS);
+        const uint32_t ph = (uint32_t)((it / NS) & 1);
+        if (it >= NS) mbar_wait(empty0 + 8 * s, ph ^ 1u);
+        const int64_t a0 = it * RPS;
+        const int rows = (int)min((int64_t)RPS, n_sft - a0);
+        uint32_t bytes = 0;
+        for (int r = 0; r < rows; ++r) {
+          const int64_t src = (a0 + r) * d.ld + kst[a0 + r];
+          bytes += 4u * (uint32_t)min((int64_t)a.copy_floats, total - src);
+        }
+        mbar_expect_tx(full0 + 8 * s, bytes);
+        for (int r = 0; r < rows; ++r) {
+          const int64_t src = (a0 + r) * d.ld + kst[a0 + r];
+          const uint32_t nb = 4u * (uint32_t)min((int64_t)a.copy_floats, total - src);
+          bulk_g2s(smem_u32(ring + ((size_t)s * RPS + r) * a.pitch), a.A + src, nb, full0 + 8 * s);
+        }
+      }
+    }
+    return;
+  }
+  if (warp > n_cw) return;
+
+  // ---- consumers -------------------------------------------------------------------------------
+  const int r_pt = warp / a.wpp, sub = warp % a.wpp;
+  uint64_t pt = a.pt_begin + group * (uint64_t)a.R + (uint64_t)r_pt;
+  const bool pt_active = pt < a.pt_end;
+  if (!pt_active) pt = a.pt_end - 1;  // keep the barrier protocol; results are discarded
+  const FtPoint p = ft_decode_point(d, pt);
+  const int64_t tile_i0 = (int64_t)tile * a.tile_w;
+  const int wlo = sub * J * 32;                                    // warp's first output, tile-relative
+  const int64_t tile_n = min((int64_t)a.tile_w, d.n_f0 - tile_i0);  // valid f0 in this tile
+  const int warp_n = (int)max((int64_t)0, min((int64_t)(J * 32), tile_n - wlo));  // valid outputs of this warp
+  const int64_t i_first = tile_i0 + wlo;
+  const int64_t i_last = i_first + max(warp_n, 1) - 1;
+  float acc[J], tot[J];
+#pragma unroll
+  for (int j = 0; j < J; ++j) { acc[j] = 0.f; tot[j] = 0.f; }
+  unsigned ties = 0;
+  const uint32_t lane_bytes = smem_u32(ring) + 4u * (uint32_t)lane;
+  const uint32_t row_bytes = 4u * (uint32_t)a.pitch;
+
+  for (int64_t a0 = 0; a0 < n_sft; a0 += 32) {
+    // -- A1/A2: this lane's SFT: canonical track at both ends of the warp's f0 range ---------------
+    uint32_t entry = 0;
+    {
+      const int64_t al = a0 + lane;
+      if (al < n_sft && warp_n > 0) {
+        const double t = d.t_mid[al];
+        const double D = ft_doppler(d, p, al, t);
+        const double f1dt = __dmul_rn(p.f1, __dsub_rn(t, d.t_ref));
+        const double xa = ft_track_x(ft_f0(d, i_first), f1dt, D, d.f_min, d.inv_df);
+        const double xb = ft_track_x(ft_f0(d, i_last), f1dt, D, d.f_min, d.inv_df);
+        ties += (ft_near_tie(xa) ? 1u : 0u) + (ft_near_tie(xb) ? 1u : 0u);
+        const int64_t ka = __double2ll_rn(xa), kb = __double2ll_rn(xb);
+        const int64_t s = ka - i_first, sb = kb - i_last;
+        const int64_t off = ka - (int64_t)kst[al];  // strip index of the warp's first output
+        int rel = 0;
+        bool neg = false;
+        if (sb != s) {
+          neg = sb < s;
+          // smallest i in (i_first, i_last] with rint(x_i) - i != s
+          int64_t lo = i_first, hi = i_last;
+          const double frac = xa - (double)ka;
+          const double slope = fabs(D - 1.0);
+          double nest = ceil((0.5 - (neg ? -frac : frac)) / fmax(slope, 1e-300));
+          nest = fmin(fmax(nest, 1.0), (double)(i_last - i_first));
+          auto pred = [&](int64_t i) {
+            const double x = ft_track_x(ft_f0(d, i), f1dt, D, d.f_min, d.inv_df);
+            ties += ft_near_tie(x) ? 1u : 0u;
+            return (__double2ll_rn(x) - i) != s;
+          };
+          const int64_t cand = i_first + (int64_t)nest;
+          if (pred(cand)) {
+            hi = cand;
+            if (cand - 1 > lo) { if (!pred(cand - 1)) lo = cand - 1; else hi = cand - 1; }
+          } else {
+            lo = cand;
+            if (cand + 1 < hi) { if (pred(cand + 1)) hi = cand + 1; else lo = cand + 1; }
+          }
+          while (hi - lo > 1) {
+            const int64_t mid = (lo + hi) >> 1;
+            if (pred(mid)) hi = mid; else lo = mid;
+          }
+          rel = (int)(hi - i_first);
+          if (sb - s > 1 || s - sb > 1) atomicExch(a.err, 2);
+        }
+        // every pixel read for a valid output must lie inside the copied strip (else: plan bug)
+        const int64_t hi_idx = off + (warp_n - 1) + ((rel && !neg) ? 1 : 0);
+        if (off < 0 || off > kMaxPitch || hi_idx >= a.copy_floats) {
+          atomicExch(a.err, 1);
+        } else {
+          entry = pack_entry((int)off, rel, neg);
+        }
+      }
+    }
+    // -- A4: gather + reduce over the block's SFTs -----------------------------------------------
+    const int n_rows = (int)min((int64_t)32, n_sft - a0);
+    for (int q = 0; q < n_rows; q += RPS) {
+      const int64_t it = (a0 + q) / RPS;
+      const int s = (int)(it % NS);
+      mbar_wait(full0 + 8 * s, (uint32_t)((it / NS) & 1));
+      const int rows = min(RPS, n_rows - q);
+      const uint32_t stage_bytes = lane_bytes + (uint32_t)(s * RPS) * row_bytes;
+      for (int r = 0; r < rows; ++r) {
+        const uint32_t e = __shfl_sync(0xffffffffu, entry, q + r);
+        const uint32_t base = stage_bytes + (uint32_t)r * row_bytes;
+        if (e < 8192u) {  // no break inside this warp's range: J conflict-free LDS.32 + FADD
+          const uint32_t ad = base + 4u * e;
+          float v[J];
+#pragma unroll
+          for (int j = 0; j < J; ++j)
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v[j]) : "r"(ad + 128u * j));
+#pragma unroll
+          for (int j = 0; j < J; ++j) acc[j] += v[j];
+        } else {
+          const uint32_t off = e & 8191u;
+          const int rel = (int)((e >> 13) & 2047u);
+          const uint32_t ad_lo = base + 4u * off;
+          const uint32_t ad_hi = (e & (1u << 24)) ? ad_lo - 4u : ad_lo + 4u;
+          const int t_lane = rel - lane;
+#pragma unroll
+          for (int j = 0; j < J; ++j) {
+            const uint32_t ad = ((32 * j >= t_lane) ? ad_hi : ad_lo) + 128u * j;
+            float v;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(ad));
+            acc[j] += v;
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty0 + 8 * s);
+    }
+#pragma unroll
+    for (int j = 0; j < J; ++j) { tot[j] += acc[j]; acc[j] = 0.f; }
+  }
+
+  // ---- A5/A6: epilogue ---------------------------------------------------------------------------
+  if (ties && a.near_ties) {
+    for (int o = 16; o > 0; o >>= 1) ties += __shfl_xor_sync(0xffffffffu, ties, o);
+    if (lane == 0 && pt_active) atomicAdd(a.near_ties, (unsigned long long)ties);
+  }
+  if (!pt_active) return;
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+    const int ii = 32 * j + lane;
+    if (ii < warp_n) {
+      const int64_t i = i_first + ii;
+      const uint64_t idx = pt * (uint64_t)d.n_f0 + (uint64_t)i;
+      const float v = tot[j];
+      if (a.out_f) a.out_f[idx - a.out_base] = v;
+      if (a.out_i) a.out_i[idx - a.out_base] = __float2int_rn(v);
+      if (a.has_sel) {
+        const int band = (int)(i / a.bpb);
+        if (v >= __ldg(a.sel.thr + band)) ft_select_append(a.sel, band, v, idx);
+      }
+    }
+  }
+}
+
+// min / max over the sky axis of v_alpha . n / c, per SFT (for the point-independent strip bounds)
+__global__ void __launch_bounds__(256)
+ft_vrange_kernel(const double* __restrict__ vel, const double* __restrict__ sky, int64_t n_sky,
+                 double* __restrict__ vrange) {
+  __shared__ double smin[256], smax[256];
+  const int64_t a = blockIdx.x;
+  const double vx = vel[3 * a], vy = vel[3 * a + 1], vz = vel[3 * a + 2];
+  double lo = INFINITY, hi = -INFINITY;
+  for (int64_t i = threadIdx.x; i < n_sky; i += blockDim.x) {
+    const double v = (vx * sky[3 * i] + vy * sky[3 * i + 1] + vz * sky[3 * i + 2]) / FT_C_LIGHT;
+    lo = fmin(lo, v); hi = fmax(hi, v);
+  }
+  smin[threadIdx.x] = lo; smax[threadIdx.x] = hi;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) {
+      smin[threadIdx.x] = fmin(smin[threadIdx.x], smin[threadIdx.x + o]);
+      smax[threadIdx.x] = fmax(smax[threadIdx.x], smax[threadIdx.x + o]);
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { vrange[2 * a] = smin[0]; vrange[2 * a + 1] = smax[0]; }
+}
+
+__global__ void ft_hitmap_kernel(const float* __restrict__ P, float rho, float* __restrict__ H, int64_t n) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+    H[i] = (P[i] > rho) ? 1.f : 0.f;
+}
+
+__global__ void ft_fold_sft_kernel(const float* __restrict__ P, const float* __restrict__ w,
+                                   float* __restrict__ Q, int64_t n_sft, int64_t ld) {
+  const int64_t n = n_sft * ld, stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+    Q[i] = __fmul_rn(w[i / ld], P[i]);
+}
+
+// J values the kernel is instantiated for (the plan rounds the per-warp chunk count up to one)
+constexpr int kJList[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 15, 16, 20, 24, 28, 29, 30, 32};
+
+template <int J>
+cudaError_t launch_J(const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s) {
+  static bool configured = false;  // one attribute call per instantiation and process
+  if (!configured) {
+    const cudaError_t e = cudaFuncSetAttribute(ft_tile_kernel<J>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  ft_tile_kernel<J><<<grid, block, smem, s>>>(d, a);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_any(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s) {
+  switch (J) {
+#define FT_CASE(j) case j: return launch_J<j>(d, a, grid, block, smem, s);
+    FT_CASE(1) FT_CASE(2) FT_CASE(3) FT_CASE(4) FT_CASE(5) FT_CASE(6) FT_CASE(7) FT_CASE(8) FT_CASE(10)
+    FT_CASE(12) FT_CASE(15) FT_CASE(16) FT_CASE(20) FT_CASE(24) FT_CASE(28) FT_CASE(29) FT_CASE(30) FT_CASE(32)
+#undef FT_CASE
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace
+
+void ft_tile_plan_free(FtTilePlan* p) {
+  if (p->kst) cudaFree(p->kst);
+  if (p->err) cudaFree(p->err);
+  *p = FtTilePlan{};
+}
+
+cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s, FtTilePlan* plan,
+                         std::string* why, int* launches) {
+  *launches = 0;
+  why->clear();
+  ft_tile_plan_free(plan);
+  if (d.df0 != in.df && d.n_f0 > 1) { *why = "f0 step differs from the bin width"; return cudaSuccess; }
+  if (!d.Q) { *why = "no folded array"; return cudaSuccess; }
+  const int64_t n_sft = d.n_sft;
+  // --- tiling: n_tiles x wpp warps x J chunks of 32 f0, least issue slots (J+1.5 per chunk row) -----
+  const int64_t chunks = (d.n_f0 + 31) / 32;
+  double best = 1e300;
+  int bJ = 0, bW = 0; int64_t bT = 0;
+  const int maxJ_eps = (int)std::floor(0.45 / (32.0 * std::fmax(in.eps_bound, 1e-12)));
+  for (int64_t nt = 1; nt <= chunks; ++nt) {
+    const int64_t cpt = (chunks + nt - 1) / nt;
+    if (nt > 1 && (chunks + nt - 2) / (nt - 1) == cpt) continue;  // same tile size as nt-1
+    for (int wpp = 1; wpp <= 4; ++wpp) {
+      const int64_t Jn = (cpt + wpp - 1) / wpp;
+      if (Jn > 32) continue;
+      int J = 0;
+      for (int c : kJList) if (c >= Jn) { J = c; break; }
+      if (J == 0 || J > maxJ_eps) continue;
+      const double cost = (double)nt * wpp * (J + 1.5) * (1.0 + 0.02 * (double)(nt - 1));
+      if (cost < best) { best = cost; bJ = J; bW = wpp; bT = nt; }
+    }
+    if (cpt == 1) break;
+  }
+  if (bJ == 0) { *why = "Doppler spread too large for a single break per warp range"; return cudaSuccess; }
+  FtTilePlan pl;
+  pl.J = bJ; pl.wpp = bW;
+  pl.tile_w = (int32_t)(((chunks + bT - 1) / bT) * 32);
+  pl.n_tiles = (int32_t)((d.n_f0 + pl.tile_w - 1) / pl.tile_w);
+  int R = in.points_per_cta > 0 ? in.points_per_cta : 8;
+  R = std::min<int>(R, 15 / pl.wpp);  // 15 consumer warps + 1 producer = 512 threads (128 registers)
+  R = (int)std::min<uint64_t>((uint64_t)R, d.n_points);
+  pl.R = std::max(R, 1);
+  // --- point-independent strip bounds per (tile, SFT) -----------------------------------------------
+  double* vr_dev = nullptr;
+  cudaError_t e = cudaMalloc(&vr_dev, sizeof(double) * 2 * n_sft);
+  if (e != cudaSuccess) return e;
+  ft_vrange_kernel<<<(unsigned)n_sft, 256, 0, s>>>(d.vel, d.sky, d.n_sky, vr_dev);
+  *launches += 1;
+  std::vector<double> vr(2 * (size_t)n_sft);
+  e = cudaMemcpyAsync(vr.data(), vr_dev, sizeof(double) * 2 * n_sft, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  cudaFree(vr_dev);
+  if (e != cudaSuccess) return e;
+  double bmax = 0.0;
+  {
+    double apm = 0.0, pmin = in.P_orb[0];
+    for (int i = 0; i < d.n_ap; ++i) apm = std::fmax(apm, std::fabs(in.a_p[i]));
+    for (int i = 0; i < d.n_porb; ++i) pmin = std::fmin(pmin, in.P_orb[i]);
+    bmax = apm * FT_TWO_PI / pmin;
+  }
+  const double f1a = d.f1_start, f1b = d.f1_start + (double)(d.n_f1 - 1) * d.df1;
+  std::vector<int32_t> kst((size_t)pl.n_tiles * n_sft);
+  int64_t max_w = 0;
+  for (int t = 0; t < pl.n_tiles; ++t) {
+    const int64_t i_lo = (int64_t)t * pl.tile_w, i_hi = std::min<int64_t>(d.n_f0, i_lo + pl.tile_w) - 1;
+    const double f0_lo = d.f0_start + (double)i_lo * d.df0, f0_hi = d.f0_start + (double)i_hi * d.df0;
+    for (int64_t a = 0; a < n_sft; ++a) {
+      const double dt = in.t_mid[a] - d.t_ref;
+      const double g_lo = std::fmin(f1a * dt, f1b * dt), g_hi = std::fmax(f1a * dt, f1b * dt);
+      const double D_lo = 1.0 + vr[2 * a] - bmax, D_hi = 1.0 + vr[2 * a + 1] + bmax;
+      const double x_lo = ((f0_lo + g_lo) * D_lo - d.f_min) * d.inv_df;
+      const double x_hi = ((f0_hi + g_hi) * D_hi - d.f_min) * d.inv_df;
+      int64_t lo = (int64_t)std::floor(x_lo) - 1, hi = (int64_t)std::ceil(x_hi) + 1;
+      lo = std::max<int64_t>(lo, 0);
+      hi = std::min<int64_t>(hi, d.n_bins - 1);
+      const int64_t k0 = lo / 4 * 4;
+      kst[(size_t)t * n_sft + a] = (int32_t)k0;
+      max_w = std::max(max_w, hi - k0 + 1);
+    }
+  }
+  pl.copy_floats = (int32_t)((max_w + 3) / 4 * 4);
+  int min_warp_n = 32 * pl.J;
+  for (int t = 0; t < pl.n_tiles; ++t) {
+    const int64_t tile_n = std::min<int64_t>(pl.tile_w, d.n_f0 - (int64_t)t * pl.tile_w);
+    for (int sub = 0; sub < pl.wpp; ++sub) {
+      const int64_t wn = std::min<int64_t>(32 * pl.J, tile_n - (int64_t)sub * pl.J * 32);
+      if (wn > 0) min_warp_n = (int)std::min<int64_t>(min_warp_n, wn);
+    }
+  }
+  pl.pitch = (pl.copy_floats + 32 * pl.J - min_warp_n + 2 + 3) / 4 * 4;
+  pl.pitch = std::max(pl.pitch, 32 * pl.J + 4);  // warps without valid outputs read [0, 32 J)
+  if (pl.copy_floats > kMaxPitch + 1) { *why = "strip too wide for the packed track entry"; return cudaSuccess; }
+  // --- shared-memory ring ---------------------------------------------------------------------------
+  const int threads = (pl.R * pl.wpp + 1) * 32;
+  const int regs_est = 3 * pl.J + 34;
+  int ctas = std::min(4, std::min(2048 / threads, 65536 / (threads * regs_est)));
+  ctas = std::max(ctas, 1);
+  const size_t row_bytes = (size_t)pl.pitch * 4;
+  const size_t budget = (size_t)(228 * 1024) / ctas - 2048;
+  int64_t rows_fit = (int64_t)((budget - 1024) / row_bytes);
+  if (rows_fit < 2) { *why = "strip does not fit shared memory twice"; return cudaSuccess; }
+  rows_fit = std::min<int64_t>(rows_fit, 32);
+  pl.rows_per_stage = rows_fit >= 12 ? 4 : (rows_fit >= 6 ? 2 : 1);
+  pl.n_stages = (int32_t)(rows_fit / pl.rows_per_stage);
+  pl.ctas_per_sm = ctas;
+  pl.smem_bytes = (size_t)pl.n_stages * pl.rows_per_stage * row_bytes + 2 * 8 * (size_t)pl.n_stages;
+  e = cudaMalloc(&pl.kst, sizeof(int32_t) * kst.size());
+  if (e != cudaSuccess) return e;
+  e = cudaMalloc(&pl.err, sizeof(int32_t));
+  if (e == cudaSuccess) e = cudaMemcpyAsync(pl.kst, kst.data(), sizeof(int32_t) * kst.size(), cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(pl.err, 0, sizeof(int32_t), s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);  // kst (host vector) goes out of scope
+  if (e != cudaSuccess) { ft_tile_plan_free(&pl); return e; }
+  *plan = pl;
+  return cudaSuccess;
+}
+
+uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points) {
+  uint64_t s = std::max<uint64_t>(n_points / 64, (uint64_t)plan.R * 296);
+  s = (s + plan.R - 1) / plan.R * plan.R;
+  return std::min(s, n_points);
+}
+
+cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, uint64_t pt_begin,
+                           uint64_t pt_end, float* out_f, int32_t* out_i, uint64_t out_base,
+                           const FtSelectDev* sel, int32_t bpb, unsigned long long* near_ties,
+                           cudaStream_t s, int* launches) {
+  *launches = 0;
+  if (pt_end <= pt_begin) return cudaSuccess;
+  FtTileArgs a{};
+  a.A = A; a.kst = plan.kst; a.err = plan.err;
+  a.tile_w = plan.tile_w; a.n_tiles = plan.n_tiles; a.R = plan.R; a.wpp = plan.wpp;
+  a.pitch = plan.pitch; a.copy_floats = plan.copy_floats;
+  a.rows_per_stage = plan.rows_per_stage; a.n_stages = plan.n_stages;
+  a.out_f = out_f; a.out_i = out_i; a.out_base = out_base;
+  if (sel) { a.sel = *sel; a.has_sel = 1; }
+  a.bpb = bpb > 0 ? bpb : 1;
+  a.near_ties = near_ties;
+  const unsigned block = (unsigned)((plan.R * plan.wpp + 1) * 32);
+  const uint64_t max_groups = 0x7fffffffull / (uint64_t)plan.n_tiles;
+  uint64_t pt = pt_begin;
+  while (pt < pt_end) {
+    uint64_t groups = (pt_end - pt + plan.R - 1) / plan.R;
+    if (groups > max_groups) groups = max_groups;
+    a.pt_begin = pt;
+    a.pt_end = std::min<uint64_t>(pt_end, pt + groups * plan.R);
+    const cudaError_t e = launch_any(plan.J, d, a, (unsigned)(groups * plan.n_tiles), block, plan.smem_bytes, s);
+    if (e != cudaSuccess) return e;
+    *launches += 1;
+    pt = a.pt_end;
+  }
+  return cudaSuccess;
+}
+
+cudaError_t ft_launch_hitmap(const float* P, float rho, float* H, int64_t n, cudaStream_t s) {
+  ft_hitmap_kernel<<<148 * 8, 256, 0, s>>>(P, rho, H, n);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_launch_fold_sft(const float* P, const float* w_sft, float* Q, int64_t n_sft, int64_t ld, cudaStream_t s) {
+  ft_fold_sft_kernel<<<148 * 8, 256, 0, s>>>(P, w_sft, Q, n_sft, ld);
+  return cudaGetLastError();
+}

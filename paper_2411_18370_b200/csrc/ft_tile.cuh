@@ -1,4 +1,4 @@
-// Tile kernel K2 (ft_tile.cu): host-side plan and launchers.
+// Tile kernel K2 (ft_tile.cu): host-side plan and launchers.  DESIGN.md "Kernel K2".
 #pragma once
 #include <string>
 
@@ -6,28 +6,39 @@
 #include "ft_select.cuh"
 
 struct FtTilePlan {
-  int32_t* kst = nullptr;     // [n_tiles][n_sft] first staged bin of the strip (multiple of 4)
-  double* vrange = nullptr;   // [n_sft][2] min / max of v.n/c over the sky axis
-  int32_t n_tiles = 0;        // f0 tiles
-  int32_t tile_w = 0;         // f0 per tile
-  int32_t pitch = 0;          // floats per staged row
-  int32_t points_per_cta = 0; // R
-  int32_t j_per_thread = 0;   // J
-  int32_t rows_per_stage = 0; // C
+  int32_t* kst = nullptr;       // device [n_tiles][n_sft] first staged bin of the strip (multiple of 4)
+  int32_t* err = nullptr;       // device [1] set by the kernel if a track left its staged strip (plan bug)
+  int32_t n_tiles = 0;          // f0 tiles
+  int32_t tile_w = 0;           // f0 per tile (multiple of 32; the last tile may hold fewer)
+  int32_t J = 0;                // 32-wide f0 chunks per consumer warp (template parameter)
+  int32_t wpp = 0;              // consumer warps per outer point
+  int32_t R = 0;                // outer points per CTA
+  int32_t pitch = 0;            // floats per staged row in shared memory
+  int32_t copy_floats = 0;      // floats copied per row (multiple of 4, <= pitch)
+  int32_t rows_per_stage = 0;   // divides 32
   int32_t n_stages = 0;
-  int32_t n_consumer_warps = 0;
-  int32_t n_producer_warps = 0;
-  int32_t variant = -1;
+  int32_t ctas_per_sm = 0;
   size_t smem_bytes = 0;
-  int64_t n_sft_alloc = 0;
 };
 
 // Decide eligibility (why->empty() == eligible) and build the per-(tile, SFT) strip table.
-cudaError_t ft_tile_plan(const FtDev& d, double df, double eps_bound, int stat, int points_per_cta,
-                         cudaStream_t s, FtTilePlan* plan, std::string* why, int* launches);
+// `t_mid` / `vel` are the host copies of the per-SFT tables; `sky_host` etc. the grid axes.
+struct FtTileHostIn {
+  const double* t_mid; const double* vel;   // [n_sft], [n_sft][3]
+  const double* sky; const double* a_p; const double* P_orb;
+  double df; double eps_bound;
+  int points_per_cta;
+};
+cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s, FtTilePlan* plan,
+                         std::string* why, int* launches);
 uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points);
-cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, int stat, uint64_t pt_begin,
-                           uint64_t pt_end, float* out_power, int32_t* out_count, uint64_t out_base,
+// One pass of the gather-reduce over array A (folded w*P for the power statistic, the 0/1 hit map
+// for the number count).  Writes out_f (fp32) and/or out_i (int32) indexed from out_base, and/or
+// filters into sel (bands of bpb f0 bins).
+cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, uint64_t pt_begin,
+                           uint64_t pt_end, float* out_f, int32_t* out_i, uint64_t out_base,
                            const FtSelectDev* sel, int32_t bpb, unsigned long long* near_ties,
                            cudaStream_t s, int* launches);
+cudaError_t ft_launch_hitmap(const float* P, float rho, float* H, int64_t n, cudaStream_t s);
+cudaError_t ft_launch_fold_sft(const float* P, const float* w_sft, float* Q, int64_t n_sft, int64_t ld, cudaStream_t s);
 void ft_tile_plan_free(FtTilePlan* plan);
