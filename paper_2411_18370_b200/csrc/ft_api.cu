@@ -22,6 +22,7 @@ struct ft_ctx {
   float* Q_dev = nullptr;       // folded w*P (tile kernel input)
   float* H_dev = nullptr;       // hit map (tile kernel input for the number count)
   float H_rho = 0.f; bool H_valid = false;
+  double add_back = 0.0;        // sum over SFTs of the per-row constant the fold removed from Q
   double* axes_dev = nullptr;   // sky | a_p | P_orb | tasc
   // host copies used for validation
   std::vector<double> t_mid, vel;
@@ -138,12 +139,12 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
     const FtSelectDev* sel = filter ? &c->sel : nullptr;
     int launches = 0;
     if (stat != FT_STAT_HOUGH && (out_power || (filter && stat == FT_STAT_POWER))) {
-      FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.Q, pt_begin, pt_end, out_power, nullptr, out_base,
+      FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.Q, c->add_back, pt_begin, pt_end, out_power, nullptr, out_base,
                                 stat == FT_STAT_POWER ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
       c->counters.kernel_launches += launches;
     }
     if (stat != FT_STAT_POWER && (out_count || (filter && stat == FT_STAT_HOUGH))) {
-      FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.H, pt_begin, pt_end, nullptr, out_count, out_base,
+      FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.H, 0.0, pt_begin, pt_end, nullptr, out_count, out_base,
                                 stat == FT_STAT_HOUGH ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
       c->counters.kernel_launches += launches;
     }
@@ -206,17 +207,28 @@ int ft_create(ft_ctx** out, const float* P_dev, int64_t n_sft, int64_t n_bins, i
   d.wkind = wkind; d.f_min = f_min; d.inv_df = 1.0 / df;
   c->df = df;
   c->per_bin = (wkind == FT_W_PER_SFT_BIN);
-  // fold Q = w*P once (one fp32 rounding per pixel; the fp64 refinement uses w and P unfolded)
+  // A0: Q = fl(fl(w P) - c_row) (the fp64 refinement uses w and P unfolded); add_back = sum c_row
   FT_CUDA(c, cudaMalloc(&c->Q_dev, sizeof(float) * (size_t)n_sft * ld_bins));
+  float* c_row_dev = nullptr;
+  FT_CUDA(c, cudaMalloc(&c_row_dev, sizeof(float) * n_sft));
   if (!c->per_bin) {
     FT_CUDA(c, cudaMalloc(&c->w_dev, sizeof(float) * n_sft));
     FT_CUDA(c, cudaMemcpyAsync(c->w_dev, w, sizeof(float) * n_sft, cudaMemcpyHostToDevice, c->stream));
     d.w = c->w_dev;
-    FT_CUDA(c, ft_launch_fold_sft(P_dev, c->w_dev, c->Q_dev, n_sft, ld_bins, c->stream));
   } else {
-    if (reinterpret_cast<uintptr_t>(w) & 15) return fail(c, FT_ERR_ARG, "ft_create: per-bin weights must be 16-byte aligned");
+    if (reinterpret_cast<uintptr_t>(w) & 15) { cudaFree(c_row_dev); return fail(c, FT_ERR_ARG, "ft_create: per-bin weights must be 16-byte aligned"); }
     d.w = w;
-    FT_CUDA(c, ft_launch_fold(P_dev, w, c->Q_dev, n_sft * ld_bins, c->stream));
+  }
+  {
+    cudaError_t e = ft_launch_fold_centered(P_dev, c->per_bin ? nullptr : c->w_dev, c->per_bin ? w : nullptr,
+                                            c->Q_dev, c_row_dev, n_sft, n_bins, ld_bins, c->stream);
+    std::vector<float> c_row((size_t)n_sft);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c_row.data(), c_row_dev, sizeof(float) * n_sft, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(c_row_dev);
+    if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_create: fold: ") + cudaGetErrorString(e));
+    c->add_back = 0.0;
+    for (float v : c_row) c->add_back += (double)v;
   }
   c->counters.kernel_launches += 1;
   d.Q = c->Q_dev; d.H = nullptr;

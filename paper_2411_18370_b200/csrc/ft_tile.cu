@@ -50,12 +50,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
+constexpr int kRPS = 4;  // spectrogram rows per ring stage (divides 32)
+
 struct FtTileArgs {
   const float* A;
   const int32_t* kst;
   int32_t* err;
-  int32_t tile_w, n_tiles, R, wpp, pitch, copy_floats, rows_per_stage, n_stages;
+  int32_t tile_w, n_tiles, R, wpp, pitch, copy_floats, n_stages;
   uint64_t pt_begin, pt_end;
+  double add_back;  // sum over SFTs of the per-row constant removed from A at fold time
   float* out_f;
   int32_t* out_i;
   uint64_t out_base;
@@ -64,6 +67,10 @@ struct FtTileArgs {
   unsigned long long* near_ties;
 };
 
+// Threads per CTA the kernel is compiled for: (consumer warps + 1 producer warp) * 32.  The
+// accumulators (J) and the loads in flight (J) set the register need, hence the bound.
+__host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 1024 : 768; }
+
 // Packed per-(warp, SFT) track entry: bits 0-12 strip offset of the warp's first output (floats),
 // bits 13-23 break position relative to the warp's first output (0 = no break in the warp's range),
 // bit 24 set when the shift decreases at the break.  No break <=> entry < 8192.
@@ -71,18 +78,72 @@ __device__ __forceinline__ uint32_t pack_entry(int off, int rel, bool neg) {
   return (uint32_t)off | ((uint32_t)rel << 13) | (neg ? (1u << 24) : 0u);
 }
 
+// A1 + A2 for one (outer point, SFT, warp range): canonical track at the first and last f0 of the
+// range, and, if the two shifts differ, the canonical position of the single break.
+__device__ __forceinline__ uint32_t ft_tile_entry(const FtDev& d, const FtPoint& p, int al, int kst_al,
+                                               int i_first, int warp_n, int copy_floats,
+                                               unsigned* ties, int32_t* err) {
+  const double t = d.t_mid[al];
+  const double D = ft_doppler(d, p, al, t);
+  const double f1dt = __dmul_rn(p.f1, __dsub_rn(t, d.t_ref));
+  auto xof = [&](int i) {
+    const double f0 = __dadd_rn(d.f0_start, __dmul_rn((double)i, d.df0));
+    const double x = ft_track_x(f0, f1dt, D, d.f_min, d.inv_df);
+    *ties += ft_near_tie(x) ? 1u : 0u;
+    return x;
+  };
+  const int i_last = i_first + warp_n - 1;
+  const double xa = xof(i_first);
+  const int ka = __double2int_rn(xa);
+  const int s = ka - i_first;
+  const int sb = __double2int_rn(xof(i_last)) - i_last;
+  const int off = ka - kst_al;  // strip index of the warp's first output
+  int rel = 0;
+  const bool neg = sb < s;
+  if (sb != s) {
+    // smallest i in (i_first, i_last] with rint(x_i) - i != s: estimate from the slope, verify
+    // with the canonical arithmetic, bisect if the estimate is off
+    auto pred = [&](int i) { return (__double2int_rn(xof(i)) - i) != s; };
+    int lo = i_first, hi = i_last;
+    const double frac = xa - (double)ka;
+    double nest = ceil((0.5 - (neg ? -frac : frac)) / fmax(fabs(D - 1.0), 1e-300));
+    nest = fmin(fmax(nest, 1.0), (double)(warp_n - 1));
+    const int cand = i_first + (int)nest;
+    if (pred(cand)) {
+      hi = cand;
+      if (cand - 1 > lo) { if (!pred(cand - 1)) lo = cand - 1; else hi = cand - 1; }
+    } else {
+      lo = cand;
+      if (cand + 1 < hi) { if (pred(cand + 1)) hi = cand + 1; else lo = cand + 1; }
+    }
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (pred(mid)) hi = mid; else lo = mid;
+    }
+    rel = hi - i_first;
+    if (sb - s > 1 || s - sb > 1) atomicExch(err, 2);
+  }
+  // every pixel read for a valid output must lie inside the copied strip (else: a planning bug)
+  const int hi_idx = off + (warp_n - 1) + ((rel && !neg) ? 1 : 0);
+  if (off < 0 || off > kMaxPitch || hi_idx >= copy_floats) {
+    atomicExch(err, 1);
+    return 0u;
+  }
+  return pack_entry(off, rel, neg);
+}
+
 template <int J>
-__global__ void __launch_bounds__(512, 1)
+__global__ void __launch_bounds__(ft_tile_max_threads(J), 1)
 ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_cw = a.R * a.wpp;
   const int tile = (int)(blockIdx.x % (unsigned)a.n_tiles);
   const uint64_t group = blockIdx.x / (unsigned)a.n_tiles;
-  const int64_t n_sft = d.n_sft;
-  const int RPS = a.rows_per_stage, NS = a.n_stages;
+  const int n_sft = (int)d.n_sft;
+  const int NS = a.n_stages;
   float* ring = reinterpret_cast<float*>(smem_raw);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NS * RPS * a.pitch * sizeof(float));
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NS * kRPS * a.pitch * sizeof(float));
   const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + NS);
   if (threadIdx.x == 0) {
     for (int s = 0; s < NS; ++s) {
@@ -93,29 +154,33 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
   }
   __syncthreads();
   const int32_t* kst = a.kst + (size_t)tile * n_sft;
-  const int64_t n_iters = (n_sft + RPS - 1) / RPS;
+  const uint32_t row_bytes = 4u * (uint32_t)a.pitch;
 
   if (warp == n_cw) {
     // ---- producer: one elected lane streams the strips (A3) ------------------------------------
     if (lane == 0) {
-      const int64_t total = n_sft * d.ld;
-      for (int64_t it = 0; it < n_iters; ++it) {
-        const int s = (int)(it % NS);
-        const uint32_t ph = (uint32_t)((it / NS) & 1);
-        if (it >= NS) mbar_wait(empty0 + 8 * s, ph ^ 1u);
-        const int64_t a0 = it * RPS;
-        const int rows = (int)min((int64_t)RPS, n_sft - a0);
-        uint32_t bytes = 0;
-        for (int r = 0; r < rows; ++r) {
-          const int64_t src = (a0 + r) * d.ld + kst[a0 + r];
-          bytes += 4u * (uint32_t)min((int64_t)a.copy_floats, total - src);
+      const int64_t total = (int64_t)n_sft * d.ld;
+      int s = 0;
+      uint32_t lap = 0;  // how many times the ring has wrapped
+      for (int a0 = 0; a0 < n_sft; a0 += kRPS) {
+        if (lap > 0) mbar_wait(empty0 + 8 * s, (lap - 1u) & 1u);  // consumers released the previous use
+        const int rows = min(kRPS, n_sft - a0);
+        int64_t src[kRPS];
+        uint32_t nb[kRPS], bytes = 0;
+#pragma unroll
+        for (int r = 0; r < kRPS; ++r) {
+          if (r < rows) {
+            src[r] = (int64_t)(a0 + r) * d.ld + kst[a0 + r];
+            nb[r] = 4u * (uint32_t)min((int64_t)a.copy_floats, total - src[r]);
+            bytes += nb[r];
+          }
         }
         mbar_expect_tx(full0 + 8 * s, bytes);
-        for (int r = 0; r < rows; ++r) {
-          const int64_t src = (a0 + r) * d.ld + kst[a0 + r];
-          const uint32_t nb = 4u * (uint32_t)min((int64_t)a.copy_floats, total - src);
-          bulk_g2s(smem_u32(ring + ((size_t)s * RPS + r) * a.pitch), a.A + src, nb, full0 + 8 * s);
-        }
+        const uint32_t dst = smem_u32(ring) + (uint32_t)(s * kRPS) * row_bytes;
+#pragma unroll
+        for (int r = 0; r < kRPS; ++r)
+          if (r < rows) bulk_g2s(dst + (uint32_t)r * row_bytes, a.A + src[r], nb[r], full0 + 8 * s);
+        if (++s == NS) { s = 0; ++lap; }
       }
     }
     return;
@@ -128,118 +193,66 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
   const bool pt_active = pt < a.pt_end;
   if (!pt_active) pt = a.pt_end - 1;  // keep the barrier protocol; results are discarded
   const FtPoint p = ft_decode_point(d, pt);
-  const int64_t tile_i0 = (int64_t)tile * a.tile_w;
-  const int wlo = sub * J * 32;                                    // warp's first output, tile-relative
-  const int64_t tile_n = min((int64_t)a.tile_w, d.n_f0 - tile_i0);  // valid f0 in this tile
-  const int warp_n = (int)max((int64_t)0, min((int64_t)(J * 32), tile_n - wlo));  // valid outputs of this warp
-  const int64_t i_first = tile_i0 + wlo;
-  const int64_t i_last = i_first + max(warp_n, 1) - 1;
-  float acc[J], tot[J];
+  const int tile_i0 = tile * a.tile_w;
+  const int wlo = sub * J * 32;                                        // warp's first output, tile-relative
+  const int tile_n = min(a.tile_w, (int)d.n_f0 - tile_i0);             // valid f0 in this tile
+  const int warp_n = max(0, min(J * 32, tile_n - wlo));                // valid outputs of this warp
+  const int i_first = tile_i0 + wlo;
+  float acc[J];
 #pragma unroll
-  for (int j = 0; j < J; ++j) { acc[j] = 0.f; tot[j] = 0.f; }
+  for (int j = 0; j < J; ++j) acc[j] = 0.f;
   unsigned ties = 0;
   const uint32_t lane_bytes = smem_u32(ring) + 4u * (uint32_t)lane;
-  const uint32_t row_bytes = 4u * (uint32_t)a.pitch;
+  uint32_t stage_addr = lane_bytes;
+  int s = 0;
+  uint32_t ph = 0;
 
-  for (int64_t a0 = 0; a0 < n_sft; a0 += 32) {
-    // -- A1/A2: this lane's SFT: canonical track at both ends of the warp's f0 range ---------------
+  for (int a0 = 0; a0 < n_sft; a0 += 32) {
+    // -- A1/A2: this lane's SFT ---------------------------------------------------------------------
     uint32_t entry = 0;
-    {
-      const int64_t al = a0 + lane;
-      if (al < n_sft && warp_n > 0) {
-        const double t = d.t_mid[al];
-        const double D = ft_doppler(d, p, al, t);
-        const double f1dt = __dmul_rn(p.f1, __dsub_rn(t, d.t_ref));
-        const double xa = ft_track_x(ft_f0(d, i_first), f1dt, D, d.f_min, d.inv_df);
-        const double xb = ft_track_x(ft_f0(d, i_last), f1dt, D, d.f_min, d.inv_df);
-        ties += (ft_near_tie(xa) ? 1u : 0u) + (ft_near_tie(xb) ? 1u : 0u);
-        const int64_t ka = __double2ll_rn(xa), kb = __double2ll_rn(xb);
-        const int64_t s = ka - i_first, sb = kb - i_last;
-        const int64_t off = ka - (int64_t)kst[al];  // strip index of the warp's first output
-        int rel = 0;
-        bool neg = false;
-        if (sb != s) {
-          neg = sb < s;
-          // smallest i in (i_first, i_last] with rint(x_i) - i != s
-          int64_t lo = i_first, hi = i_last;
-          const double frac = xa - (double)ka;
-          const double slope = fabs(D - 1.0);
-          double nest = ceil((0.5 - (neg ? -frac : frac)) / fmax(slope, 1e-300));
-          nest = fmin(fmax(nest, 1.0), (double)(i_last - i_first));
-          auto pred = [&](int64_t i) {
-            const double x = ft_track_x(ft_f0(d, i), f1dt, D, d.f_min, d.inv_df);
-            ties += ft_near_tie(x) ? 1u : 0u;
-            return (__double2ll_rn(x) - i) != s;
-          };
-          const int64_t cand = i_first + (int64_t)nest;
-          if (pred(cand)) {
-            hi = cand;
-            if (cand - 1 > lo) { if (!pred(cand - 1)) lo = cand - 1; else hi = cand - 1; }
-          } else {
-            lo = cand;
-            if (cand + 1 < hi) { if (pred(cand + 1)) hi = cand + 1; else lo = cand + 1; }
-          }
-          while (hi - lo > 1) {
-            const int64_t mid = (lo + hi) >> 1;
-            if (pred(mid)) hi = mid; else lo = mid;
-          }
-          rel = (int)(hi - i_first);
-          if (sb - s > 1 || s - sb > 1) atomicExch(a.err, 2);
-        }
-        // every pixel read for a valid output must lie inside the copied strip (else: plan bug)
-        const int64_t hi_idx = off + (warp_n - 1) + ((rel && !neg) ? 1 : 0);
-        if (off < 0 || off > kMaxPitch || hi_idx >= a.copy_floats) {
-          atomicExch(a.err, 1);
-        } else {
-          entry = pack_entry((int)off, rel, neg);
-        }
-      }
-    }
+    if (a0 + lane < n_sft && warp_n > 0)
+      entry = ft_tile_entry(d, p, a0 + lane, kst[a0 + lane], i_first, warp_n, a.copy_floats, &ties, a.err);
     // -- A4: gather + reduce over the block's SFTs -----------------------------------------------
-    const int n_rows = (int)min((int64_t)32, n_sft - a0);
-    for (int q = 0; q < n_rows; q += RPS) {
-      const int64_t it = (a0 + q) / RPS;
-      const int s = (int)(it % NS);
-      mbar_wait(full0 + 8 * s, (uint32_t)((it / NS) & 1));
-      const int rows = min(RPS, n_rows - q);
-      const uint32_t stage_bytes = lane_bytes + (uint32_t)(s * RPS) * row_bytes;
-      for (int r = 0; r < rows; ++r) {
-        const uint32_t e = __shfl_sync(0xffffffffu, entry, q + r);
-        const uint32_t base = stage_bytes + (uint32_t)r * row_bytes;
-        if (e < 8192u) {  // no break inside this warp's range: J conflict-free LDS.32 + FADD
-          const uint32_t ad = base + 4u * e;
-          float v[J];
+    const int n_rows = min(32, n_sft - a0);
+    for (int q = 0; q < n_rows; q += kRPS) {
+      mbar_wait(full0 + 8 * s, ph);
 #pragma unroll
-          for (int j = 0; j < J; ++j)
-            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v[j]) : "r"(ad + 128u * j));
+      for (int r = 0; r < kRPS; ++r) {
+        if (q + r < n_rows) {
+          const uint32_t e = __shfl_sync(0xffffffffu, entry, q + r);
+          const uint32_t base = stage_addr + (uint32_t)r * row_bytes;
+          if (e < 8192u) {  // no break inside this warp's range: J conflict-free LDS.32 + FADD
+            const uint32_t ad = base + 4u * e;
+            float v[J];
 #pragma unroll
-          for (int j = 0; j < J; ++j) acc[j] += v[j];
-        } else {
-          const uint32_t off = e & 8191u;
-          const int rel = (int)((e >> 13) & 2047u);
-          const uint32_t ad_lo = base + 4u * off;
-          const uint32_t ad_hi = (e & (1u << 24)) ? ad_lo - 4u : ad_lo + 4u;
-          const int t_lane = rel - lane;
+            for (int j = 0; j < J; ++j)
+              asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v[j]) : "r"(ad + 128u * j));
 #pragma unroll
-          for (int j = 0; j < J; ++j) {
-            const uint32_t ad = ((32 * j >= t_lane) ? ad_hi : ad_lo) + 128u * j;
-            float v;
-            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(ad));
-            acc[j] += v;
+            for (int j = 0; j < J; ++j) acc[j] += v[j];
+          } else {
+            const uint32_t ad_lo = base + 4u * (e & 8191u);
+            const uint32_t ad_hi = (e & (1u << 24)) ? ad_lo - 4u : ad_lo + 4u;
+            const int t_lane = (int)((e >> 13) & 2047u) - lane;
+#pragma unroll
+            for (int j = 0; j < J; ++j) {
+              const uint32_t ad = ((32 * j >= t_lane) ? ad_hi : ad_lo) + 128u * j;
+              float v;
+              asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(ad));
+              acc[j] += v;
+            }
           }
         }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(empty0 + 8 * s);
+      if (++s == NS) { s = 0; ph ^= 1u; stage_addr = lane_bytes; } else { stage_addr += kRPS * row_bytes; }
     }
-#pragma unroll
-    for (int j = 0; j < J; ++j) { tot[j] += acc[j]; acc[j] = 0.f; }
   }
 
   // ---- A5/A6: epilogue ---------------------------------------------------------------------------
-  if (ties && a.near_ties) {
+  if (a.near_ties) {
     for (int o = 16; o > 0; o >>= 1) ties += __shfl_xor_sync(0xffffffffu, ties, o);
-    if (lane == 0 && pt_active) atomicAdd(a.near_ties, (unsigned long long)ties);
+    if (lane == 0 && pt_active && ties) atomicAdd(a.near_ties, (unsigned long long)ties);
   }
   if (!pt_active) return;
 #pragma unroll
@@ -248,7 +261,7 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
     if (ii < warp_n) {
       const int64_t i = i_first + ii;
       const uint64_t idx = pt * (uint64_t)d.n_f0 + (uint64_t)i;
-      const float v = tot[j];
+      const float v = (float)((double)acc[j] + a.add_back);
       if (a.out_f) a.out_f[idx - a.out_base] = v;
       if (a.out_i) a.out_i[idx - a.out_base] = __float2int_rn(v);
       if (a.has_sel) {
@@ -289,11 +302,33 @@ __global__ void ft_hitmap_kernel(const float* __restrict__ P, float rho, float* 
     H[i] = (P[i] > rho) ? 1.f : 0.f;
 }
 
-__global__ void ft_fold_sft_kernel(const float* __restrict__ P, const float* __restrict__ w,
-                                   float* __restrict__ Q, int64_t n_sft, int64_t ld) {
-  const int64_t n = n_sft * ld, stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-    Q[i] = __fmul_rn(w[i / ld], P[i]);
+// A0: fold the weights into the gathered array and remove a per-row constant, one CTA per SFT row:
+//   q = fl(w P);  c_a = fl(mean_k q);  Q[a][k] = fl(q - c_a).
+// Removing c_a keeps the running sums of K2 near zero (a random walk of ~sqrt(n_sft) pixel sigmas
+// instead of a ramp to n_sft means), so one level of fp32 accumulation is enough (DESIGN.md
+// "Accumulation"); sum_a c_a is added back in fp64 in the epilogue.
+__global__ void __launch_bounds__(256)
+ft_fold_centered_kernel(const float* __restrict__ P, const float* __restrict__ w_sft,
+                        const float* __restrict__ w_bin, float* __restrict__ Q,
+                        float* __restrict__ c_row, int64_t n_bins, int64_t ld) {
+  __shared__ double red[256];
+  const int64_t a = blockIdx.x;
+  const float* Pr = P + a * ld;
+  const float* wr = w_bin ? w_bin + a * ld : nullptr;
+  const float ws = w_sft ? w_sft[a] : 0.f;
+  double sum = 0.0;
+  for (int64_t k = threadIdx.x; k < n_bins; k += blockDim.x)
+    sum += (double)__fmul_rn(wr ? wr[k] : ws, Pr[k]);
+  red[threadIdx.x] = sum;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    __syncthreads();
+  }
+  const float c = (float)(red[0] / (double)n_bins);
+  if (threadIdx.x == 0) c_row[a] = c;
+  for (int64_t k = threadIdx.x; k < ld; k += blockDim.x)
+    Q[a * ld + k] = (k < n_bins) ? __fsub_rn(__fmul_rn(wr ? wr[k] : ws, Pr[k]), c) : 0.f;
 }
 
 // J values the kernel is instantiated for (the plan rounds the per-warp chunk count up to one)
@@ -362,7 +397,7 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   pl.tile_w = (int32_t)(((chunks + bT - 1) / bT) * 32);
   pl.n_tiles = (int32_t)((d.n_f0 + pl.tile_w - 1) / pl.tile_w);
   int R = in.points_per_cta > 0 ? in.points_per_cta : 8;
-  R = std::min<int>(R, 15 / pl.wpp);  // 15 consumer warps + 1 producer = 512 threads (128 registers)
+  R = std::min<int>(R, (ft_tile_max_threads(pl.J) / 32 - 1) / pl.wpp);  // + 1 producer warp
   R = (int)std::min<uint64_t>((uint64_t)R, d.n_points);
   pl.R = std::max(R, 1);
   // --- point-independent strip bounds per (tile, SFT) -----------------------------------------------
@@ -417,16 +452,16 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   if (pl.copy_floats > kMaxPitch + 1) { *why = "strip too wide for the packed track entry"; return cudaSuccess; }
   // --- shared-memory ring ---------------------------------------------------------------------------
   const int threads = (pl.R * pl.wpp + 1) * 32;
-  const int regs_est = 3 * pl.J + 34;
+  const int regs_est = 2 * pl.J + 30;
   int ctas = std::min(4, std::min(2048 / threads, 65536 / (threads * regs_est)));
   ctas = std::max(ctas, 1);
   const size_t row_bytes = (size_t)pl.pitch * 4;
   const size_t budget = (size_t)(228 * 1024) / ctas - 2048;
   int64_t rows_fit = (int64_t)((budget - 1024) / row_bytes);
-  if (rows_fit < 2) { *why = "strip does not fit shared memory twice"; return cudaSuccess; }
+  if (rows_fit < 2 * kRPS) { *why = "strip does not fit shared memory twice"; return cudaSuccess; }
   rows_fit = std::min<int64_t>(rows_fit, 32);
-  pl.rows_per_stage = rows_fit >= 12 ? 4 : (rows_fit >= 6 ? 2 : 1);
-  pl.n_stages = (int32_t)(rows_fit / pl.rows_per_stage);
+  pl.rows_per_stage = kRPS;
+  pl.n_stages = (int32_t)(rows_fit / kRPS);
   pl.ctas_per_sm = ctas;
   pl.smem_bytes = (size_t)pl.n_stages * pl.rows_per_stage * row_bytes + 2 * 8 * (size_t)pl.n_stages;
   e = cudaMalloc(&pl.kst, sizeof(int32_t) * kst.size());
@@ -446,7 +481,7 @@ uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points) {
   return std::min(s, n_points);
 }
 
-cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, uint64_t pt_begin,
+cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, double add_back, uint64_t pt_begin,
                            uint64_t pt_end, float* out_f, int32_t* out_i, uint64_t out_base,
                            const FtSelectDev* sel, int32_t bpb, unsigned long long* near_ties,
                            cudaStream_t s, int* launches) {
@@ -456,7 +491,7 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* 
   a.A = A; a.kst = plan.kst; a.err = plan.err;
   a.tile_w = plan.tile_w; a.n_tiles = plan.n_tiles; a.R = plan.R; a.wpp = plan.wpp;
   a.pitch = plan.pitch; a.copy_floats = plan.copy_floats;
-  a.rows_per_stage = plan.rows_per_stage; a.n_stages = plan.n_stages;
+  a.n_stages = plan.n_stages; a.add_back = add_back;
   a.out_f = out_f; a.out_i = out_i; a.out_base = out_base;
   if (sel) { a.sel = *sel; a.has_sel = 1; }
   a.bpb = bpb > 0 ? bpb : 1;
@@ -482,7 +517,8 @@ cudaError_t ft_launch_hitmap(const float* P, float rho, float* H, int64_t n, cud
   return cudaGetLastError();
 }
 
-cudaError_t ft_launch_fold_sft(const float* P, const float* w_sft, float* Q, int64_t n_sft, int64_t ld, cudaStream_t s) {
-  ft_fold_sft_kernel<<<148 * 8, 256, 0, s>>>(P, w_sft, Q, n_sft, ld);
+cudaError_t ft_launch_fold_centered(const float* P, const float* w_sft, const float* w_bin, float* Q, float* c_row,
+                                    int64_t n_sft, int64_t n_bins, int64_t ld, cudaStream_t s) {
+  ft_fold_centered_kernel<<<(unsigned)n_sft, 256, 0, s>>>(P, w_sft, w_bin, Q, c_row, n_bins, ld);
   return cudaGetLastError();
 }

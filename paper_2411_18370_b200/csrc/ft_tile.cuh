@@ -33,12 +33,15 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
                          std::string* why, int* launches);
 uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points);
 // One pass of the gather-reduce over array A (folded w*P for the power statistic, the 0/1 hit map
-// for the number count).  Writes out_f (fp32) and/or out_i (int32) indexed from out_base, and/or
+// for the number count); add_back is the constant the fold removed from A, summed over SFTs.
+// Writes out_f (fp32) and/or out_i (int32) indexed from out_base, and/or
 // filters into sel (bands of bpb f0 bins).
-cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, uint64_t pt_begin,
+cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, double add_back, uint64_t pt_begin,
                            uint64_t pt_end, float* out_f, int32_t* out_i, uint64_t out_base,
                            const FtSelectDev* sel, int32_t bpb, unsigned long long* near_ties,
                            cudaStream_t s, int* launches);
 cudaError_t ft_launch_hitmap(const float* P, float rho, float* H, int64_t n, cudaStream_t s);
-cudaError_t ft_launch_fold_sft(const float* P, const float* w_sft, float* Q, int64_t n_sft, int64_t ld, cudaStream_t s);
+// Q[a][k] = fl(fl(w P) - c_a) with c_a = fl(mean_k fl(w P)) per row; w_sft (per-SFT) or w_bin (per-bin).
+cudaError_t ft_launch_fold_centered(const float* P, const float* w_sft, const float* w_bin, float* Q, float* c_row,
+                                    int64_t n_sft, int64_t n_bins, int64_t ld, cudaStream_t s);
 void ft_tile_plan_free(FtTilePlan* plan);
