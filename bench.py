@@ -29,6 +29,9 @@ from paper_2411_18370_b200 import workloads as W  # noqa: E402
 
 METRIC = "template_sft_evals_per_sec"
 UNIT = "evals/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per statistic launch (profiles/r01_k2_ncu_full.md: the
+# spectrogram is read from HBM once per launch, everything else is served from L2 / shared memory)
+NCU_TRAFFIC = {2: 31.19e6}
 SMEM_BYTES_PER_CLK_SM = 128.0   # B200_MICROARCH "smem crossbar BW 128 B/cyc/SM"
 N_SM = 148
 
@@ -164,6 +167,7 @@ def run_gpu(args):
     ctx = B.Context(P_dev, wl.t_mid, wl.vel, w_arg, wl.f_min, wl.df, stream)
     ctx.set_option(B.FT_OPT_KERNEL, args.kernel)
     ctx.set_option(B.FT_OPT_FUSED_TOPK, args.fused)
+    ctx.set_option(B.FT_OPT_POINTS_PER_CTA, args.ppc)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     evals = g.n_templates * wl.n_sft
 
@@ -186,14 +190,15 @@ def run_gpu(args):
     c0 = ctx.counters()
     sampler = ClockSampler(local); sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kern_ms = []
+    kern_ms, kern_n = [], []
     barrier()
     for s in range(args.steps):
         flush.fill_(s & 255)                                # flush L2 between timed steps
         ev[s][0].record(stream)
         step(ctx)
         ev[s][1].record(stream)
-        kern_ms.append(ctx.counters()["last_kernel_ms"])
+        cs = ctx.counters()
+        kern_ms.append(cs["last_kernel_ms"]); kern_n.append(cs["stat_launches"])
     barrier()
     clocks = sampler.stop()
     c1 = ctx.counters()
@@ -216,6 +221,7 @@ def run_gpu(args):
             wa = torch.empty_like(w_arg); wa.copy_(w_host, non_blocking=True)
         c2 = B.Context(Pd, wl.t_mid, wl.vel, wa, wl.f_min, wl.df, stream)
         c2.set_option(B.FT_OPT_KERNEL, args.kernel); c2.set_option(B.FT_OPT_FUSED_TOPK, args.fused)
+        c2.set_option(B.FT_OPT_POINTS_PER_CTA, args.ppc)
         cands = step(c2)
         barrier()
         if s > 0:
@@ -234,8 +240,11 @@ def run_gpu(args):
         except OSError:
             pass
         hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-        k_ms = float(np.mean(kern_ms))
-        achieved = 4.0 * evals / (k_ms * 1e-3) / 1e9       # algorithmic gather bytes: 4 B per eval
+        k_ms = float(np.mean(kern_ms))                     # statistic-kernel device time per step
+        n_launch = float(np.mean(kern_n))                  # statistic-kernel launches per step
+        # per launch: 4 B x (evals / n_launch) over (k_ms / n_launch) -- algorithmic gather bytes
+        achieved = 4.0 * evals / (k_ms * 1e-3) / 1e9
+        traffic = args.traffic if args.traffic is not None else NCU_TRAFFIC.get(args.config)
         sm_mhz = clocks.get("sm_mhz") or 1965.0
         smem_peak = SMEM_BYTES_PER_CLK_SM * N_SM * sm_mhz * 1e6 / 1e9
         out = {
@@ -249,9 +258,11 @@ def run_gpu(args):
             "e2e": {"value": evals * world / (float(e2e_t.item()) * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": d2h},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                         "frac": achieved / hbm_peak, "traffic": args.traffic,
-                         "kernel": "statistic kernel(s) of ft_topk_per_band (CUDA events inside the library, mean over timed steps)",
-                         "kernel_ms": k_ms,
+                         "frac": achieved / hbm_peak, "traffic": traffic,
+                         "kernel": "ft_tile_kernel (K2) / ft_generic_kernel (K0): the statistic launches of ft_topk_per_band, CUDA events on the library's stream around each launch, summed per step, mean over timed steps",
+                         "kernel_ms": k_ms, "launches_per_step": n_launch,
+                         "algorithmic_bytes_per_launch": 4.0 * evals / max(n_launch, 1.0),
+                         "share_of_step": k_ms / (total_ms / args.steps),
                          "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "fallback 6650 GB/s (of fallback)",
                          "note": "north_star gather roofline: 4 B per template·SFT eval over HBM/L2 bandwidth; strips staged once in shared memory are re-read by many templates, so frac can exceed 1 — see tight",
                          "tight": {"bound": "smem", "peak": smem_peak, "unit": "GB/s", "frac": achieved / smem_peak,
@@ -276,6 +287,7 @@ def main():
     ap.add_argument("--n-sft", type=int, default=0)
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 tile")
     ap.add_argument("--fused", type=int, default=1)
+    ap.add_argument("--ppc", type=int, default=0, help="outer points per CTA (0 = library default)")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per launch (from profiles/)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

@@ -149,12 +149,13 @@ typedef enum {
 int ft_set_option(ft_ctx* ctx, int option, int64_t value);
 
 typedef struct {
-  uint64_t near_ties;        /* (template-tile, SFT) pairs whose break evaluation fell within 1e-9 bin of a rounding tie */
+  uint64_t near_ties;        /* canonical track evaluations that fell within 1e-9 bin of a rounding tie, since ft_create */
   uint64_t refine_fallbacks; /* selections that had to be redone with a tighter threshold */
   uint64_t appended;         /* candidates that passed the fused fp32 filter (last top-k call) */
   uint64_t refined;          /* candidates re-evaluated in fp64 (last top-k call) */
   uint64_t kernel_launches;  /* CUDA kernels launched by this handle since ft_create */
-  double last_kernel_ms;     /* device time of the last statistic kernel (CUDA events on the handle's stream) */
+  uint64_t stat_launches;    /* statistic-kernel launches (K0/K2) of the last ft_eval / ft_topk_per_band call */
+  double last_kernel_ms;     /* summed device time of those launches (CUDA events on the handle's stream) */
 } ft_counters;
 int ft_get_counters(ft_ctx* ctx, ft_counters* out);
 

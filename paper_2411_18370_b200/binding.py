@@ -38,7 +38,8 @@ CAND_DTYPE = np.dtype([("power", "<f8"), ("wcount", "<f8"), ("idx", "<u8"), ("co
 class FtCounters(C.Structure):
     _fields_ = [("near_ties", C.c_uint64), ("refine_fallbacks", C.c_uint64),
                 ("appended", C.c_uint64), ("refined", C.c_uint64),
-                ("kernel_launches", C.c_uint64), ("last_kernel_ms", C.c_double)]
+                ("kernel_launches", C.c_uint64), ("stat_launches", C.c_uint64),
+                ("last_kernel_ms", C.c_double)]
 
 
 class FtError(RuntimeError):

@@ -50,8 +50,8 @@ struct ft_ctx {
   unsigned long long* near_ties_dev = nullptr;
   // bookkeeping
   ft_counters counters{};
-  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-  bool ev_valid = false;
+  std::vector<cudaEvent_t> evs;  // pairs around every statistic-kernel pass of the last call
+  size_t ev_used = 0;
   std::string err = "";
 };
 
@@ -120,13 +120,20 @@ int ensure_scratch(ft_ctx* c, size_t elems, bool need_int) {
   return FT_OK;
 }
 
+// CUDA events on the handle's stream around each statistic pass (ft_counters.last_kernel_ms)
 void tick(ft_ctx* c) {
-  if (!c->ev0) { cudaEventCreate(&c->ev0); cudaEventCreate(&c->ev1); }
-  cudaEventRecord(c->ev0, c->stream);
+  if (c->ev_used + 2 > c->evs.size()) {
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    c->evs.push_back(e0); c->evs.push_back(e1);
+  }
+  cudaEventRecord(c->evs[c->ev_used], c->stream);
 }
-void tock(ft_ctx* c) {
-  cudaEventRecord(c->ev1, c->stream);
-  c->ev_valid = true;
+void tock(ft_ctx* c, int launches) {
+  cudaEventRecord(c->evs[c->ev_used + 1], c->stream);
+  c->ev_used += 2;
+  c->counters.stat_launches += (uint64_t)launches;
+  c->counters.kernel_launches += (uint64_t)launches;
 }
 
 // Statistic over points [pt_begin, pt_end): full write-out (out_* indexed from out_base) and/or
@@ -135,23 +142,26 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
              uint64_t out_base, bool filter, int32_t bpb) {
   const bool use_tile = c->tile_ok && c->opt_kernel != 1;
   if (use_tile) {
-    // one gather-reduce pass per statistic: power over Q = w*P, number count over the hit map
+    // one gather-reduce pass per statistic: power over Q, number count over the hit map
     const FtSelectDev* sel = filter ? &c->sel : nullptr;
     int launches = 0;
     if (stat != FT_STAT_HOUGH && (out_power || (filter && stat == FT_STAT_POWER))) {
+      tick(c);
       FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.Q, c->add_back, pt_begin, pt_end, out_power, nullptr, out_base,
                                 stat == FT_STAT_POWER ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
-      c->counters.kernel_launches += launches;
+      tock(c, launches);
     }
     if (stat != FT_STAT_POWER && (out_count || (filter && stat == FT_STAT_HOUGH))) {
+      tick(c);
       FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.H, 0.0, pt_begin, pt_end, nullptr, out_count, out_base,
                                 stat == FT_STAT_HOUGH ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
-      c->counters.kernel_launches += launches;
+      tock(c, launches);
     }
   } else {
     if (filter) return fail(c, FT_ERR_UNSUPPORTED, "fused filter needs the tile kernel");
+    tick(c);
     FT_CUDA(c, ft_launch_generic(c->d, stat, pt_begin, pt_end, out_power, out_count, out_base, c->stream));
-    c->counters.kernel_launches += 1;
+    tock(c, 1);
   }
   return FT_OK;
 }
@@ -324,9 +334,8 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   d.H = c->H_dev;
   c->bound = true;
   if (out_power_dev || out_count_dev) {
-    tick(c);
+    c->ev_used = 0; c->counters.stat_launches = 0;
     const int rc = run_stat(c, stat, 0, d.n_points, out_power_dev, out_count_dev, 0, false, 1);
-    tock(c);
     if (rc != FT_OK) return rc;
   }
   return FT_OK;
@@ -367,7 +376,7 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
   uint32_t* overflow = c->final_n + 1;
   FT_CUDA(c, ft_select_reset(c->sel, c->final_n, overflow, c->stream));
   c->counters.kernel_launches += 1;
-  tick(c);
+  c->ev_used = 0; c->counters.stat_launches = 0;
   for (uint64_t pt = 0; pt < d.n_points; pt += chunk_pts) {
     const uint64_t pe = (pt + chunk_pts < d.n_points) ? pt + chunk_pts : d.n_points;
     if (fused && pt > 0) {  // phase B: everything after the sample goes through the fused filter
@@ -390,7 +399,6 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
     FT_CUDA(c, ft_select_append_keys(c->scratch_f, rows, d.n_f0, (int32_t)bpb, pt, c->sel, c->stream));
     c->counters.kernel_launches += 1;
   }
-  tock(c);
   FT_CUDA(c, ft_select_trim(c->sel, (uint32_t)k, margin, c->final_idx, c->final_band, c->final_n, c->final_cap, overflow, c->stream));
   FT_CUDA(c, ft_launch_refine(d, c->final_idx, c->final_n, c->final_cap, c->cand, c->near_ties_dev, c->stream));
   FT_CUDA(c, ft_select_rank(c->cand, c->final_band, c->final_n, c->final_cap, by_count ? 1 : 0, (uint32_t)k, n_bands, c->out_dev, overflow, c->stream));
@@ -444,10 +452,12 @@ int ft_get_counters(ft_ctx* c, ft_counters* out) {
   unsigned long long nt = 0;
   FT_CUDA(c, cudaMemcpy(&nt, c->near_ties_dev, sizeof nt, cudaMemcpyDeviceToHost));
   c->counters.near_ties = nt;
-  if (c->ev_valid) {
+  double ms_sum = 0.0;
+  for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
     float ms = 0.f;
-    if (cudaEventElapsedTime(&ms, c->ev0, c->ev1) == cudaSuccess) c->counters.last_kernel_ms = ms;
+    if (cudaEventElapsedTime(&ms, c->evs[i], c->evs[i + 1]) == cudaSuccess) ms_sum += ms;
   }
+  c->counters.last_kernel_ms = ms_sum;
   *out = c->counters;
   return FT_OK;
 }
@@ -461,7 +471,7 @@ void ft_destroy(ft_ctx* c) {
   ft_tile_plan_free(&c->plan);
   dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->H_dev); dfree(c->axes_dev);
   dfree(c->scratch_f); dfree(c->scratch_i); dfree(c->near_ties_dev);
-  if (c->ev0) { cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1); }
+  for (cudaEvent_t e : c->evs) cudaEventDestroy(e);
   delete c;
 }
 

@@ -396,7 +396,8 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   pl.J = bJ; pl.wpp = bW;
   pl.tile_w = (int32_t)(((chunks + bT - 1) / bT) * 32);
   pl.n_tiles = (int32_t)((d.n_f0 + pl.tile_w - 1) / pl.tile_w);
-  int R = in.points_per_cta > 0 ? in.points_per_cta : 8;
+  // default: ~20 consumer warps per CTA (measured best on B200: R = 10 at wpp = 2, R = 23 at wpp = 1)
+  int R = in.points_per_cta > 0 ? in.points_per_cta : (pl.wpp == 1 ? 23 : 20 / pl.wpp);
   R = std::min<int>(R, (ft_tile_max_threads(pl.J) / 32 - 1) / pl.wpp);  // + 1 producer warp
   R = (int)std::min<uint64_t>((uint64_t)R, d.n_points);
   pl.R = std::max(R, 1);

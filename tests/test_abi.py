@@ -27,7 +27,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_struct_layouts():
     assert C.sizeof(B.FtCand) == 32 and B.CAND_DTYPE.itemsize == 32
-    assert C.sizeof(B.FtCounters) == 48
+    assert C.sizeof(B.FtCounters) == 56
     assert B.FtGrid.n_f0.offset == 16 and B.FtGrid.t_ref.offset == 48
     assert C.sizeof(B.FtGrid) == 120
 
