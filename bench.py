@@ -37,22 +37,24 @@ N_SM = 148
 
 
 def make_workload(args, rank=0, world=1):
-    kw = {}
+    """The rank's shard of the bank (weak scaling: the sky grid grows with the world size; the
+    binary config shards its a_p axis).  Returns (workload with the local grid, index offset)."""
+    from paper_2411_18370_b200 import sharding as S
+    kw = {"n_sft": args.n_sft} if args.n_sft else {}
     if args.config == 2:
-        n_sky = args.n_sky or 20000
-        wl = W.config2(n_sky=n_sky * world, **({"n_sft": args.n_sft} if args.n_sft else {}))
-        wl.grid.sky = np.ascontiguousarray(wl.grid.sky[rank * n_sky:(rank + 1) * n_sky])
+        wl = W.config2(n_sky=(args.n_sky or 20000) * world, **kw)
     elif args.config == 3:
-        wl = W.config3(**({"n_sft": args.n_sft} if args.n_sft else {}))
-        if world > 1:  # shard the a_p axis
-            wl.grid.a_p = np.array_split(wl.grid.a_p, world)[rank]
+        wl = W.config3(**kw)
     elif args.config == 4:
-        n_sky = args.n_sky or 5000
-        wl = W.config4(n_sky=n_sky * world, **({"n_sft": args.n_sft} if args.n_sft else {}))
-        wl.grid.sky = np.ascontiguousarray(wl.grid.sky[rank * n_sky:(rank + 1) * n_sky])
+        wl = W.config4(n_sky=(args.n_sky or 5000) * world, **kw)
     else:
         wl = W.config1()
-    return wl
+    off = 0
+    if world > 1:
+        g, off = S.shard_grid(wl.grid, rank, world)
+        assert g is not None, "more ranks than entries on the sharded axis"
+        wl.grid = g
+    return wl, off
 
 
 class ClockSampler:
@@ -115,7 +117,7 @@ def run_reference(args):
     """--impl reference: the CPU oracle on the host cores (rank 0 only), a bounded sample per step."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    wl = make_workload(args)
+    wl, _ = make_workload(args)
     per_step = 8.0
     for _ in range(args.warmup):
         oracle_sample(wl, seconds=1.0)
@@ -156,7 +158,8 @@ def run_gpu(args):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    wl = make_workload(args, rank, world)
+    wl, idx_off = make_workload(args, rank, world)
+    from paper_2411_18370_b200 import sharding as S
     g = wl.grid
     bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
     stream = torch.cuda.current_stream(dev)
@@ -174,10 +177,9 @@ def run_gpu(args):
     def step(c):
         c.eval(g, wl.stat, wl.rho_th)                      # bind grid (+ fold weights / threshold bit)
         cands = c.topk_per_band(wl.band_width, wl.k, n_bands)   # evaluate + fused selection; syncs
-        if world > 1:
-            t = torch.from_numpy(cands.view(np.uint8).reshape(-1)).to(dev)
-            allc = [torch.empty_like(t) for _ in range(world)]
-            dist.all_gather(allc, t)
+        if world > 1:  # KBs of records: all-gather + merge under the same total order
+            cands = S.merge_candidates(S.all_gather_candidates(S.to_global(cands, idx_off), dev), wl.k,
+                                       by_count=(wl.stat == "hough"))
         return cands
 
     def barrier():
@@ -268,6 +270,7 @@ def run_gpu(args):
                          "tight": {"bound": "smem", "peak": smem_peak, "unit": "GB/s", "frac": achieved / smem_peak,
                                    "how": f"128 B/clk/SM x 148 SMs x {sm_mhz:.0f} MHz (median SM clock during the timed region)"}},
             "counters": {k: c1[k] for k in ("near_ties", "appended", "refined", "refine_fallbacks")},
+            "kernel_geometry": ctx.describe(),
         }
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"], _ = oracle_sample(wl, seconds=args.cpu_seconds)

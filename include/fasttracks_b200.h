@@ -160,6 +160,8 @@ typedef struct {
 int ft_get_counters(ft_ctx* ctx, ft_counters* out);
 
 const char* ft_last_error(const ft_ctx* ctx); /* never NULL; valid until the next call on ctx */
+/* Which kernel the bound grid runs and its launch geometry (diagnostics; never NULL; valid until the next ft_eval). */
+const char* ft_describe(const ft_ctx* ctx);
 void ft_destroy(ft_ctx* ctx);                 /* synchronises the stream, frees library-owned memory */
 
 #ifdef __cplusplus

@@ -13,7 +13,7 @@ from . import build as _build
 FT_STAT = {"power": 0, "hough": 1, "both": 2}
 FT_OPT_KERNEL, FT_OPT_FUSED_TOPK, FT_OPT_POINTS_PER_CTA = 0, 1, 2
 SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_eval_list", "ft_set_option",
-           "ft_get_counters", "ft_last_error", "ft_destroy"]
+           "ft_get_counters", "ft_last_error", "ft_describe", "ft_destroy"]
 
 
 class FtGrid(C.Structure):
@@ -75,6 +75,8 @@ def load_library(path: str | None = None):
         lib.ft_get_counters.argtypes = [C.c_void_p, C.POINTER(FtCounters)]
         lib.ft_last_error.restype = C.c_char_p
         lib.ft_last_error.argtypes = [C.c_void_p]
+        lib.ft_describe.restype = C.c_char_p
+        lib.ft_describe.argtypes = [C.c_void_p]
         lib.ft_destroy.restype = None
         lib.ft_destroy.argtypes = [C.c_void_p]
         _lib = lib
@@ -150,6 +152,9 @@ class Context:
         c = FtCounters()
         self._check(self.lib.ft_get_counters(self.h, C.byref(c)))
         return {f: getattr(c, f) for f, _ in FtCounters._fields_}
+
+    def describe(self) -> str:
+        return self.lib.ft_describe(self.h).decode()
 
     def close(self):
         if self.h:

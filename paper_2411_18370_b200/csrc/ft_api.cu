@@ -53,6 +53,8 @@ struct ft_ctx {
   std::vector<cudaEvent_t> evs;  // pairs around every statistic-kernel pass of the last call
   size_t ev_used = 0;
   std::string err = "";
+  std::string desc = "no grid bound";
+  std::string why;
 };
 
 namespace {
@@ -139,7 +141,7 @@ void tock(ft_ctx* c, int launches) {
 // Statistic over points [pt_begin, pt_end): full write-out (out_* indexed from out_base) and/or
 // fused filter into c->sel.  Chooses the tile or the generic kernel.
 int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out_power, int32_t* out_count,
-             uint64_t out_base, bool filter, int32_t bpb) {
+             uint64_t out_base, bool filter, int32_t bpb, uint32_t stride = 1, uint64_t n_strided = 0) {
   const bool use_tile = c->tile_ok && c->opt_kernel != 1;
   if (use_tile) {
     // one gather-reduce pass per statistic: power over Q, number count over the hit map
@@ -148,13 +150,13 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
     if (stat != FT_STAT_HOUGH && (out_power || (filter && stat == FT_STAT_POWER))) {
       tick(c);
       FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.Q, c->add_back, pt_begin, pt_end, out_power, nullptr, out_base,
-                                stat == FT_STAT_POWER ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
+                                stat == FT_STAT_POWER ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches, stride, n_strided));
       tock(c, launches);
     }
     if (stat != FT_STAT_POWER && (out_count || (filter && stat == FT_STAT_HOUGH))) {
       tick(c);
       FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.H, 0.0, pt_begin, pt_end, nullptr, out_count, out_base,
-                                stat == FT_STAT_HOUGH ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches));
+                                stat == FT_STAT_HOUGH ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches, stride, n_strided));
       tock(c, launches);
     }
   } else {
@@ -316,7 +318,7 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   // tile-kernel eligibility and plan
   c->tile_ok = false;
   if (c->opt_kernel != 1) {
-    std::string why;
+    std::string& why = c->why;
     int launches = 0;
     FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc};
     const cudaError_t e = ft_tile_plan(d, hin, c->stream, &c->plan, &why, &launches);
@@ -332,6 +334,16 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
     c->H_rho = d.rho; c->H_valid = true;
   }
   d.H = c->H_dev;
+  {
+    char buf[320];
+    if (c->tile_ok && c->opt_kernel != 1)
+      std::snprintf(buf, sizeof buf, "K2 tile kernel: J=%d wpp=%d R=%d n_tiles=%d tile_w=%d threads=%d pitch=%d copy=%d stages=%dx%d smem=%zu",
+                    c->plan.J, c->plan.wpp, c->plan.R, c->plan.n_tiles, c->plan.tile_w, (c->plan.R * c->plan.wpp + 1) * 32,
+                    c->plan.pitch, c->plan.copy_floats, c->plan.n_stages, c->plan.rows_per_stage, c->plan.smem_bytes);
+    else
+      std::snprintf(buf, sizeof buf, "K0 generic kernel (%s)", c->opt_kernel == 1 ? "forced" : c->why.c_str());
+    c->desc = buf;
+  }
   c->bound = true;
   if (out_power_dev || out_count_dev) {
     c->ev_used = 0; c->counters.stat_launches = 0;
@@ -361,43 +373,69 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
   const float margin = by_count ? 0.f : 4e-5f;  // fp32 accumulation error bound 1e-5
   const bool use_tile = c->tile_ok && c->opt_kernel != 1;
   const bool fused = use_tile && c->opt_fused;
-  // sample / chunk size in points
-  uint64_t chunk_pts;
-  if (fused) {
-    chunk_pts = ft_tile_sample_points(c->plan, d.n_points);
-  } else {
-    const uint64_t max_elems = (uint64_t)1 << 27;  // 512 MB of fp32 scratch per chunk
-    chunk_pts = max_elems / (uint64_t)d.n_f0;
-    if (chunk_pts < 1) chunk_pts = 1;
-  }
-  if (chunk_pts > d.n_points) chunk_pts = d.n_points;
-  rc = ensure_scratch(c, (size_t)chunk_pts * d.n_f0, by_count);
-  if (rc != FT_OK) return rc;
   uint32_t* overflow = c->final_n + 1;
   FT_CUDA(c, ft_select_reset(c->sel, c->final_n, overflow, c->stream));
   c->counters.kernel_launches += 1;
   c->ev_used = 0; c->counters.stat_launches = 0;
-  for (uint64_t pt = 0; pt < d.n_points; pt += chunk_pts) {
-    const uint64_t pe = (pt + chunk_pts < d.n_points) ? pt + chunk_pts : d.n_points;
-    if (fused && pt > 0) {  // phase B: everything after the sample goes through the fused filter
-      rc = run_stat(c, sel_stat, pt, d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb);
-      if (rc != FT_OK) return rc;
-      break;
-    }
-    rc = run_stat(c, sel_stat, pt, pe, by_count ? nullptr : c->scratch_f, by_count ? c->scratch_i : nullptr,
-                  pt * (uint64_t)d.n_f0, false, (int32_t)bpb);
+  std::vector<uint32_t> cnt(n_bands);
+  if (fused) {
+    // Phase A: per-band thresholds from a strided sample of point groups (every stride-th CTA group
+    // of the bank, so the sample sees every region of parameter space), written out in full.
+    const uint64_t R = (uint64_t)c->plan.R;
+    const uint64_t n_groups = (d.n_points + R - 1) / R;
+    uint64_t n_sg = ft_tile_sample_points(c->plan, d.n_points) / R;
+    n_sg = n_sg < 1 ? 1 : (n_sg > n_groups ? n_groups : n_sg);
+    const uint64_t stride = n_groups / n_sg;
+    const int64_t rows = (int64_t)(n_sg * R);
+    rc = ensure_scratch(c, (size_t)rows * d.n_f0, by_count);
     if (rc != FT_OK) return rc;
-    const int64_t rows = (int64_t)(pe - pt);
-    if (by_count) {
-      FT_CUDA(c, ft_count_to_key(c->scratch_i, c->scratch_f, rows * d.n_f0, c->stream));
-      c->counters.kernel_launches += 1;
-    }
-    if (pt == 0) {
-      FT_CUDA(c, ft_select_threshold(c->scratch_f, rows, d.n_f0, (int32_t)bpb, (uint32_t)k, margin, c->sel, c->stream));
-      c->counters.kernel_launches += 1;
-    }
-    FT_CUDA(c, ft_select_append_keys(c->scratch_f, rows, d.n_f0, (int32_t)bpb, pt, c->sel, c->stream));
+    // rows of a ragged last group are never written: make them lose every comparison
+    if (by_count) FT_CUDA(c, cudaMemsetAsync(c->scratch_i, 0x80, sizeof(int32_t) * (size_t)rows * d.n_f0, c->stream));
+    else { FT_CUDA(c, ft_fill_f32(c->scratch_f, rows * d.n_f0, -INFINITY, c->stream)); c->counters.kernel_launches += 1; }
+    if (stride > 1)
+      rc = run_stat(c, sel_stat, 0, d.n_points, by_count ? nullptr : c->scratch_f, by_count ? c->scratch_i : nullptr,
+                    0, false, (int32_t)bpb, (uint32_t)stride, n_sg);
+    else
+      rc = run_stat(c, sel_stat, 0, std::min<uint64_t>(d.n_points, (uint64_t)rows), by_count ? nullptr : c->scratch_f,
+                    by_count ? c->scratch_i : nullptr, 0, false, (int32_t)bpb);
+    if (rc != FT_OK) return rc;
+    if (by_count) { FT_CUDA(c, ft_count_to_key(c->scratch_i, c->scratch_f, rows * d.n_f0, c->stream)); c->counters.kernel_launches += 1; }
+    FT_CUDA(c, ft_select_threshold(c->scratch_f, rows, d.n_f0, (int32_t)bpb, (uint32_t)k, margin, c->sel, c->stream));
     c->counters.kernel_launches += 1;
+    // Phase B: the whole bank through the fused filter.  If a band's buffer overflows (a region far
+    // louder than the sample suggested), tighten its threshold from the entries kept and repeat.
+    for (int attempt = 0;; ++attempt) {
+      rc = run_stat(c, sel_stat, 0, d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb);
+      if (rc != FT_OK) return rc;
+      FT_CUDA(c, cudaMemcpyAsync(cnt.data(), c->sel.cnt, sizeof(uint32_t) * n_bands, cudaMemcpyDeviceToHost, c->stream));
+      FT_CUDA(c, cudaStreamSynchronize(c->stream));
+      uint32_t worst = 0;
+      for (uint32_t v : cnt) worst = std::max(worst, v);
+      if (worst <= c->sel.cap) break;
+      if (attempt == 3) return fail(c, FT_ERR_STATE, "ft_topk_per_band: a band's candidate buffer keeps overflowing (too many exact ties at the k-th value)");
+      c->counters.refine_fallbacks += 1;
+      FT_CUDA(c, ft_select_tighten(c->sel, (uint32_t)k, margin, c->stream));
+      FT_CUDA(c, cudaMemsetAsync(c->sel.cnt, 0, sizeof(uint32_t) * n_bands, c->stream));
+      c->counters.kernel_launches += 1;
+    }
+  } else {
+    // full write-out in chunks of <= 512 MB; every chunk tightens the thresholds with its own k-th
+    // largest (a valid lower bound of the band's), then appends what passes
+    uint64_t chunk_pts = ((uint64_t)1 << 27) / (uint64_t)d.n_f0;
+    chunk_pts = chunk_pts < 1 ? 1 : (chunk_pts > d.n_points ? d.n_points : chunk_pts);
+    rc = ensure_scratch(c, (size_t)chunk_pts * d.n_f0, by_count);
+    if (rc != FT_OK) return rc;
+    for (uint64_t pt = 0; pt < d.n_points; pt += chunk_pts) {
+      const uint64_t pe = (pt + chunk_pts < d.n_points) ? pt + chunk_pts : d.n_points;
+      rc = run_stat(c, sel_stat, pt, pe, by_count ? nullptr : c->scratch_f, by_count ? c->scratch_i : nullptr,
+                    pt * (uint64_t)d.n_f0, false, (int32_t)bpb);
+      if (rc != FT_OK) return rc;
+      const int64_t rows = (int64_t)(pe - pt);
+      if (by_count) { FT_CUDA(c, ft_count_to_key(c->scratch_i, c->scratch_f, rows * d.n_f0, c->stream)); c->counters.kernel_launches += 1; }
+      FT_CUDA(c, ft_select_threshold(c->scratch_f, rows, d.n_f0, (int32_t)bpb, (uint32_t)k, margin, c->sel, c->stream));
+      FT_CUDA(c, ft_select_append_keys(c->scratch_f, rows, d.n_f0, (int32_t)bpb, pt, c->sel, c->stream));
+      c->counters.kernel_launches += 2;
+    }
   }
   FT_CUDA(c, ft_select_trim(c->sel, (uint32_t)k, margin, c->final_idx, c->final_band, c->final_n, c->final_cap, overflow, c->stream));
   FT_CUDA(c, ft_launch_refine(d, c->final_idx, c->final_n, c->final_cap, c->cand, c->near_ties_dev, c->stream));
@@ -405,7 +443,6 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
   c->counters.kernel_launches += 3;
   uint32_t fin[2] = {0, 0};
   FT_CUDA(c, cudaMemcpyAsync(fin, c->final_n, sizeof fin, cudaMemcpyDeviceToHost, c->stream));
-  std::vector<uint32_t> cnt(n_bands);
   FT_CUDA(c, cudaMemcpyAsync(cnt.data(), c->sel.cnt, sizeof(uint32_t) * n_bands, cudaMemcpyDeviceToHost, c->stream));
   static_assert(sizeof(ft_cand) == sizeof(FtCandDev), "ft_cand layout");
   FT_CUDA(c, cudaMemcpyAsync(out_host, c->out_dev, sizeof(ft_cand) * (size_t)n_bands * k, cudaMemcpyDeviceToHost, c->stream));
@@ -463,6 +500,7 @@ int ft_get_counters(ft_ctx* c, ft_counters* out) {
 }
 
 const char* ft_last_error(const ft_ctx* c) { return c ? c->err.c_str() : "null handle"; }
+const char* ft_describe(const ft_ctx* c) { return c ? c->desc.c_str() : "null handle"; }
 
 void ft_destroy(ft_ctx* c) {
   if (!c) return;

@@ -112,6 +112,20 @@ ft_trim_kernel(FtSelectDev sel, uint32_t k, float rel_margin, uint64_t* __restri
   }
 }
 
+// Overflow recovery: the k-th largest of the entries a band's buffer did keep is a valid lower bound
+// of the band's true k-th value; tighten the threshold with it (the pass is then repeated).
+__global__ void __launch_bounds__(SEL_THREADS)
+ft_tighten_kernel(FtSelectDev sel, uint32_t k, float rel_margin) {
+  __shared__ uint32_t hist[256];
+  __shared__ uint32_t bcast[2];
+  const int b = blockIdx.x;
+  const uint32_t n = min(sel.cnt[b], sel.cap);
+  const float* keys = sel.key + (size_t)b * sel.cap;
+  auto get = [&](int64_t e) { return keys[e]; };
+  const uint32_t kk = block_kth_largest((int64_t)n, k, get, hist, bcast);
+  if (threadIdx.x == 0 && n >= k) sel.thr[b] = fmaxf(sel.thr[b], apply_margin(ft_unkey(kk), rel_margin));
+}
+
 // Per band: rank the refined candidates under (value desc, idx asc); ranks < k go to out[b][rank].
 constexpr int RANK_CAP = 2048;
 __global__ void __launch_bounds__(SEL_THREADS)
@@ -217,5 +231,16 @@ cudaError_t ft_select_rank(const FtCandDev* cand, const int32_t* cand_band, cons
 cudaError_t ft_count_to_key(const int32_t* c, float* k, int64_t n, cudaStream_t s) {
   const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
   ft_count_to_key_kernel<<<grid, 256, 0, s>>>(c, k, n);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_select_tighten(FtSelectDev sel, uint32_t k, float rel_margin, cudaStream_t s) {
+  ft_tighten_kernel<<<sel.n_bands, SEL_THREADS, 0, s>>>(sel, k, rel_margin);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_fill_f32(float* p, int64_t n, float v, cudaStream_t s) {
+  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  ft_fill_f32_kernel<<<grid, 256, 0, s>>>(p, n, v);
   return cudaGetLastError();
 }

@@ -31,3 +31,5 @@ cudaError_t ft_select_rank(const FtCandDev* cand, const int32_t* cand_band, cons
                            uint32_t cap, int by_count, uint32_t k, int32_t n_bands, FtCandDev* out,
                            uint32_t* overflow, cudaStream_t s);
 cudaError_t ft_count_to_key(const int32_t* c, float* k, int64_t n, cudaStream_t s);
+cudaError_t ft_select_tighten(FtSelectDev sel, uint32_t k, float rel_margin, cudaStream_t s);
+cudaError_t ft_fill_f32(float* p, int64_t n, float v, cudaStream_t s);

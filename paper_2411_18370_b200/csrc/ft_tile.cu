@@ -11,8 +11,8 @@
 // whole track of the warp for that SFT.  The break is located with the canonical arithmetic itself
 // (estimate, verify, bisect), so bins are bit-identical to the plain definition except within 1e-9
 // bin of a rounding tie (counted).  The main loop is then, per SFT, one shuffle (the lane's packed
-// entry) and J x (LDS.32 + FADD): a gather from shared memory, fp32 accumulation in two levels
-// (32-SFT partial sums, then totals).  Weights are folded into the gathered array beforehand
+// entry) and J x (LDS.32 + FADD): a gather from shared memory, fp32 accumulation over the centred
+// array.  Weights are folded into the gathered array beforehand
 // (Q = w P, or the 0/1 hit map for the number count), so both statistics are the same kernel.
 #include <algorithm>
 #include <cmath>
@@ -65,6 +65,7 @@ struct FtTileArgs {
   FtSelectDev sel;
   int32_t has_sel, bpb;
   unsigned long long* near_ties;
+  uint32_t group_stride;  // > 1: every stride-th group only (threshold sample), outputs packed by launch-local row
 };
 
 // Threads per CTA the kernel is compiled for: (consumer warps + 1 producer warp) * 32.  The
@@ -139,7 +140,8 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_cw = a.R * a.wpp;
   const int tile = (int)(blockIdx.x % (unsigned)a.n_tiles);
-  const uint64_t group = blockIdx.x / (unsigned)a.n_tiles;
+  const uint64_t group_l = blockIdx.x / (unsigned)a.n_tiles;  // launch-local group
+  const uint64_t group = group_l * a.group_stride;
   const int n_sft = (int)d.n_sft;
   const int NS = a.n_stages;
   float* ring = reinterpret_cast<float*>(smem_raw);
@@ -261,9 +263,11 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
     if (ii < warp_n) {
       const int64_t i = i_first + ii;
       const uint64_t idx = pt * (uint64_t)d.n_f0 + (uint64_t)i;
+      const uint64_t o = a.group_stride > 1 ? (group_l * (uint64_t)a.R + (uint64_t)r_pt) * (uint64_t)d.n_f0 + (uint64_t)i
+                                            : idx - a.out_base;
       const float v = (float)((double)acc[j] + a.add_back);
-      if (a.out_f) a.out_f[idx - a.out_base] = v;
-      if (a.out_i) a.out_i[idx - a.out_base] = __float2int_rn(v);
+      if (a.out_f) a.out_f[o] = v;
+      if (a.out_i) a.out_i[o] = __float2int_rn(v);
       if (a.has_sel) {
         const int band = (int)(i / a.bpb);
         if (v >= __ldg(a.sel.thr + band)) ft_select_append(a.sel, band, v, idx);
@@ -457,8 +461,12 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   int ctas = std::min(4, std::min(2048 / threads, 65536 / (threads * regs_est)));
   ctas = std::max(ctas, 1);
   const size_t row_bytes = (size_t)pl.pitch * 4;
-  const size_t budget = (size_t)(228 * 1024) / ctas - 2048;
-  int64_t rows_fit = (int64_t)((budget - 1024) / row_bytes);
+  int64_t rows_fit = 0;
+  for (;; --ctas) {  // fewer CTAs per SM until the ring holds two stages
+    const size_t budget = (size_t)(228 * 1024) / ctas - 2048;
+    rows_fit = (int64_t)((budget - 1024) / row_bytes);
+    if (rows_fit >= 2 * kRPS || ctas == 1) break;
+  }
   if (rows_fit < 2 * kRPS) { *why = "strip does not fit shared memory twice"; return cudaSuccess; }
   rows_fit = std::min<int64_t>(rows_fit, 32);
   pl.rows_per_stage = kRPS;
@@ -485,7 +493,7 @@ uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points) {
 cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, double add_back, uint64_t pt_begin,
                            uint64_t pt_end, float* out_f, int32_t* out_i, uint64_t out_base,
                            const FtSelectDev* sel, int32_t bpb, unsigned long long* near_ties,
-                           cudaStream_t s, int* launches) {
+                           cudaStream_t s, int* launches, uint32_t group_stride, uint64_t n_groups_strided) {
   *launches = 0;
   if (pt_end <= pt_begin) return cudaSuccess;
   FtTileArgs a{};
@@ -497,8 +505,16 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* 
   if (sel) { a.sel = *sel; a.has_sel = 1; }
   a.bpb = bpb > 0 ? bpb : 1;
   a.near_ties = near_ties;
+  a.group_stride = group_stride > 1 ? group_stride : 1;
   const unsigned block = (unsigned)((plan.R * plan.wpp + 1) * 32);
   const uint64_t max_groups = 0x7fffffffull / (uint64_t)plan.n_tiles;
+  if (a.group_stride > 1) {  // strided sample: one launch, n_groups_strided groups
+    if (n_groups_strided == 0 || n_groups_strided > max_groups) return cudaErrorInvalidValue;
+    a.pt_begin = pt_begin; a.pt_end = pt_end;
+    const cudaError_t e = launch_any(plan.J, d, a, (unsigned)(n_groups_strided * plan.n_tiles), block, plan.smem_bytes, s);
+    if (e == cudaSuccess) *launches = 1;
+    return e;
+  }
   uint64_t pt = pt_begin;
   while (pt < pt_end) {
     uint64_t groups = (pt_end - pt + plan.R - 1) / plan.R;

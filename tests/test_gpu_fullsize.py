@@ -1,0 +1,141 @@
+"""-m gpu: parity at BASELINE.json's FULL sizes (configs 2-4) in the launch configuration bench.py
+times (auto kernel choice = tile kernel K2, fused top-k), on outputs the oracle can compute one by
+one, plus properties that hold at any size; and the tile kernel's geometry edge cases (several f0
+tiles, ragged tails, every points-per-CTA value class) at sizes the oracle finishes in seconds."""
+import numpy as np
+import pytest
+
+from oracle import ft_oracle as fo
+from paper_2411_18370_b200 import workloads as W
+
+import ft_helpers as H
+
+pytestmark = pytest.mark.gpu
+PAD = np.uint64(2 ** 64 - 1)
+
+
+def _full(cfg):
+    return H.apply_injections({2: W.config2, 3: W.config3, 4: W.config4}[cfg]())
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_full_size_sampled_outputs_and_candidates(cfg):
+    import torch
+    wl = _full(cfg)
+    g = wl.grid
+    o = fo.Oracle(wl)
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    ctx = H.gpu_context(wl)                       # kernel auto, fused top-k: what bench.py runs
+    stat = "both" if wl.stat == "both" else "power"
+    gp, gc = H.gpu_full(ctx, wl, stat=stat)
+    assert "K2 tile kernel" in ctx.describe()
+    # (a) sampled templates, one by one against the oracle (plus every injected template)
+    rng = np.random.Generator(np.random.PCG64(100 + cfg))
+    idx = rng.integers(0, g.n_templates, 4096).astype(np.uint64)
+    inj = [int(g.ravel(*t)) for t, _ in wl.planned_injections]
+    idx = np.unique(np.concatenate([idx, np.array(inj, dtype=np.uint64)]))
+    op, oc, _, otie = o.eval_list(idx)
+    j = idx.astype(np.int64)
+    ok = otie == 0
+    rel = np.abs(gp[j].astype(np.float64) - op) / op
+    assert rel[ok].max() <= H.POWER_RTOL, f"max rel power error {rel[ok].max():.3e}"
+    if gc is not None:
+        assert np.array_equal(gc[j][ok], oc[ok])
+    # (b) candidates: every one re-evaluated by the oracle, bit-identical value, total order
+    ctx.eval(g, wl.stat, wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    assert cands.shape == (n_bands, wl.k) and np.all(cands["idx"] != PAD)
+    flat = cands.reshape(-1)
+    cp, cc, cw, _ = o.eval_list(flat["idx"])
+    assert np.array_equal(flat["power"], cp) and np.array_equal(flat["count"], cc)
+    assert np.array_equal(flat["wcount"], cw)
+    for b in range(n_bands):
+        c = cands[b]
+        assert np.all((c["idx"] % np.uint64(g.n_f0)).astype(np.int64) // bpb == b)
+        key = list(zip(-c["power"], c["idx"]))
+        assert key == sorted(key), f"band {b} not in (value desc, idx asc) order"
+    # (c) nothing louder was missed: exact per-band top-k of the GPU's own full fp32 array
+    full = torch.from_numpy(gp).cuda().view(-1, g.n_f0)
+    for b in range(n_bands):
+        blk = full[:, b * bpb:(b + 1) * bpb]
+        v, pos = torch.topk(blk.reshape(-1), wl.k)
+        kth = float(cands[b]["power"][-1])
+        w = blk.shape[1]
+        tid = (pos // w) * g.n_f0 + b * bpb + (pos % w)
+        must = tid[v.double() > kth * (1 + 2e-5)].cpu().numpy().astype(np.uint64)
+        assert np.isin(must, cands[b]["idx"]).all(), f"band {b}: a louder template is missing"
+        assert float(v[-1]) >= kth * (1 - 2e-5)
+    # the loudest injected signal of a band is that band's rank-1 candidate (config 3: amplitudes
+    # 0.5-3 against a noise maximum of ~1 + 5/sqrt(n_sft))
+    loudest = {}
+    for (t, amp) in wl.planned_injections:
+        b = t[5] // bpb
+        if b not in loudest or amp > loudest[b][1]:
+            loudest[b] = (int(g.ravel(*t)), amp)
+    for b, (tid, _) in loudest.items():
+        assert int(cands[b, 0]["idx"]) == tid, f"band {b}: injection not at rank 1"
+    ctx.close()
+
+
+def test_config3_ranked_by_count_full_size():
+    wl = _full(3)
+    g = wl.grid
+    o = fo.Oracle(wl)
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    ctx = H.gpu_context(wl)
+    ctx.eval(g, "hough", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    flat = cands.reshape(-1)
+    cp, cc, _, _ = o.eval_list(flat["idx"])
+    assert np.array_equal(flat["count"], cc) and np.array_equal(flat["power"], cp)
+    for b in range(n_bands):
+        key = list(zip(-cands[b]["count"].astype(np.int64), cands[b]["idx"]))
+        assert key == sorted(key)
+    ctx.close()
+
+
+GEOMETRY = [
+    # (n_f0 via band_hz at T_SFT = 1800, n_sft, n_sky, points per CTA)
+    (1.3, 77, 3, 0),     # 2340 f0 -> two f0 tiles, ragged last chunk, n_sft not a multiple of 4 or 32
+    (1.3, 33, 4, 1),     # one point per CTA
+    (0.35, 130, 9, 4),   # 630 f0, groups of 4 with a ragged last group (45 points)
+    (0.02, 64, 2, 0),    # 36 f0: two chunks, second ragged
+    (2.4, 40, 2, 3),     # 4320 f0: three tiles
+]
+
+
+@pytest.mark.parametrize("band_hz,n_sft,n_sky,ppc", GEOMETRY)
+def test_tile_geometry_edge_cases(band_hz, n_sft, n_sky, ppc):
+    wl = W.config2(n_sft=n_sft, n_sky=n_sky, band_hz=band_hz, band_width=0.01, k=3)
+    o = fo.Oracle(wl)
+    op, oc, _, otie = o.eval_range()
+    ctx = H.gpu_context(wl, kernel=2, ppc=ppc)     # tile kernel forced: ineligible would raise
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    H.assert_full_parity(wl, gp, gc, op, oc, otie)
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    ctx.eval(wl.grid, "power", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    H.assert_topk_parity(wl, cands, op, op, oc, wl.k, bpb)
+    ctx.close()
+
+
+def test_generic_kernel_when_f0_step_differs_from_bin_width():
+    """df0 = df/2 (a finer f0 grid than Eq. A1): not tileable, runs K0; forcing K2 is an error."""
+    from paper_2411_18370_b200 import binding as B
+    wl = W.config1()
+    g = wl.grid
+    fine = W.Grid(f0_start=g.f0_start, df0=g.df0 / 2, n_f0=2 * g.n_f0 - 1, sky=g.sky)
+    wl2 = W.Workload("fine", 1, wl.P, wl.t_mid, wl.vel, wl.w, wl.f_min, wl.df, fine, "both", 1.6,
+                     18 * fine.df0, 4, wl.T_sft)
+    op, oc, _, otie = fo.Oracle(wl2).eval_range()
+    ctx = H.gpu_context(wl2)
+    gp, gc = H.gpu_full(ctx, wl2, stat="both")
+    assert "K0" in ctx.describe()
+    H.assert_full_parity(wl2, gp, gc, op, oc, otie)
+    cands = ctx.topk_per_band(wl2.band_width, wl2.k, -(-fine.n_f0 // 18))
+    H.assert_topk_parity(wl2, cands, op, op, oc, wl2.k, 18)
+    ctx.set_option(B.FT_OPT_KERNEL, 2)
+    with pytest.raises(B.FtError) as e:
+        ctx.eval(fine, "power", 1.6)
+    assert e.value.code == -7
+    ctx.close()
