@@ -24,6 +24,7 @@ struct ft_ctx {
   float H_rho = 0.f; bool H_valid = false;
   double add_back = 0.0;        // sum over SFTs of the per-row constant the fold removed from Q
   double* axes_dev = nullptr;   // sky | a_p | P_orb | tasc
+  double* ctab_dev = nullptr;   // orbital cosine table of the bound grid (binary grids)
   // host copies used for validation
   std::vector<double> t_mid, vel;
   double vmax = 0.0, dt_min = 0.0, dt_max = 0.0;
@@ -141,7 +142,8 @@ void tock(ft_ctx* c, int launches) {
 // Statistic over points [pt_begin, pt_end): full write-out (out_* indexed from out_base) and/or
 // fused filter into c->sel.  Chooses the tile or the generic kernel.
 int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out_power, int32_t* out_count,
-             uint64_t out_base, bool filter, int32_t bpb, uint32_t stride = 1, uint64_t n_strided = 0) {
+             uint64_t out_base, bool filter, int32_t bpb, uint32_t stride = 1, uint64_t n_strided = 0,
+             bool complement = false) {
   const bool use_tile = c->tile_ok && c->opt_kernel != 1;
   if (use_tile) {
     // one gather-reduce pass per statistic: power over Q, number count over the hit map
@@ -150,13 +152,13 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
     if (stat != FT_STAT_HOUGH && (out_power || (filter && stat == FT_STAT_POWER))) {
       tick(c);
       FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.Q, c->add_back, pt_begin, pt_end, out_power, nullptr, out_base,
-                                stat == FT_STAT_POWER ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches, stride, n_strided));
+                                stat == FT_STAT_POWER ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches, stride, n_strided, complement));
       tock(c, launches);
     }
     if (stat != FT_STAT_POWER && (out_count || (filter && stat == FT_STAT_HOUGH))) {
       tick(c);
       FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.H, 0.0, pt_begin, pt_end, nullptr, out_count, out_base,
-                                stat == FT_STAT_HOUGH ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches, stride, n_strided));
+                                stat == FT_STAT_HOUGH ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches, stride, n_strided, complement));
       tock(c, launches);
     }
   } else {
@@ -315,6 +317,16 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   d.rho = (float)rho_th;
   d.n_points = (uint64_t)g->n_sky * g->n_ap * g->n_porb * g->n_tasc * g->n_f1;
   c->stat = stat;
+  // binary grids: cos(Om (t - t_asc)) per (P_orb, t_asc, SFT) once, shared by every a_p (<= 1 GiB)
+  dfree(c->ctab_dev);
+  d.ctab = nullptr;
+  const size_t ctab_elems = (size_t)g->n_porb * g->n_tasc * (size_t)d.n_sft;
+  if (ap_max != 0.0 && g->n_porb * (int64_t)g->n_tasc <= 65535 && ctab_elems <= ((size_t)1 << 27)) {
+    FT_CUDA(c, cudaMalloc(&c->ctab_dev, sizeof(double) * ctab_elems));
+    FT_CUDA(c, ft_launch_ctab(d, c->ctab_dev, c->stream));
+    c->counters.kernel_launches += 1;
+    d.ctab = c->ctab_dev;
+  }
   // tile-kernel eligibility and plan
   c->tile_ok = false;
   if (c->opt_kernel != 1) {
@@ -402,10 +414,15 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
     if (by_count) { FT_CUDA(c, ft_count_to_key(c->scratch_i, c->scratch_f, rows * d.n_f0, c->stream)); c->counters.kernel_launches += 1; }
     FT_CUDA(c, ft_select_threshold(c->scratch_f, rows, d.n_f0, (int32_t)bpb, (uint32_t)k, margin, c->sel, c->stream));
     c->counters.kernel_launches += 1;
-    // Phase B: the whole bank through the fused filter.  If a band's buffer overflows (a region far
-    // louder than the sample suggested), tighten its threshold from the entries kept and repeat.
+    // Phase B: the sample's own survivors from the scratch array, the rest of the bank through the
+    // fused filter.  If a band's buffer overflows (a region far louder than the sample suggested),
+    // tighten its threshold from the entries kept and repeat.
     for (int attempt = 0;; ++attempt) {
-      rc = run_stat(c, sel_stat, 0, d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb);
+      FT_CUDA(c, ft_select_append_keys(c->scratch_f, rows, d.n_f0, (int32_t)bpb, 0, c->sel, c->stream, (uint32_t)R,
+                                       (uint32_t)stride, d.n_points));
+      c->counters.kernel_launches += 1;
+      if (stride > 1) rc = run_stat(c, sel_stat, 0, d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb, (uint32_t)stride, n_sg, true);
+      else rc = run_stat(c, sel_stat, std::min<uint64_t>(d.n_points, (uint64_t)rows), d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb);
       if (rc != FT_OK) return rc;
       FT_CUDA(c, cudaMemcpyAsync(cnt.data(), c->sel.cnt, sizeof(uint32_t) * n_bands, cudaMemcpyDeviceToHost, c->stream));
       FT_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -507,7 +524,7 @@ void ft_destroy(ft_ctx* c) {
   cudaStreamSynchronize(c->stream);
   free_select(c);
   ft_tile_plan_free(&c->plan);
-  dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->H_dev); dfree(c->axes_dev);
+  dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->H_dev); dfree(c->ctab_dev); dfree(c->axes_dev);
   dfree(c->scratch_f); dfree(c->scratch_i); dfree(c->near_ties_dev);
   for (cudaEvent_t e : c->evs) cudaEventDestroy(e);
   delete c;

@@ -19,6 +19,7 @@ struct FtDev {
   const double* a_p;    // [n_ap]
   const double* P_orb;  // [n_porb]
   const double* tasc;   // [n_tasc]
+  const double* ctab;   // [n_porb*n_tasc][n_sft] cos(Om (t_mid - t_asc)) or nullptr (binary grids, bind time)
   int64_t n_sft, n_bins, ld;
   int64_t n_f0, n_sky;
   int32_t n_f1, n_ap, n_porb, n_tasc;
@@ -35,6 +36,7 @@ struct FtPoint {
   double Om;     // 2 pi / P_orb
   double t_asc;  // t_ref + u * P_orb
   double f1;
+  const double* crow;  // row of ctab for this (P_orb, t_asc), or nullptr
   bool binary;   // a_p != 0
 };
 
@@ -51,6 +53,7 @@ __device__ __forceinline__ FtPoint ft_decode_point(const FtDev& d, uint64_t pt) 
   p.t_asc = __dadd_rn(d.t_ref, __dmul_rn(d.tasc[i_ta], P_orb));
   p.apOm = __dmul_rn(a_p, p.Om);
   p.binary = (a_p != 0.0);
+  p.crow = d.ctab ? d.ctab + ((size_t)i_po * (size_t)d.n_tasc + i_ta) * (size_t)d.n_sft : nullptr;
   p.f1 = __dadd_rn(d.f1_start, __dmul_rn((double)i_f1, d.df1));
   return p;
 }
@@ -60,7 +63,7 @@ __device__ __forceinline__ double ft_doppler(const FtDev& d, const FtPoint& p, i
   const double vx = d.vel[3 * a + 0], vy = d.vel[3 * a + 1], vz = d.vel[3 * a + 2];
   const double V = __ddiv_rn(__dadd_rn(__dadd_rn(__dmul_rn(vx, p.nx), __dmul_rn(vy, p.ny)), __dmul_rn(vz, p.nz)), FT_C_LIGHT);
   double B = 0.0;
-  if (p.binary) B = __dmul_rn(p.apOm, cos(__dmul_rn(p.Om, __dsub_rn(t, p.t_asc))));
+  if (p.binary) B = __dmul_rn(p.apOm, p.crow ? p.crow[a] : cos(__dmul_rn(p.Om, __dsub_rn(t, p.t_asc))));
   return __dsub_rn(__dadd_rn(1.0, V), B);
 }
 
@@ -102,3 +105,5 @@ cudaError_t ft_launch_generic(const FtDev& d, int stat, uint64_t pt_begin, uint6
 cudaError_t ft_launch_refine(const FtDev& d, const uint64_t* idx_dev, const uint32_t* n_dev, int64_t n_max,
                              FtCandDev* out, unsigned long long* near_ties, cudaStream_t s);
 cudaError_t ft_launch_fold(const float* P, const float* w, float* Q, int64_t n, cudaStream_t s);
+// ctab[(i_porb*n_tasc + i_tasc)][a] = cos(Om (t_mid[a] - t_asc)), the same expression ft_doppler evaluates
+cudaError_t ft_launch_ctab(const FtDev& d, double* ctab, cudaStream_t s);

@@ -117,7 +117,25 @@ __global__ void ft_fold_kernel(const float* __restrict__ P, const float* __restr
     Q[i] = __fmul_rn(w[i], P[i]);
 }
 
+// A1 hoisted to bind time for binary grids: the orbital cosine depends on (P_orb, t_asc, SFT) only,
+// so the 64 a_p values of config 3 share it (Eq. 2; separability noted at :600).
+__global__ void ft_ctab_kernel(const __grid_constant__ FtDev d, double* __restrict__ ctab) {
+  const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t row = blockIdx.y;  // i_porb * n_tasc + i_tasc
+  if (a >= d.n_sft) return;
+  const double P_orb = d.P_orb[row / (uint32_t)d.n_tasc];
+  const double Om = __ddiv_rn(FT_TWO_PI, P_orb);
+  const double t_asc = __dadd_rn(d.t_ref, __dmul_rn(d.tasc[row % (uint32_t)d.n_tasc], P_orb));
+  ctab[(size_t)row * (size_t)d.n_sft + a] = cos(__dmul_rn(Om, __dsub_rn(d.t_mid[a], t_asc)));
+}
+
 }  // namespace
+
+cudaError_t ft_launch_ctab(const FtDev& d, double* ctab, cudaStream_t s) {
+  const dim3 grid((unsigned)((d.n_sft + 255) / 256), (unsigned)(d.n_porb * d.n_tasc));
+  ft_ctab_kernel<<<grid, 256, 0, s>>>(d, ctab);
+  return cudaGetLastError();
+}
 
 cudaError_t ft_launch_generic(const FtDev& d, int stat, uint64_t pt_begin, uint64_t pt_end,
                               float* out_power, int32_t* out_count, uint64_t out_base_idx,

@@ -70,15 +70,19 @@ ft_band_threshold_kernel(const float* __restrict__ keys, int64_t n_rows, int64_t
 }
 
 // Append every key >= thr[band] of a [n_rows][n_f0] key array (rows = points pt_begin + r).
+// Row r of the key array is outer point pt_begin + (r / R) * stride * R + r % R (stride = 1: contiguous).
 __global__ void ft_append_from_keys_kernel(const float* __restrict__ keys, int64_t n_rows, int64_t n_f0,
-                                           int32_t bpb, uint64_t pt_begin, FtSelectDev sel) {
+                                           int32_t bpb, uint64_t pt_begin, uint32_t R, uint32_t gstride,
+                                           uint64_t pt_end, FtSelectDev sel) {
   const int64_t n = n_rows * n_f0;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
     const int64_t c = e % n_f0;
     const int b = (int)(c / bpb);
     const float v = keys[e];
-    if (v >= sel.thr[b]) ft_select_append(sel, b, v, (pt_begin + (uint64_t)(e / n_f0)) * (uint64_t)n_f0 + (uint64_t)c);
+    const uint64_t r = (uint64_t)(e / n_f0);
+    const uint64_t pt = pt_begin + (r / R) * (uint64_t)gstride * R + r % R;
+    if (pt < pt_end && v >= sel.thr[b]) ft_select_append(sel, b, v, pt * (uint64_t)n_f0 + (uint64_t)c);
   }
 }
 
@@ -207,10 +211,11 @@ cudaError_t ft_select_threshold(const float* keys, int64_t n_rows, int64_t n_f0,
 }
 
 cudaError_t ft_select_append_keys(const float* keys, int64_t n_rows, int64_t n_f0, int32_t bpb,
-                                  uint64_t pt_begin, FtSelectDev sel, cudaStream_t s) {
+                                  uint64_t pt_begin, FtSelectDev sel, cudaStream_t s, uint32_t R, uint32_t stride,
+                                  uint64_t pt_end) {
   const int64_t n = n_rows * n_f0;
   const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
-  ft_append_from_keys_kernel<<<grid, 256, 0, s>>>(keys, n_rows, n_f0, bpb, pt_begin, sel);
+  ft_append_from_keys_kernel<<<grid, 256, 0, s>>>(keys, n_rows, n_f0, bpb, pt_begin, R ? R : 1, stride ? stride : 1, pt_end, sel);
   return cudaGetLastError();
 }
 

@@ -23,7 +23,8 @@ cudaError_t ft_select_reset(FtSelectDev sel, uint32_t* final_n, uint32_t* overfl
 cudaError_t ft_select_threshold(const float* keys, int64_t n_rows, int64_t n_f0, int32_t bpb, uint32_t k,
                                 float rel_margin, FtSelectDev sel, cudaStream_t s);
 cudaError_t ft_select_append_keys(const float* keys, int64_t n_rows, int64_t n_f0, int32_t bpb,
-                                  uint64_t pt_begin, FtSelectDev sel, cudaStream_t s);
+                                  uint64_t pt_begin, FtSelectDev sel, cudaStream_t s, uint32_t R = 1,
+                                  uint32_t stride = 1, uint64_t pt_end = ~0ull);
 cudaError_t ft_select_trim(FtSelectDev sel, uint32_t k, float rel_margin, uint64_t* final_idx,
                            int32_t* final_band, uint32_t* final_n, uint32_t final_cap,
                            uint32_t* overflow, cudaStream_t s);

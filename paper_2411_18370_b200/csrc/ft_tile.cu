@@ -66,10 +66,14 @@ struct FtTileArgs {
   int32_t has_sel, bpb;
   unsigned long long* near_ties;
   uint32_t group_stride;  // > 1: every stride-th group only (threshold sample), outputs packed by launch-local row
+  uint32_t skip_stride;   // > 1: every group EXCEPT the first skip_n multiples of skip_stride (the rest of the bank)
+  uint64_t skip_n;
 };
 
 // Threads per CTA the kernel is compiled for: (consumer warps + 1 producer warp) * 32.  The
 // accumulators (J) and the loads in flight (J) set the register need, hence the bound.
+// (the register file is 4 x 16 384: 80 registers allow 6 warps per SM sub-partition, 64 allow 8)
+__host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 1024 : 768; }
 
 // Packed per-(warp, SFT) track entry: bits 0-12 strip offset of the warp's first output (floats),
@@ -134,14 +138,18 @@ __device__ __forceinline__ uint32_t ft_tile_entry(const FtDev& d, const FtPoint&
 }
 
 template <int J>
-__global__ void __launch_bounds__(ft_tile_max_threads(J), 1)
+__global__ void __maxnreg__(ft_tile_max_regs(J))
 ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_cw = a.R * a.wpp;
   const int tile = (int)(blockIdx.x % (unsigned)a.n_tiles);
   const uint64_t group_l = blockIdx.x / (unsigned)a.n_tiles;  // launch-local group
-  const uint64_t group = group_l * a.group_stride;
+  uint64_t group = group_l * a.group_stride;
+  if (a.skip_stride > 1) {
+    const uint64_t m = a.skip_stride - 1, nb = a.skip_n * m;
+    group = group_l < nb ? (group_l / m) * a.skip_stride + 1 + group_l % m : a.skip_n * a.skip_stride + (group_l - nb);
+  }
   const int n_sft = (int)d.n_sft;
   const int NS = a.n_stages;
   float* ring = reinterpret_cast<float*>(smem_raw);
@@ -194,7 +202,10 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
   uint64_t pt = a.pt_begin + group * (uint64_t)a.R + (uint64_t)r_pt;
   const bool pt_active = pt < a.pt_end;
   if (!pt_active) pt = a.pt_end - 1;  // keep the barrier protocol; results are discarded
-  const FtPoint p = ft_decode_point(d, pt);
+  // the point's parameters live in shared memory (17 registers less across the main loop)
+  FtPoint* sp = reinterpret_cast<FtPoint*>(bars + 2 * NS) + warp;
+  if (lane == 0) *sp = ft_decode_point(d, pt);
+  __syncwarp();
   const int tile_i0 = tile * a.tile_w;
   const int wlo = sub * J * 32;                                        // warp's first output, tile-relative
   const int tile_n = min(a.tile_w, (int)d.n_f0 - tile_i0);             // valid f0 in this tile
@@ -213,7 +224,7 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
     // -- A1/A2: this lane's SFT ---------------------------------------------------------------------
     uint32_t entry = 0;
     if (a0 + lane < n_sft && warp_n > 0)
-      entry = ft_tile_entry(d, p, a0 + lane, kst[a0 + lane], i_first, warp_n, a.copy_floats, &ties, a.err);
+      entry = ft_tile_entry(d, *sp, a0 + lane, kst[a0 + lane], i_first, warp_n, a.copy_floats, &ties, a.err);
     // -- A4: gather + reduce over the block's SFTs -----------------------------------------------
     const int n_rows = min(32, n_sft - a0);
     for (int q = 0; q < n_rows; q += kRPS) {
@@ -472,7 +483,8 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   pl.rows_per_stage = kRPS;
   pl.n_stages = (int32_t)(rows_fit / kRPS);
   pl.ctas_per_sm = ctas;
-  pl.smem_bytes = (size_t)pl.n_stages * pl.rows_per_stage * row_bytes + 2 * 8 * (size_t)pl.n_stages;
+  pl.smem_bytes = (size_t)pl.n_stages * pl.rows_per_stage * row_bytes + 2 * 8 * (size_t)pl.n_stages +
+                  sizeof(FtPoint) * (size_t)(pl.R * pl.wpp);
   e = cudaMalloc(&pl.kst, sizeof(int32_t) * kst.size());
   if (e != cudaSuccess) return e;
   e = cudaMalloc(&pl.err, sizeof(int32_t));
@@ -493,7 +505,7 @@ uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points) {
 cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, double add_back, uint64_t pt_begin,
                            uint64_t pt_end, float* out_f, int32_t* out_i, uint64_t out_base,
                            const FtSelectDev* sel, int32_t bpb, unsigned long long* near_ties,
-                           cudaStream_t s, int* launches, uint32_t group_stride, uint64_t n_groups_strided) {
+                           cudaStream_t s, int* launches, uint32_t group_stride, uint64_t n_groups_strided, bool complement) {
   *launches = 0;
   if (pt_end <= pt_begin) return cudaSuccess;
   FtTileArgs a{};
@@ -505,13 +517,18 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* 
   if (sel) { a.sel = *sel; a.has_sel = 1; }
   a.bpb = bpb > 0 ? bpb : 1;
   a.near_ties = near_ties;
-  a.group_stride = group_stride > 1 ? group_stride : 1;
+  a.group_stride = (group_stride > 1 && !complement) ? group_stride : 1;
+  a.skip_stride = (group_stride > 1 && complement) ? group_stride : 1;
+  a.skip_n = n_groups_strided;
   const unsigned block = (unsigned)((plan.R * plan.wpp + 1) * 32);
   const uint64_t max_groups = 0x7fffffffull / (uint64_t)plan.n_tiles;
-  if (a.group_stride > 1) {  // strided sample: one launch, n_groups_strided groups
-    if (n_groups_strided == 0 || n_groups_strided > max_groups) return cudaErrorInvalidValue;
+  if (group_stride > 1) {  // strided sample (or its complement): one launch
+    const uint64_t all_groups = (pt_end - pt_begin + plan.R - 1) / plan.R;
+    const uint64_t n_launch = complement ? all_groups - n_groups_strided : n_groups_strided;
+    if (n_groups_strided == 0 || n_groups_strided > all_groups || n_launch > max_groups) return cudaErrorInvalidValue;
+    if (n_launch == 0) return cudaSuccess;
     a.pt_begin = pt_begin; a.pt_end = pt_end;
-    const cudaError_t e = launch_any(plan.J, d, a, (unsigned)(n_groups_strided * plan.n_tiles), block, plan.smem_bytes, s);
+    const cudaError_t e = launch_any(plan.J, d, a, (unsigned)(n_launch * plan.n_tiles), block, plan.smem_bytes, s);
     if (e == cudaSuccess) *launches = 1;
     return e;
   }

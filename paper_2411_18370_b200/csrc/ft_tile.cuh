@@ -37,11 +37,12 @@ uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points);
 // Writes out_f (fp32) and/or out_i (int32) indexed from out_base, and/or
 // filters into sel (bands of bpb f0 bins).  group_stride > 1: evaluate only groups 0, stride, 2 stride, ...
 // (n_groups_strided of them; the threshold sample) and pack the outputs by launch-local row
-// (group_local * R + r) * n_f0 + i_f0.
+// (group_local * R + r) * n_f0 + i_f0.  complement = true: every group EXCEPT those (the rest of the bank).
 cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, double add_back, uint64_t pt_begin,
                            uint64_t pt_end, float* out_f, int32_t* out_i, uint64_t out_base,
                            const FtSelectDev* sel, int32_t bpb, unsigned long long* near_ties,
-                           cudaStream_t s, int* launches, uint32_t group_stride = 1, uint64_t n_groups_strided = 0);
+                           cudaStream_t s, int* launches, uint32_t group_stride = 1, uint64_t n_groups_strided = 0,
+                           bool complement = false);
 cudaError_t ft_launch_hitmap(const float* P, float rho, float* H, int64_t n, cudaStream_t s);
 // Q[a][k] = fl(fl(w P) - c_a) with c_a = fl(mean_k fl(w P)) per row; w_sft (per-SFT) or w_bin (per-bin).
 cudaError_t ft_launch_fold_centered(const float* P, const float* w_sft, const float* w_bin, float* Q, float* c_row,
