@@ -63,23 +63,23 @@ static void fto_unravel(const fto_problem* pb, uint64_t idx, int64_t ax[6]) {
   ax[0] = (int64_t)idx;
 }
 
+/* One explicit template lambda = (f0, f1, n, a_p, P_orb, t_asc): "no assumption on the properties of
+ * lambda"; random template banks are drawn this way. */
+typedef struct { double f0, f1, nx, ny, nz, a_p, P_orb, t_asc; } fto_template;
+
 /*
  * One template: track -> bin per SFT (Eq. 2), then the statistics (Eq. 3, Eq. 7).
  * k_out / x_out may be NULL.  Returns FTO_ERR_RANGE if any bin falls outside the spectrogram.
  */
-static int fto_one_template(const fto_problem* pb, uint64_t idx, double* power, int32_t* count,
-                            double* wcount, uint8_t* near_tie, int64_t* k_out, double* x_out) {
-  int64_t ax[6];
-  fto_unravel(pb, idx, ax);
+static int fto_one_params(const fto_problem* pb, const fto_template* tp, double t_ref, double* power,
+                          int32_t* count, double* wcount, uint8_t* near_tie, int64_t* k_out,
+                          double* x_out) {
   const double inv_df = 1.0 / pb->df;
-  const double f0 = pb->f0_start + (double)ax[5] * pb->df0;
-  const double f1 = pb->f1_start + (double)ax[4] * pb->df1;
-  const double nx = pb->sky[3 * ax[0] + 0], ny = pb->sky[3 * ax[0] + 1], nz = pb->sky[3 * ax[0] + 2];
-  const double a_p = pb->a_p[ax[1]];
-  const double P_orb = pb->P_orb[ax[2]];
-  const double u = pb->tasc_frac[ax[3]];
-  const double Om = TWO_PI / P_orb;              /* Omega */
-  const double t_asc = pb->t_ref + u * P_orb;    /* phi_b = t_asc * Omega */
+  const double f0 = tp->f0, f1 = tp->f1;
+  const double nx = tp->nx, ny = tp->ny, nz = tp->nz;
+  const double a_p = tp->a_p;
+  const double Om = TWO_PI / tp->P_orb;          /* Omega */
+  const double t_asc = tp->t_asc;                /* phi_b = t_asc * Omega */
   const float rho = (float)pb->rho_th;
 
   double s_power = 0.0, s_wcount = 0.0;
@@ -87,7 +87,7 @@ static int fto_one_template(const fto_problem* pb, uint64_t idx, double* power, 
   uint8_t tie = 0;
   for (int64_t a = 0; a < pb->n_sft; ++a) {
     const double t = pb->t_mid[a];
-    const double dt = t - pb->t_ref;
+    const double dt = t - t_ref;
     const double fs = f0 + f1 * dt;                               /* spun-down frequency */
     const double V = ((pb->vel[3 * a] * nx + pb->vel[3 * a + 1] * ny) + pb->vel[3 * a + 2] * nz) / C_LIGHT;
     double B = 0.0;                                               /* a_p = 0: isolated */
@@ -113,6 +113,21 @@ static int fto_one_template(const fto_problem* pb, uint64_t idx, double* power, 
   if (wcount) *wcount = s_wcount;
   if (near_tie) *near_tie = tie;
   return FTO_OK;
+}
+
+/* Grid template: canonical index -> parameters (f0 = f0_start + i df0, ..., t_asc = t_ref + u P_orb). */
+static int fto_one_template(const fto_problem* pb, uint64_t idx, double* power, int32_t* count,
+                            double* wcount, uint8_t* near_tie, int64_t* k_out, double* x_out) {
+  int64_t ax[6];
+  fto_unravel(pb, idx, ax);
+  fto_template tp;
+  tp.f0 = pb->f0_start + (double)ax[5] * pb->df0;
+  tp.f1 = pb->f1_start + (double)ax[4] * pb->df1;
+  tp.nx = pb->sky[3 * ax[0] + 0]; tp.ny = pb->sky[3 * ax[0] + 1]; tp.nz = pb->sky[3 * ax[0] + 2];
+  tp.a_p = pb->a_p[ax[1]];
+  tp.P_orb = pb->P_orb[ax[2]];
+  tp.t_asc = pb->t_ref + pb->tasc_frac[ax[3]] * tp.P_orb;
+  return fto_one_params(pb, &tp, pb->t_ref, power, count, wcount, near_tie, k_out, x_out);
 }
 
 /* Track of ONE template: bins k[n_sft] and positions x[n_sft]. */
@@ -148,6 +163,23 @@ int fto_eval_list(const fto_problem* pb, const uint64_t* idx, int64_t n, double*
     const int rc = fto_one_template(pb, idx[j], power ? power + j : NULL, count ? count + j : NULL,
                                     wcount ? wcount + j : NULL, near_tie ? near_tie + j : NULL,
                                     NULL, NULL);
+    if (rc != FTO_OK) {
+#pragma omp atomic write
+      status = rc;
+    }
+  }
+  return status;
+}
+
+/* Statistics of an explicit list of templates (an unstructured bank); t_ref is the reference
+ * time of f0 and f1.  The grid axes of pb are not used. */
+int fto_eval_templates(const fto_problem* pb, const fto_template* tl, int64_t n, double t_ref,
+                       double* power, int32_t* count, double* wcount, uint8_t* near_tie) {
+  int status = FTO_OK;
+#pragma omp parallel for schedule(static)
+  for (int64_t j = 0; j < n; ++j) {
+    const int rc = fto_one_params(pb, tl + j, t_ref, power ? power + j : NULL, count ? count + j : NULL,
+                                  wcount ? wcount + j : NULL, near_tie ? near_tie + j : NULL, NULL, NULL);
     if (rc != FTO_OK) {
 #pragma omp atomic write
       status = rc;

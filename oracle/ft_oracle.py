@@ -57,6 +57,7 @@ def _load():
         _lib.fto_track.restype = C.c_int
         _lib.fto_eval_range.restype = C.c_int
         _lib.fto_eval_list.restype = C.c_int
+        _lib.fto_eval_templates.restype = C.c_int
         _lib.fto_num_threads.restype = C.c_int
     return _lib
 
@@ -130,6 +131,22 @@ class Oracle:
         if rc != 0:
             raise ValueError(f"oracle: a track left the spectrogram (rc={rc})")
         return o
+
+
+TEMPLATE_DTYPE = np.dtype([("f0", "<f8"), ("f1", "<f8"), ("nx", "<f8"), ("ny", "<f8"), ("nz", "<f8"),
+                           ("a_p", "<f8"), ("P_orb", "<f8"), ("t_asc", "<f8")])
+
+
+def eval_templates(oracle: "Oracle", templates, t_ref: float):
+    """Unstructured bank: (power, count, wcount, near_tie) of an explicit
+    list of templates (TEMPLATE_DTYPE records) on the oracle's spectrogram; grid axes unused."""
+    tl = np.ascontiguousarray(templates, dtype=TEMPLATE_DTYPE)
+    o = oracle._outs(tl.size)
+    rc = oracle.lib.fto_eval_templates(C.byref(oracle.pb), tl.ctypes.data_as(C.c_void_p), C.c_int64(tl.size),
+                                       C.c_double(float(t_ref)), *[a.ctypes.data_as(C.c_void_p) for a in o])
+    if rc != 0:
+        raise ValueError(f"oracle: a track left the spectrogram (rc={rc})")
+    return o
 
 
 def topk_per_band(values, n_f0: int, bins_per_band: int, k: int, idx_begin: int = 0):

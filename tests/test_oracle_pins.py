@@ -377,3 +377,84 @@ def test_config1_injection_is_loudest_in_its_band():
     assert after[star] == pytest.approx(before[star] + amp * float(wl.w.astype(np.float64).sum()), rel=1e-6)  # fp32 pixels
     top = fo.topk_per_band(after, wl.grid.n_f0, 18, 5)
     assert int(top[90 // 18][0][0]) == star
+
+
+# ------------------------------------------------- unstructured banks (explicit template lists)
+def _explicit_from_grid(wl):
+    """Every grid template written out as an explicit (f0, f1, n, a_p, P_orb, t_asc) record, in
+    canonical order, by plain loops (no oracle code)."""
+    g = wl.grid
+    recs = []
+    for sky in g.sky:
+        for ap in g.a_p:
+            for Po in g.P_orb:
+                for u in g.tasc_frac:
+                    for j in range(g.n_f1):
+                        for i in range(g.n_f0):
+                            recs.append((g.f0_start + i * g.df0, g.f1_start + j * g.df1, sky[0], sky[1], sky[2],
+                                         ap, Po, g.t_ref + u * Po))
+    return np.array(recs, dtype=fo.TEMPLATE_DTYPE)
+
+
+def test_template_list_reproduces_the_grid_bit_for_bit():
+    """An explicit list that enumerates a product grid gives the grid's statistics exactly
+    (parameter mapping, t_asc = t_ref + u P_orb, index order)."""
+    g = dict(n_f0=9, f1_start=-1e-9, df1=1e-9, n_f1=2, sky=W.fibonacci_sphere(3),
+             a_p=np.array([0.0, 2.0]), P_orb=np.array([1.5]) * 86400.0, tasc_frac=np.array([0.25, 0.5]))
+    wl = _simple_workload(n_sft=23, n_bins=96, pad=40, grid_kw=g, n_f0=9)
+    wl.grid.f0_start, wl.grid.df0 = 100.0, wl.df
+    o = fo.Oracle(wl)
+    pw, ct, wc, tie = o.eval_range()
+    lp, lc, lw, lt = fo.eval_templates(o, _explicit_from_grid(wl), wl.grid.t_ref)
+    assert np.array_equal(lp, pw) and np.array_equal(lc, ct) and np.array_equal(lw, wc) and np.array_equal(lt, tie)
+
+
+def test_template_list_brute_force_off_grid_with_reference_time():
+    """Off-grid templates (random f0 between bins, random sky, binary parameters) and t_ref != 0,
+    against an independent Python loop.  Catches: t_ref used in the wrong place, t_asc treated as
+    a fraction, a swapped field of the record."""
+    wl = _simple_workload(n_sft=17, n_bins=96, pad=40, grid_kw={}, n_f0=4)
+    rng = np.random.Generator(np.random.PCG64(77))
+    n, t_ref = 40, 3000.0
+    tl = np.zeros(n, dtype=fo.TEMPLATE_DTYPE)
+    tl["f0"] = 100.0 + rng.random(n) * 10 * wl.df
+    tl["f1"] = -2e-9 * rng.random(n)
+    v = rng.normal(size=(n, 3)); v /= np.linalg.norm(v, axis=1, keepdims=True)
+    tl["nx"], tl["ny"], tl["nz"] = v[:, 0], v[:, 1], v[:, 2]
+    tl["a_p"] = np.where(rng.random(n) < 0.3, 0.0, 0.3 * rng.random(n))
+    tl["P_orb"] = (0.5 + 2.0 * rng.random(n)) * 86400.0
+    tl["t_asc"] = 1e5 * rng.random(n)
+    o = fo.Oracle(wl)
+    pw, ct, wc, _ = fo.eval_templates(o, tl, t_ref)
+    for q in range(n):
+        f0, f1, nx, ny, nz, ap, Po, tasc = (float(tl[q][k]) for k in fo.TEMPLATE_DTYPE.names)
+        Om = 6.283185307179586 / Po
+        s, c, sw = 0.0, 0, 0.0
+        for a in range(wl.n_sft):
+            t = float(wl.t_mid[a])
+            V = ((wl.vel[a, 0] * nx + wl.vel[a, 1] * ny) + wl.vel[a, 2] * nz) / 299792458.0
+            B = (ap * Om) * math.cos(Om * (t - tasc)) if ap != 0.0 else 0.0
+            x = (((f0 + f1 * (t - t_ref)) * ((1.0 + V) - B)) - wl.f_min) * (1.0 / wl.df)
+            k = round(x)
+            p = wl.P[a, k]
+            s += float(wl.w[a]) * float(p)
+            if p > np.float32(1.6):
+                c += 1
+                sw += float(wl.w[a])
+        assert pw[q] == s and ct[q] == c and wc[q] == sw, q
+
+
+def test_template_list_straight_line_is_a_column_sum():
+    """v = 0, a_p = 0, f1 = 0 at an OFF-grid f0: the track is the single column rint((f0 - f_min)/df)
+    and the statistic is the weighted sum of that column (a GEMV row)."""
+    wl = _simple_workload(n_sft=50, n_bins=64, pad=10, grid_kw={}, n_f0=4)
+    wl.vel[:] = 0.0
+    o = fo.Oracle(wl)
+    tl = np.zeros(3, dtype=fo.TEMPLATE_DTYPE)
+    tl["nz"], tl["P_orb"] = 1.0, 86400.0
+    tl["f0"] = wl.f_min + np.array([12.3, 12.7, 40.49]) * wl.df
+    pw, ct, _, _ = fo.eval_templates(o, tl, 0.0)
+    colsum = (wl.w.astype(np.float64)[:, None] * wl.P.astype(np.float64))
+    for q, col in enumerate([12, 13, 40]):
+        assert abs(pw[q] - colsum[:, col].sum()) <= 1e-12 * pw[q]
+        assert ct[q] == int((wl.P[:, col] > np.float32(1.6)).sum())
