@@ -140,6 +140,30 @@ int ft_topk_per_band(ft_ctx* ctx, double band_width_hz, int32_t k, ft_cand* out_
  */
 int ft_eval_list(ft_ctx* ctx, const uint64_t* idx_host, int64_t n, ft_cand* out_host);
 
+/*
+ * One explicit template lambda = (f0, f1, n, a_p, P_orb, t_asc): the unstructured-bank form of the
+ * problem ("no assumption on the properties of lambda", :213; random template banks :312-316).
+ */
+typedef struct {
+  double f0, f1;        /* Hz at t_ref, Hz/s                                   */
+  double nx, ny, nz;    /* unit vector n, equatorial Cartesian                 */
+  double a_p, P_orb;    /* light-seconds (0 = isolated), seconds (> 0 always)  */
+  double t_asc;         /* time of ascending node, seconds (absolute, not a fraction) */
+} ft_template;
+
+/*
+ * ft_eval_templates — statistic of every template of an explicit list (vmap s over an arbitrary
+ * bank, :213), by the canonical fp64 arithmetic per (template, SFT): kernel K1, bound by the fp64
+ * pipe.  Needs no bound grid and does not disturb one.
+ *   templates_dev [device] ft_template [n], borrowed until the call returns.
+ *   t_ref         reference time of f0 / f1, seconds.
+ *   stat, rho_th  as ft_eval.   out_power_dev [device] fp32 [n] or NULL; out_count_dev [device] int32 [n] or NULL.
+ * Synchronises the stream.  A track that leaves [0, n_bins) is an error, not a clamp: the call
+ * returns FT_ERR_TRACK_RANGE, that template's outputs are NaN / -1 and the others are valid.
+ */
+int ft_eval_templates(ft_ctx* ctx, const ft_template* templates_dev, int64_t n, double t_ref, int stat,
+                      double rho_th, float* out_power_dev, int32_t* out_count_dev);
+
 /* Options (ft_set_option): */
 typedef enum {
   FT_OPT_KERNEL = 0,        /* 0 auto (default), 1 force generic kernel, 2 force tile kernel (FT_ERR_UNSUPPORTED if ineligible) */

@@ -12,7 +12,7 @@ from . import build as _build
 
 FT_STAT = {"power": 0, "hough": 1, "both": 2}
 FT_OPT_KERNEL, FT_OPT_FUSED_TOPK, FT_OPT_POINTS_PER_CTA = 0, 1, 2
-SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_eval_list", "ft_set_option",
+SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_eval_list", "ft_eval_templates", "ft_set_option",
            "ft_get_counters", "ft_last_error", "ft_describe", "ft_destroy"]
 
 
@@ -33,6 +33,10 @@ class FtCand(C.Structure):
 
 CAND_DTYPE = np.dtype([("power", "<f8"), ("wcount", "<f8"), ("idx", "<u8"), ("count", "<i4"),
                        ("band", "<i4")])
+
+
+TEMPLATE_DTYPE = np.dtype([("f0", "<f8"), ("f1", "<f8"), ("nx", "<f8"), ("ny", "<f8"), ("nz", "<f8"),
+                           ("a_p", "<f8"), ("P_orb", "<f8"), ("t_asc", "<f8")])   # ft_template
 
 
 class FtCounters(C.Structure):
@@ -69,6 +73,9 @@ def load_library(path: str | None = None):
         lib.ft_topk_per_band.argtypes = [C.c_void_p, C.c_double, C.c_int32, C.c_void_p, C.POINTER(C.c_int32)]
         lib.ft_eval_list.restype = C.c_int
         lib.ft_eval_list.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+        lib.ft_eval_templates.restype = C.c_int
+        lib.ft_eval_templates.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int, C.c_double,
+                                          C.c_void_p, C.c_void_p]
         lib.ft_set_option.restype = C.c_int
         lib.ft_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         lib.ft_get_counters.restype = C.c_int
@@ -147,6 +154,19 @@ class Context:
         out = np.zeros(idx.size, dtype=CAND_DTYPE)
         self._check(self.lib.ft_eval_list(self.h, _hp(idx), idx.size, _hp(out)))
         return out
+
+    def eval_templates(self, templates_dev, t_ref: float, stat: str, rho_th: float, out_power=None, out_count=None):
+        """templates_dev: torch uint8/float64 device tensor holding n ft_template records (64 B each)."""
+        assert templates_dev.is_cuda and templates_dev.is_contiguous()
+        nbytes = templates_dev.numel() * templates_dev.element_size()
+        assert nbytes % 64 == 0
+        n = nbytes // 64
+        for o in (out_power, out_count):
+            assert o is None or (o.is_cuda and o.numel() == n and o.is_contiguous())
+        pp = C.c_void_p(out_power.data_ptr()) if out_power is not None else None
+        pc = C.c_void_p(out_count.data_ptr()) if out_count is not None else None
+        self._check(self.lib.ft_eval_templates(self.h, C.c_void_p(templates_dev.data_ptr()), n, float(t_ref),
+                                               FT_STAT[stat], float(rho_th), pp, pc))
 
     def counters(self) -> dict:
         c = FtCounters()

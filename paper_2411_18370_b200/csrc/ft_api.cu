@@ -499,6 +499,34 @@ int ft_eval_list(ft_ctx* c, const uint64_t* idx_host, int64_t n, ft_cand* out_ho
   return FT_OK;
 }
 
+int ft_eval_templates(ft_ctx* c, const ft_template* templates_dev, int64_t n, double t_ref, int stat,
+                      double rho_th, float* out_power_dev, int32_t* out_count_dev) {
+  if (!c) return FT_ERR_ARG;
+  if (n < 0 || (n > 0 && !templates_dev)) return fail(c, FT_ERR_ARG, "ft_eval_templates: NULL list");
+  if (stat < 0 || stat > 2) return fail(c, FT_ERR_ARG, "ft_eval_templates: bad stat");
+  if (!std::isfinite(t_ref) || !std::isfinite(rho_th)) return fail(c, FT_ERR_ARG, "ft_eval_templates: non-finite argument");
+  if (!c->d.P) return fail(c, FT_ERR_STATE, "ft_eval_templates: handle not created");
+  static_assert(sizeof(ft_template) == 64, "ft_template layout");
+  if (n == 0) return FT_OK;
+  int32_t* err_dev = nullptr;
+  FT_CUDA(c, cudaMalloc(&err_dev, sizeof(int32_t)));
+  FtDev d = c->d;
+  d.rho = (float)rho_th;
+  cudaError_t e = cudaMemsetAsync(err_dev, 0, sizeof(int32_t), c->stream);
+  c->ev_used = 0; c->counters.stat_launches = 0;
+  tick(c);
+  if (e == cudaSuccess) e = ft_launch_list(d, stat, templates_dev, n, t_ref, out_power_dev, out_count_dev, err_dev,
+                                           c->near_ties_dev, c->stream);
+  tock(c, 1);
+  int32_t flag = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&flag, err_dev, sizeof flag, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(err_dev);
+  if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_eval_templates: ") + cudaGetErrorString(e));
+  if (flag) return fail(c, FT_ERR_TRACK_RANGE, "ft_eval_templates: some tracks leave the spectrogram (their outputs are NaN / -1)");
+  return FT_OK;
+}
+
 int ft_get_counters(ft_ctx* c, ft_counters* out) {
   if (!c || !out) return FT_ERR_ARG;
   FT_CUDA(c, cudaStreamSynchronize(c->stream));

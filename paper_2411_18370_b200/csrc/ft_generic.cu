@@ -117,6 +117,70 @@ __global__ void ft_fold_kernel(const float* __restrict__ P, const float* __restr
     Q[i] = __fmul_rn(w[i], P[i]);
 }
 
+// K1: an explicit list of templates (an unstructured bank: "no assumption on the properties of
+// lambda"; random banks :312-316).  One thread per template, the canonical fp64 track
+// per (template, SFT), gather through L1/L2, fp64 accumulation in ascending SFT order.  Nothing can
+// be hoisted or staged (every template has its own sky position and orbit), so this kernel is bound
+// by the fp64 pipe; it is the paper's own formulation of the problem.  A track leaving the
+// spectrogram raises *err (reading R9: an error, not a clamp) and the template's outputs are NaN / -1.
+struct FtTemplateDev { double f0, f1, nx, ny, nz, a_p, P_orb, t_asc; };
+
+template <int STAT>
+__global__ void __launch_bounds__(K0_THREADS)
+ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict__ tl, int64_t n, double t_ref,
+               float* __restrict__ out_power, int32_t* __restrict__ out_count, int32_t* __restrict__ err,
+               unsigned long long* __restrict__ near_ties) {
+  __shared__ double sT[K0_THREADS], sVx[K0_THREADS], sVy[K0_THREADS], sVz[K0_THREADS];
+  __shared__ float sW[K0_THREADS];
+  const int64_t q = (int64_t)blockIdx.x * K0_THREADS + threadIdx.x;
+  const bool active = q < n;
+  FtTemplateDev tp = tl[active ? q : 0];
+  const double Om = __ddiv_rn(FT_TWO_PI, tp.P_orb);
+  const double apOm = __dmul_rn(tp.a_p, Om);
+  const bool binary = tp.a_p != 0.0;
+  double power = 0.0;
+  int32_t count = 0;
+  unsigned ties = 0;
+  bool bad = false;
+  for (int64_t a0 = 0; a0 < d.n_sft; a0 += K0_THREADS) {
+    const int64_t a = a0 + threadIdx.x;
+    __syncthreads();
+    if (a < d.n_sft) {
+      sT[threadIdx.x] = d.t_mid[a];
+      sVx[threadIdx.x] = d.vel[3 * a]; sVy[threadIdx.x] = d.vel[3 * a + 1]; sVz[threadIdx.x] = d.vel[3 * a + 2];
+      sW[threadIdx.x] = (d.wkind == 1) ? d.w[a] : 0.f;
+    }
+    __syncthreads();
+    const int m = (int)min((int64_t)K0_THREADS, d.n_sft - a0);
+    if (active) {
+      for (int c = 0; c < m; ++c) {
+        const double t = sT[c];
+        const double V = __ddiv_rn(__dadd_rn(__dadd_rn(__dmul_rn(sVx[c], tp.nx), __dmul_rn(sVy[c], tp.ny)),
+                                             __dmul_rn(sVz[c], tp.nz)), FT_C_LIGHT);
+        double B = 0.0;
+        if (binary) B = __dmul_rn(apOm, cos(__dmul_rn(Om, __dsub_rn(t, tp.t_asc))));
+        const double D = __dsub_rn(__dadd_rn(1.0, V), B);
+        const double x = ft_track_x(tp.f0, __dmul_rn(tp.f1, __dsub_rn(t, t_ref)), D, d.f_min, d.inv_df);
+        ties += ft_near_tie(x) ? 1u : 0u;
+        const int64_t k = __double2ll_rn(x);
+        if (k < 0 || k >= d.n_bins || !(x == x)) { bad = true; continue; }
+        const int64_t off = (a0 + c) * d.ld + k;
+        const float pix = __ldg(d.P + off);
+        if (STAT != 1) {
+          const float w = (d.wkind == 1) ? sW[c] : __ldg(d.w + off);
+          power = fma((double)w, (double)pix, power);  // exact product: same as mul then add
+        }
+        if (STAT != 0) count += (pix > d.rho) ? 1 : 0;
+      }
+    }
+  }
+  if (!active) return;
+  if (bad) atomicExch(err, 1);
+  if (STAT != 1 && out_power) out_power[q] = bad ? __int_as_float(0x7fc00000) : (float)power;
+  if (STAT != 0 && out_count) out_count[q] = bad ? -1 : count;
+  if (ties && near_ties) atomicAdd(near_ties, (unsigned long long)ties);
+}
+
 // A1 hoisted to bind time for binary grids: the orbital cosine depends on (P_orb, t_asc, SFT) only,
 // so the 64 a_p values of config 3 share it (Eq. 2; separability noted at :600).
 __global__ void ft_ctab_kernel(const __grid_constant__ FtDev d, double* __restrict__ ctab) {
@@ -166,5 +230,17 @@ cudaError_t ft_launch_refine(const FtDev& d, const uint64_t* idx_dev, const uint
 
 cudaError_t ft_launch_fold(const float* P, const float* w, float* Q, int64_t n, cudaStream_t s) {
   ft_fold_kernel<<<148 * 8, 256, 0, s>>>(P, w, Q, n);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_launch_list(const FtDev& d, int stat, const void* templates_dev, int64_t n, double t_ref,
+                           float* out_power, int32_t* out_count, int32_t* err, unsigned long long* near_ties,
+                           cudaStream_t s) {
+  if (n <= 0) return cudaSuccess;
+  const FtTemplateDev* tl = static_cast<const FtTemplateDev*>(templates_dev);
+  const unsigned grid = (unsigned)((n + K0_THREADS - 1) / K0_THREADS);
+  if (stat == 0) ft_list_kernel<0><<<grid, K0_THREADS, 0, s>>>(d, tl, n, t_ref, out_power, out_count, err, near_ties);
+  else if (stat == 1) ft_list_kernel<1><<<grid, K0_THREADS, 0, s>>>(d, tl, n, t_ref, out_power, out_count, err, near_ties);
+  else ft_list_kernel<2><<<grid, K0_THREADS, 0, s>>>(d, tl, n, t_ref, out_power, out_count, err, near_ties);
   return cudaGetLastError();
 }

@@ -61,9 +61,32 @@ def run_size(tag, n_sft, band_hz, n_sky, reps, full_writeout, dev, hbm_gbs):
     return out
 
 
+def run_bank(n, cfg, reps, dev):
+    """Unstructured bank of n random templates on config cfg's spectrogram: K1."""
+    import torch
+    wl = W.by_id(cfg)
+    tl = W.random_bank(wl, n)
+    P = torch.from_numpy(wl.P).to(dev)
+    w = torch.from_numpy(wl.w).to(dev) if wl.per_bin_weights else wl.w
+    ctx = B.Context(P, wl.t_mid, wl.vel, w, wl.f_min, wl.df)
+    t = torch.from_numpy(tl.view(np.float64).reshape(-1, 8).copy()).to(dev)
+    out = torch.empty(n, dtype=torch.float32, device=dev)
+    best = None
+    for r in range(reps + 1):
+        ctx.eval_templates(t, wl.grid.t_ref, "power", wl.rho_th, out, None)   # synchronises
+        ms = ctx.counters()["last_kernel_ms"]
+        if r > 0 and (best is None or ms < best):
+            best = ms
+    evals = n * wl.n_sft
+    ctx.close()
+    return {"bank": "random", "config": cfg, "n_templates": n, "n_sft": wl.n_sft, "evals": evals,
+            "kernel_ms": best, "evals_per_s": evals / (best * 1e-3), "kernel": "K1 ft_list_kernel (fp64 per evaluation)"}
+
+
 def main():
     import torch
     ap = argparse.ArgumentParser()
+    ap.add_argument("--bank", type=int, default=0, help="also time an unstructured bank of this many templates (configs 2, 3)")
     ap.add_argument("--max-templates", type=float, default=1.2e9)
     ap.add_argument("--min-templates", type=float, default=0.0)
     ap.add_argument("--reps", type=int, default=2)
@@ -75,6 +98,9 @@ def main():
         hbm = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
     except OSError:
         hbm = 6650.0
+    if args.bank:
+        for cfg in (2, 3):
+            print(json.dumps(run_bank(args.bank, cfg, args.reps, dev)), flush=True)
     for tag, sizes in (("A", W.SWEEP_A), ("B", W.SWEEP_B)):
         for n_sft, band_hz, n_sky in sizes:
             n_templates = n_sky * 5 * int(round(band_hz * 1800))

@@ -313,3 +313,35 @@ def config5(n_sft: int, band_hz: float, n_sky: int) -> Workload:
 
 def by_id(config_id: int, **kw) -> Workload:
     return {1: config1, 2: config2, 3: config3, 4: config4}[config_id](**kw)
+
+
+TEMPLATE_DTYPE = np.dtype([("f0", "<f8"), ("f1", "<f8"), ("nx", "<f8"), ("ny", "<f8"), ("nz", "<f8"),
+                           ("a_p", "<f8"), ("P_orb", "<f8"), ("t_asc", "<f8")])
+
+
+def random_bank(wl: Workload, n: int, seed: int = 0) -> np.ndarray:
+    """Unstructured template bank (PAPER.md:312-316 draws banks at random over the parameter space;
+    here uniformly over the physical box the workload's grid spans, a stand-in for the paper's
+    uniform draw in the xi coordinates of Eq. A11): n records (f0, f1, n, a_p, P_orb, t_asc).
+    f0 uniform over the grid's band, f1 over its spindown range, sky isotropic when the grid is
+    all-sky (else the grid's point), orbit uniform over the grid's a_p / P_orb ranges, t_asc over
+    one orbit after t_ref.  Parameters only: no track, no statistic."""
+    g = wl.grid
+    rng = np.random.Generator(np.random.PCG64((BASE_SEED + wl.config_id) * 16 + 8 + 16 * seed))
+    tl = np.zeros(n, dtype=TEMPLATE_DTYPE)
+    tl["f0"] = g.f0_start + rng.random(n) * (g.n_f0 - 1) * g.df0
+    f1_hi = g.f1_start + (g.n_f1 - 1) * g.df1
+    tl["f1"] = g.f1_start + rng.random(n) * (f1_hi - g.f1_start)
+    if len(g.sky) > 1:
+        z = 2.0 * rng.random(n) - 1.0
+        phi = 2.0 * math.pi * rng.random(n)
+        r = np.sqrt(1.0 - z * z)
+        tl["nx"], tl["ny"], tl["nz"] = r * np.cos(phi), r * np.sin(phi), z
+    else:
+        tl["nx"], tl["ny"], tl["nz"] = g.sky[0]
+    a_lo, a_hi = float(np.min(g.a_p)), float(np.max(g.a_p))
+    p_lo, p_hi = float(np.min(g.P_orb)), float(np.max(g.P_orb))
+    tl["a_p"] = a_lo + rng.random(n) * (a_hi - a_lo)
+    tl["P_orb"] = p_lo + rng.random(n) * (p_hi - p_lo)
+    tl["t_asc"] = g.t_ref + rng.random(n) * tl["P_orb"]
+    return tl
