@@ -30,7 +30,7 @@ struct FtDev {
 };
 
 // Parameters of one "outer point" = everything of a template but f0.
-struct FtPoint {
+struct alignas(16) FtPoint {
   double nx, ny, nz;
   double apOm;   // a_p * Om
   double Om;     // 2 pi / P_orb

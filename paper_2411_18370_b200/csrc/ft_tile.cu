@@ -206,11 +206,15 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
   FtPoint* sp = reinterpret_cast<FtPoint*>(bars + 2 * NS) + warp;
   if (lane == 0) *sp = ft_decode_point(d, pt);
   __syncwarp();
+  // per-warp table of the 32 packed track entries of the current SFT block: one broadcast LDS.128
+  // per ring stage instead of one shuffle per row
+  const uint32_t etab = smem_u32(reinterpret_cast<FtPoint*>(bars + 2 * NS) + n_cw) + 128u * (uint32_t)warp;
   const int tile_i0 = tile * a.tile_w;
   const int wlo = sub * J * 32;                                        // warp's first output, tile-relative
   const int tile_n = min(a.tile_w, (int)d.n_f0 - tile_i0);             // valid f0 in this tile
   const int warp_n = max(0, min(J * 32, tile_n - wlo));                // valid outputs of this warp
   const int i_first = tile_i0 + wlo;
+  const bool last_ok = warp_n > 32 * (J - 1);  // the warp's last chunk holds valid outputs (else: skipped)
   float acc[J];
 #pragma unroll
   for (int j = 0; j < J; ++j) acc[j] = 0.f;
@@ -225,23 +229,29 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
     uint32_t entry = 0;
     if (a0 + lane < n_sft && warp_n > 0)
       entry = ft_tile_entry(d, *sp, a0 + lane, kst[a0 + lane], i_first, warp_n, a.copy_floats, &ties, a.err);
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(etab + 4u * (uint32_t)lane), "r"(entry) : "memory");
+    __syncwarp();
     // -- A4: gather + reduce over the block's SFTs -----------------------------------------------
     const int n_rows = min(32, n_sft - a0);
     for (int q = 0; q < n_rows; q += kRPS) {
+      uint32_t e4[kRPS];
+      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                   : "=r"(e4[0]), "=r"(e4[1]), "=r"(e4[2]), "=r"(e4[3]) : "r"(etab + 4u * (uint32_t)q));
       mbar_wait(full0 + 8 * s, ph);
 #pragma unroll
       for (int r = 0; r < kRPS; ++r) {
         if (q + r < n_rows) {
-          const uint32_t e = __shfl_sync(0xffffffffu, entry, q + r);
+          const uint32_t e = e4[r];
           const uint32_t base = stage_addr + (uint32_t)r * row_bytes;
           if (e < 8192u) {  // no break inside this warp's range: J conflict-free LDS.32 + FADD
             const uint32_t ad = base + 4u * e;
             float v[J];
 #pragma unroll
             for (int j = 0; j < J; ++j)
-              asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v[j]) : "r"(ad + 128u * j));
+              if (j < J - 1 || last_ok) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v[j]) : "r"(ad + 128u * j));
 #pragma unroll
-            for (int j = 0; j < J; ++j) acc[j] += v[j];
+            for (int j = 0; j < J; ++j)
+              if (j < J - 1 || last_ok) acc[j] += v[j];
           } else {
             const uint32_t ad_lo = base + 4u * (e & 8191u);
             const uint32_t ad_hi = (e & (1u << 24)) ? ad_lo - 4u : ad_lo + 4u;
@@ -484,7 +494,7 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   pl.n_stages = (int32_t)(rows_fit / kRPS);
   pl.ctas_per_sm = ctas;
   pl.smem_bytes = (size_t)pl.n_stages * pl.rows_per_stage * row_bytes + 2 * 8 * (size_t)pl.n_stages +
-                  sizeof(FtPoint) * (size_t)(pl.R * pl.wpp);
+                  (sizeof(FtPoint) + 128) * (size_t)(pl.R * pl.wpp) + 16;
   e = cudaMalloc(&pl.kst, sizeof(int32_t) * kst.size());
   if (e != cudaSuccess) return e;
   e = cudaMalloc(&pl.err, sizeof(int32_t));
