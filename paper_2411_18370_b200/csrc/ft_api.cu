@@ -33,9 +33,13 @@ struct ft_ctx {
   int stat = 0;
   double df = 0.0;
   bool tile_ok = false;
-  FtTilePlan plan{};
+  FtTilePlan plan{};            // fp32 gather (power; number count when the packed kernel is not eligible)
+  FtTilePlan plan8{};           // packed number-count kernel (ft_tile8.cu)
+  bool tile8_ok = false;
+  uint8_t* H8_dev = nullptr;    // four byte-shifted hit maps
+  float H8_rho = 0.f; bool H8_valid = false;
   // options
-  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0;
+  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1;
   // selection buffers
   FtSelectDev sel{};
   uint64_t* final_idx = nullptr;
@@ -157,7 +161,7 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
     }
     if (stat != FT_STAT_POWER && (out_count || (filter && stat == FT_STAT_HOUGH))) {
       tick(c);
-      FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.H, 0.0, pt_begin, pt_end, nullptr, out_count, out_base,
+      FT_CUDA(c, ft_launch_tile(c->d, c->tile8_ok ? c->plan8 : c->plan, c->d.H, 0.0, pt_begin, pt_end, nullptr, out_count, out_base,
                                 stat == FT_STAT_HOUGH ? sel : nullptr, bpb, c->near_ties_dev, c->stream, &launches, stride, n_strided, complement));
       tock(c, launches);
     }
@@ -173,11 +177,13 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
 // The tile kernel raises plan.err if a track left its staged strip (a planning bug, never data):
 // surfaced at the next synchronising call instead of silently wrong sums.
 int check_tile_err(ft_ctx* c) {
-  if (!c->plan.err) return FT_OK;
-  int32_t e = 0;
-  FT_CUDA(c, cudaMemcpy(&e, c->plan.err, sizeof e, cudaMemcpyDeviceToHost));
-  if (e != 0) return fail(c, FT_ERR_STATE, e == 1 ? "tile kernel: a track left its staged strip (internal planning error)"
-                                                  : "tile kernel: more than one break in a warp range (internal planning error)");
+  for (const FtTilePlan* pl : {&c->plan, &c->plan8}) {
+    if (!pl->err) continue;
+    int32_t e = 0;
+    FT_CUDA(c, cudaMemcpy(&e, pl->err, sizeof e, cudaMemcpyDeviceToHost));
+    if (e != 0) return fail(c, FT_ERR_STATE, e == 1 ? "tile kernel: a track left its staged strip (internal planning error)"
+                                                    : "tile kernel: more than one break in a warp range (internal planning error)");
+  }
   return FT_OK;
 }
 
@@ -255,6 +261,7 @@ int ft_set_option(ft_ctx* c, int option, int64_t value) {
   switch (option) {
     case FT_OPT_KERNEL: if (value < 0 || value > 2) return fail(c, FT_ERR_ARG, "FT_OPT_KERNEL: 0..2"); c->opt_kernel = value; break;
     case FT_OPT_FUSED_TOPK: c->opt_fused = value ? 1 : 0; break;
+    case FT_OPT_PACKED_COUNT: c->opt_packed = value ? 1 : 0; break;
     case FT_OPT_POINTS_PER_CTA: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_POINTS_PER_CTA >= 0"); c->opt_ppc = value; break;
     default: return fail(c, FT_ERR_ARG, "unknown option");
   }
@@ -339,7 +346,31 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
     c->tile_ok = why.empty();
     if (!c->tile_ok && c->opt_kernel == 2) return fail(c, FT_ERR_UNSUPPORTED, "tile kernel not eligible: " + why);
   }
-  if (c->tile_ok && stat != FT_STAT_POWER && !(c->H_valid && c->H_rho == d.rho)) {
+  // number count: the packed kernel when it is eligible (n_sft <= 65535), else the fp32 0/1 map
+  c->tile8_ok = false;
+  ft_tile_plan_free(&c->plan8);
+  if (c->tile_ok && stat != FT_STAT_POWER && c->opt_packed) {
+    std::string why8;
+    int launches = 0;
+    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc};
+    const cudaError_t e = ft_tile_plan(d, hin, c->stream, &c->plan8, &why8, &launches, 1);
+    c->counters.kernel_launches += launches;
+    if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_tile_plan (packed): ") + cudaGetErrorString(e));
+    // narrow bands (< 6 chunks of 128 f0 per warp) are bound by the per-(warp, SFT) bookkeeping, which the
+    // fp32 map amortises over four times as many loads: measured faster there (config 3, 450 f0)
+    c->tile8_ok = why8.empty() && c->plan8.J >= 6;
+  }
+  if (c->tile8_ok && !(c->H8_valid && c->H8_rho == d.rho)) {
+    const int64_t ld8 = (d.n_bins + 15) / 16 * 16;
+    if (!c->H8_dev) FT_CUDA(c, cudaMalloc(&c->H8_dev, (size_t)4 * d.n_sft * ld8 + 16384));
+    FT_CUDA(c, cudaMemsetAsync(c->H8_dev + (size_t)4 * d.n_sft * ld8, 0, 16384, c->stream));
+    FT_CUDA(c, ft_launch_hitmap8(d.P, d.rho, c->H8_dev, d.n_sft, d.n_bins, d.ld, ld8, c->stream));
+    c->counters.kernel_launches += 1;
+    c->H8_rho = d.rho; c->H8_valid = true;
+    d.ld8 = ld8;
+  }
+  d.H8 = c->H8_dev;
+  if (c->tile_ok && !c->tile8_ok && stat != FT_STAT_POWER && !(c->H_valid && c->H_rho == d.rho)) {
     if (!c->H_dev) FT_CUDA(c, cudaMalloc(&c->H_dev, sizeof(float) * (size_t)d.n_sft * d.ld));
     FT_CUDA(c, ft_launch_hitmap(d.P, d.rho, c->H_dev, d.n_sft * d.ld, c->stream));
     c->counters.kernel_launches += 1;
@@ -355,6 +386,12 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
     else
       std::snprintf(buf, sizeof buf, "K0 generic kernel (%s)", c->opt_kernel == 1 ? "forced" : c->why.c_str());
     c->desc = buf;
+    if (c->tile8_ok) {
+      std::snprintf(buf, sizeof buf, "; number count: packed tile kernel J=%d wpp=%d R=%d n_tiles=%d tile_w=%d threads=%d pitch=%d copy=%d stages=%dx%d",
+                    c->plan8.J, c->plan8.wpp, c->plan8.R, c->plan8.n_tiles, c->plan8.tile_w, (c->plan8.R * c->plan8.wpp + 1) * 32,
+                    c->plan8.pitch, c->plan8.copy_floats, c->plan8.n_stages, c->plan8.rows_per_stage);
+      c->desc += buf;
+    }
   }
   c->bound = true;
   if (out_power_dev || out_count_dev) {
@@ -393,9 +430,10 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
   if (fused) {
     // Phase A: per-band thresholds from a strided sample of point groups (every stride-th CTA group
     // of the bank, so the sample sees every region of parameter space), written out in full.
-    const uint64_t R = (uint64_t)c->plan.R;
+    const FtTilePlan& spl = (by_count && c->tile8_ok) ? c->plan8 : c->plan;  // the plan the statistic pass runs
+    const uint64_t R = (uint64_t)spl.R;
     const uint64_t n_groups = (d.n_points + R - 1) / R;
-    uint64_t n_sg = ft_tile_sample_points(c->plan, d.n_points) / R;
+    uint64_t n_sg = ft_tile_sample_points(spl, d.n_points) / R;
     n_sg = n_sg < 1 ? 1 : (n_sg > n_groups ? n_groups : n_sg);
     const uint64_t stride = n_groups / n_sg;
     const int64_t rows = (int64_t)(n_sg * R);
@@ -552,6 +590,8 @@ void ft_destroy(ft_ctx* c) {
   cudaStreamSynchronize(c->stream);
   free_select(c);
   ft_tile_plan_free(&c->plan);
+  ft_tile_plan_free(&c->plan8);
+  dfree(c->H8_dev);
   dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->H_dev); dfree(c->ctab_dev); dfree(c->axes_dev);
   dfree(c->scratch_f); dfree(c->scratch_i); dfree(c->near_ties_dev);
   for (cudaEvent_t e : c->evs) cudaEventDestroy(e);

@@ -13,6 +13,8 @@ struct FtDev {
   const float* w;       // per-SFT [n_sft] or per-bin [n_sft][ld]
   const float* Q;       // folded w*P, one fp32 rounding per pixel, [n_sft][ld] (tile kernel input)
   const float* H;       // hit map (P > rho) ? 1 : 0 as fp32, [n_sft][ld] (tile kernel input, number count)
+  const uint8_t* H8;    // packed hit maps: H8[m][a][b] = (P[a][b+m] > rho), m = 0..3, rows of ld8 bytes (ft_tile8.cu)
+  int64_t ld8;
   const double* t_mid;  // [n_sft]
   const double* vel;    // [n_sft][3]
   const double* sky;    // [n_sky][3]

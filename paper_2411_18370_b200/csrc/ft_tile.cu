@@ -19,123 +19,9 @@
 #include <vector>
 
 #include "ft_tile.cuh"
+#include "ft_tile_dev.cuh"
 
 namespace {
-
-constexpr int kMaxPitch = 8191;  // packed entry: 13 bits of strip offset
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-
-constexpr int kRPS = 4;  // spectrogram rows per ring stage (divides 32)
-
-struct FtTileArgs {
-  const float* A;
-  const int32_t* kst;
-  int32_t* err;
-  int32_t tile_w, n_tiles, R, wpp, pitch, copy_floats, n_stages;
-  uint64_t pt_begin, pt_end;
-  double add_back;  // sum over SFTs of the per-row constant removed from A at fold time
-  float* out_f;
-  int32_t* out_i;
-  uint64_t out_base;
-  FtSelectDev sel;
-  int32_t has_sel, bpb;
-  unsigned long long* near_ties;
-  uint32_t group_stride;  // > 1: every stride-th group only (threshold sample), outputs packed by launch-local row
-  uint32_t skip_stride;   // > 1: every group EXCEPT the first skip_n multiples of skip_stride (the rest of the bank)
-  uint64_t skip_n;
-};
-
-// Threads per CTA the kernel is compiled for: (consumer warps + 1 producer warp) * 32.  The
-// accumulators (J) and the loads in flight (J) set the register need, hence the bound.
-// (the register file is 4 x 16 384: 80 registers allow 6 warps per SM sub-partition, 64 allow 8)
-__host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : 80; }
-__host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 1024 : 768; }
-
-// Packed per-(warp, SFT) track entry: bits 0-12 strip offset of the warp's first output (floats),
-// bits 13-23 break position relative to the warp's first output (0 = no break in the warp's range),
-// bit 24 set when the shift decreases at the break.  No break <=> entry < 8192.
-__device__ __forceinline__ uint32_t pack_entry(int off, int rel, bool neg) {
-  return (uint32_t)off | ((uint32_t)rel << 13) | (neg ? (1u << 24) : 0u);
-}
-
-// A1 + A2 for one (outer point, SFT, warp range): canonical track at the first and last f0 of the
-// range, and, if the two shifts differ, the canonical position of the single break.
-__device__ __forceinline__ uint32_t ft_tile_entry(const FtDev& d, const FtPoint& p, int al, int kst_al,
-                                               int i_first, int warp_n, int copy_floats,
-                                               unsigned* ties, int32_t* err) {
-  const double t = d.t_mid[al];
-  const double D = ft_doppler(d, p, al, t);
-  const double f1dt = __dmul_rn(p.f1, __dsub_rn(t, d.t_ref));
-  auto xof = [&](int i) {
-    const double f0 = __dadd_rn(d.f0_start, __dmul_rn((double)i, d.df0));
-    const double x = ft_track_x(f0, f1dt, D, d.f_min, d.inv_df);
-    *ties += ft_near_tie(x) ? 1u : 0u;
-    return x;
-  };
-  const int i_last = i_first + warp_n - 1;
-  const double xa = xof(i_first);
-  const int ka = __double2int_rn(xa);
-  const int s = ka - i_first;
-  const int sb = __double2int_rn(xof(i_last)) - i_last;
-  const int off = ka - kst_al;  // strip index of the warp's first output
-  int rel = 0;
-  const bool neg = sb < s;
-  if (sb != s) {
-    // smallest i in (i_first, i_last] with rint(x_i) - i != s: estimate from the slope, verify
-    // with the canonical arithmetic, bisect if the estimate is off
-    auto pred = [&](int i) { return (__double2int_rn(xof(i)) - i) != s; };
-    int lo = i_first, hi = i_last;
-    const double frac = xa - (double)ka;
-    double nest = ceil((0.5 - (neg ? -frac : frac)) / fmax(fabs(D - 1.0), 1e-300));
-    nest = fmin(fmax(nest, 1.0), (double)(warp_n - 1));
-    const int cand = i_first + (int)nest;
-    if (pred(cand)) {
-      hi = cand;
-      if (cand - 1 > lo) { if (!pred(cand - 1)) lo = cand - 1; else hi = cand - 1; }
-    } else {
-      lo = cand;
-      if (cand + 1 < hi) { if (pred(cand + 1)) hi = cand + 1; else lo = cand + 1; }
-    }
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (pred(mid)) hi = mid; else lo = mid;
-    }
-    rel = hi - i_first;
-    if (sb - s > 1 || s - sb > 1) atomicExch(err, 2);
-  }
-  // every pixel read for a valid output must lie inside the copied strip (else: a planning bug)
-  const int hi_idx = off + (warp_n - 1) + ((rel && !neg) ? 1 : 0);
-  if (off < 0 || off > kMaxPitch || hi_idx >= copy_floats) {
-    atomicExch(err, 1);
-    return 0u;
-  }
-  return pack_entry(off, rel, neg);
-}
 
 template <int J>
 __global__ void __maxnreg__(ft_tile_max_regs(J))
@@ -167,29 +53,38 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
   const uint32_t row_bytes = 4u * (uint32_t)a.pitch;
 
   if (warp == n_cw) {
-    // ---- producer: one elected lane streams the strips (A3) ------------------------------------
-    if (lane == 0) {
-      const int64_t total = (int64_t)n_sft * d.ld;
-      int s = 0;
-      uint32_t lap = 0;  // how many times the ring has wrapped
-      for (int a0 = 0; a0 < n_sft; a0 += kRPS) {
+    // ---- producer: streams the strips (A3).  The whole warp fetches the 32 strip starts of a block
+    // with one coalesced load; lane 0 issues the bulk copies.
+    const int64_t total = (int64_t)n_sft * d.ld;
+    int s = 0;
+    uint32_t lap = 0;  // how many times the ring has wrapped
+    for (int a0 = 0; a0 < n_sft; a0 += 32) {
+      const int kk = (a0 + lane < n_sft) ? kst[a0 + lane] : 0;
+      const int n_rows = min(32, n_sft - a0);
+      for (int q = 0; q < n_rows; q += kRPS) {
         if (lap > 0) mbar_wait(empty0 + 8 * s, (lap - 1u) & 1u);  // consumers released the previous use
-        const int rows = min(kRPS, n_sft - a0);
-        int64_t src[kRPS];
-        uint32_t nb[kRPS], bytes = 0;
+        const int rows = min(kRPS, n_rows - q);
+        int kr[kRPS];
 #pragma unroll
-        for (int r = 0; r < kRPS; ++r) {
-          if (r < rows) {
-            src[r] = (int64_t)(a0 + r) * d.ld + kst[a0 + r];
-            nb[r] = 4u * (uint32_t)min((int64_t)a.copy_floats, total - src[r]);
-            bytes += nb[r];
+        for (int r = 0; r < kRPS; ++r) kr[r] = __shfl_sync(0xffffffffu, kk, (q + r) & 31);
+        if (lane == 0) {
+          int64_t src[kRPS];
+          uint32_t nb[kRPS], bytes = 0;
+#pragma unroll
+          for (int r = 0; r < kRPS; ++r) {
+            if (r < rows) {
+              src[r] = (int64_t)(a0 + q + r) * d.ld + kr[r];
+              nb[r] = 4u * (uint32_t)min((int64_t)a.copy_floats, total - src[r]);
+              bytes += nb[r];
+            }
           }
-        }
-        mbar_expect_tx(full0 + 8 * s, bytes);
-        const uint32_t dst = smem_u32(ring) + (uint32_t)(s * kRPS) * row_bytes;
+          mbar_expect_tx(full0 + 8 * s, bytes);
+          const uint32_t dst = smem_u32(ring) + (uint32_t)(s * kRPS) * row_bytes;
 #pragma unroll
-        for (int r = 0; r < kRPS; ++r)
-          if (r < rows) bulk_g2s(dst + (uint32_t)r * row_bytes, a.A + src[r], nb[r], full0 + 8 * s);
+          for (int r = 0; r < kRPS; ++r)
+            if (r < rows) bulk_g2s(dst + (uint32_t)r * row_bytes, a.A + src[r], nb[r], full0 + 8 * s);
+        }
+        __syncwarp();
         if (++s == NS) { s = 0; ++lap; }
       }
     }
@@ -390,24 +285,29 @@ void ft_tile_plan_free(FtTilePlan* p) {
 }
 
 cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s, FtTilePlan* plan,
-                         std::string* why, int* launches) {
+                         std::string* why, int* launches, int mode) {
   *launches = 0;
   why->clear();
   ft_tile_plan_free(plan);
   if (d.df0 != in.df && d.n_f0 > 1) { *why = "f0 step differs from the bin width"; return cudaSuccess; }
   if (!d.Q) { *why = "no folded array"; return cudaSuccess; }
+  if (d.n_f0 > (1 << 30)) { *why = "more than 2^30 f0 values"; return cudaSuccess; }
+  if (mode == 1 && d.n_sft > 65535) { *why = "packed number count holds 16-bit counters (n_sft <= 65535)"; return cudaSuccess; }
+  // chunk = the f0 a warp covers with one load instruction: 32 (one fp32 pixel per lane) or 128 (4 packed hits)
+  const int cw = mode == 1 ? 128 : 32;
+  const int align = mode == 1 ? 16 : 4;   // strip start / length granularity in bins (16-byte TMA copies)
   const int64_t n_sft = d.n_sft;
   // --- tiling: n_tiles x wpp warps x J chunks of 32 f0, least issue slots (J+1.5 per chunk row) -----
-  const int64_t chunks = (d.n_f0 + 31) / 32;
+  const int64_t chunks = (d.n_f0 + cw - 1) / cw;
   double best = 1e300;
   int bJ = 0, bW = 0; int64_t bT = 0;
-  const int maxJ_eps = (int)std::floor(0.45 / (32.0 * std::fmax(in.eps_bound, 1e-12)));
+  const int maxJ_eps = (int)std::floor(0.45 / ((double)cw * std::fmax(in.eps_bound, 1e-12)));
   for (int64_t nt = 1; nt <= chunks; ++nt) {
     const int64_t cpt = (chunks + nt - 1) / nt;
     if (nt > 1 && (chunks + nt - 2) / (nt - 1) == cpt) continue;  // same tile size as nt-1
     for (int wpp = 1; wpp <= 4; ++wpp) {
       const int64_t Jn = (cpt + wpp - 1) / wpp;
-      if (Jn > 32) continue;
+      if (Jn > (mode == 1 ? 16 : 32)) continue;
       int J = 0;
       for (int c : kJList) if (c >= Jn) { J = c; break; }
       if (J == 0 || J > maxJ_eps) continue;
@@ -419,11 +319,13 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   if (bJ == 0) { *why = "Doppler spread too large for a single break per warp range"; return cudaSuccess; }
   FtTilePlan pl;
   pl.J = bJ; pl.wpp = bW;
-  pl.tile_w = (int32_t)(((chunks + bT - 1) / bT) * 32);
+  pl.mode = mode; pl.cw = cw;
+  pl.tile_w = (int32_t)(((chunks + bT - 1) / bT) * cw);
   pl.n_tiles = (int32_t)((d.n_f0 + pl.tile_w - 1) / pl.tile_w);
   // default: ~20 consumer warps per CTA (measured best on B200: R = 10 at wpp = 2, R = 23 at wpp = 1)
   int R = in.points_per_cta > 0 ? in.points_per_cta : (pl.wpp == 1 ? 23 : 20 / pl.wpp);
-  R = std::min<int>(R, (ft_tile_max_threads(pl.J) / 32 - 1) / pl.wpp);  // + 1 producer warp
+  const int max_threads = mode == 1 ? ft_tile8_max_threads(pl.J) : ft_tile_max_threads(pl.J);
+  R = std::min<int>(R, (max_threads / 32 - 1) / pl.wpp);  // + 1 producer warp
   R = (int)std::min<uint64_t>((uint64_t)R, d.n_points);
   pl.R = std::max(R, 1);
   // --- point-independent strip bounds per (tile, SFT) -----------------------------------------------
@@ -459,22 +361,22 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
       int64_t lo = (int64_t)std::floor(x_lo) - 1, hi = (int64_t)std::ceil(x_hi) + 1;
       lo = std::max<int64_t>(lo, 0);
       hi = std::min<int64_t>(hi, d.n_bins - 1);
-      const int64_t k0 = lo / 4 * 4;
+      const int64_t k0 = lo / align * align;
       kst[(size_t)t * n_sft + a] = (int32_t)k0;
       max_w = std::max(max_w, hi - k0 + 1);
     }
   }
-  pl.copy_floats = (int32_t)((max_w + 3) / 4 * 4);
-  int min_warp_n = 32 * pl.J;
+  pl.copy_floats = (int32_t)((max_w + align - 1) / align * align);
+  int min_warp_n = cw * pl.J;
   for (int t = 0; t < pl.n_tiles; ++t) {
     const int64_t tile_n = std::min<int64_t>(pl.tile_w, d.n_f0 - (int64_t)t * pl.tile_w);
     for (int sub = 0; sub < pl.wpp; ++sub) {
-      const int64_t wn = std::min<int64_t>(32 * pl.J, tile_n - (int64_t)sub * pl.J * 32);
+      const int64_t wn = std::min<int64_t>(cw * pl.J, tile_n - (int64_t)sub * pl.J * cw);
       if (wn > 0) min_warp_n = (int)std::min<int64_t>(min_warp_n, wn);
     }
   }
-  pl.pitch = (pl.copy_floats + 32 * pl.J - min_warp_n + 2 + 3) / 4 * 4;
-  pl.pitch = std::max(pl.pitch, 32 * pl.J + 4);  // warps without valid outputs read [0, 32 J)
+  pl.pitch = (pl.copy_floats + cw * pl.J - min_warp_n + 8 + align - 1) / align * align;
+  pl.pitch = std::max(pl.pitch, (cw * pl.J + 8 + align - 1) / align * align);  // warps without valid outputs read [0, cw J)
   if (pl.copy_floats > kMaxPitch + 1) { *why = "strip too wide for the packed track entry"; return cudaSuccess; }
   // --- shared-memory ring ---------------------------------------------------------------------------
   const int threads = (pl.R * pl.wpp + 1) * 32;
@@ -482,10 +384,13 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   int ctas = std::min(4, std::min(2048 / threads, 65536 / (threads * regs_est)));
   ctas = std::max(ctas, 1);
   const size_t row_bytes = (size_t)pl.pitch * 4;
+  // per-warp state: point parameters, entry table; packed mode: the 16-bit counter levels
+  const size_t state_bytes = (sizeof(FtPoint) + 128) * (size_t)(pl.R * pl.wpp) + 16 +
+                             (mode == 1 ? (size_t)8 * pl.J * 32 * (pl.R * pl.wpp) : 0);
   int64_t rows_fit = 0;
   for (;; --ctas) {  // fewer CTAs per SM until the ring holds two stages
     const size_t budget = (size_t)(228 * 1024) / ctas - 2048;
-    rows_fit = (int64_t)((budget - 1024) / row_bytes);
+    rows_fit = budget > state_bytes + 1024 ? (int64_t)((budget - 1024 - state_bytes) / row_bytes) : 0;
     if (rows_fit >= 2 * kRPS || ctas == 1) break;
   }
   if (rows_fit < 2 * kRPS) { *why = "strip does not fit shared memory twice"; return cudaSuccess; }
@@ -493,8 +398,7 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   pl.rows_per_stage = kRPS;
   pl.n_stages = (int32_t)(rows_fit / kRPS);
   pl.ctas_per_sm = ctas;
-  pl.smem_bytes = (size_t)pl.n_stages * pl.rows_per_stage * row_bytes + 2 * 8 * (size_t)pl.n_stages +
-                  (sizeof(FtPoint) + 128) * (size_t)(pl.R * pl.wpp) + 16;
+  pl.smem_bytes = (size_t)pl.n_stages * pl.rows_per_stage * row_bytes + 2 * 8 * (size_t)pl.n_stages + state_bytes;
   e = cudaMalloc(&pl.kst, sizeof(int32_t) * kst.size());
   if (e != cudaSuccess) return e;
   e = cudaMalloc(&pl.err, sizeof(int32_t));
@@ -538,7 +442,8 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* 
     if (n_groups_strided == 0 || n_groups_strided > all_groups || n_launch > max_groups) return cudaErrorInvalidValue;
     if (n_launch == 0) return cudaSuccess;
     a.pt_begin = pt_begin; a.pt_end = pt_end;
-    const cudaError_t e = launch_any(plan.J, d, a, (unsigned)(n_launch * plan.n_tiles), block, plan.smem_bytes, s);
+    const cudaError_t e = plan.mode == 1 ? ft_tile8_launch(plan.J, d, a, (unsigned)(n_launch * plan.n_tiles), block, plan.smem_bytes, s)
+                                         : launch_any(plan.J, d, a, (unsigned)(n_launch * plan.n_tiles), block, plan.smem_bytes, s);
     if (e == cudaSuccess) *launches = 1;
     return e;
   }
@@ -548,7 +453,8 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* 
     if (groups > max_groups) groups = max_groups;
     a.pt_begin = pt;
     a.pt_end = std::min<uint64_t>(pt_end, pt + groups * plan.R);
-    const cudaError_t e = launch_any(plan.J, d, a, (unsigned)(groups * plan.n_tiles), block, plan.smem_bytes, s);
+    const cudaError_t e = plan.mode == 1 ? ft_tile8_launch(plan.J, d, a, (unsigned)(groups * plan.n_tiles), block, plan.smem_bytes, s)
+                                         : launch_any(plan.J, d, a, (unsigned)(groups * plan.n_tiles), block, plan.smem_bytes, s);
     if (e != cudaSuccess) return e;
     *launches += 1;
     pt = a.pt_end;

@@ -8,13 +8,15 @@
 struct FtTilePlan {
   int32_t* kst = nullptr;       // device [n_tiles][n_sft] first staged bin of the strip (multiple of 4)
   int32_t* err = nullptr;       // device [1] set by the kernel if a track left its staged strip (plan bug)
+  int32_t mode = 0;             // 0: fp32 gather (ft_tile_kernel), 1: packed number count (ft_tile8_kernel)
+  int32_t cw = 32;              // f0 per chunk (per warp load instruction): 32 or 128
   int32_t n_tiles = 0;          // f0 tiles
   int32_t tile_w = 0;           // f0 per tile (multiple of 32; the last tile may hold fewer)
-  int32_t J = 0;                // 32-wide f0 chunks per consumer warp (template parameter)
+  int32_t J = 0;                // cw-wide f0 chunks per consumer warp (template parameter)
   int32_t wpp = 0;              // consumer warps per outer point
   int32_t R = 0;                // outer points per CTA
-  int32_t pitch = 0;            // floats per staged row in shared memory
-  int32_t copy_floats = 0;      // floats copied per row (multiple of 4, <= pitch)
+  int32_t pitch = 0;            // bins per staged row in shared memory (mode 1: per byte-shifted copy)
+  int32_t copy_floats = 0;      // bins copied per row (multiple of 4, mode 1: 16; <= pitch)
   int32_t rows_per_stage = 0;   // divides 32
   int32_t n_stages = 0;
   int32_t ctas_per_sm = 0;
@@ -30,7 +32,7 @@ struct FtTileHostIn {
   int points_per_cta;
 };
 cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s, FtTilePlan* plan,
-                         std::string* why, int* launches);
+                         std::string* why, int* launches, int mode = 0);
 uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points);
 // One pass of the gather-reduce over array A (folded w*P for the power statistic, the 0/1 hit map
 // for the number count); add_back is the constant the fold removed from A, summed over SFTs.
@@ -44,6 +46,8 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* 
                            cudaStream_t s, int* launches, uint32_t group_stride = 1, uint64_t n_groups_strided = 0,
                            bool complement = false);
 cudaError_t ft_launch_hitmap(const float* P, float rho, float* H, int64_t n, cudaStream_t s);
+cudaError_t ft_launch_hitmap8(const float* P, float rho, uint8_t* H8, int64_t n_sft, int64_t n_bins, int64_t ld,
+                              int64_t ld8, cudaStream_t s);
 // Q[a][k] = fl(fl(w P) - c_a) with c_a = fl(mean_k fl(w P)) per row; w_sft (per-SFT) or w_bin (per-bin).
 cudaError_t ft_launch_fold_centered(const float* P, const float* w_sft, const float* w_bin, float* Q, float* c_row,
                                     int64_t n_sft, int64_t n_bins, int64_t ld, cudaStream_t s);
