@@ -139,3 +139,28 @@ def test_generic_kernel_when_f0_step_differs_from_bin_width():
         ctx.eval(fine, "power", 1.6)
     assert e.value.code == -7
     ctx.close()
+
+
+@pytest.mark.parametrize("band_hz,n_sft,n_sky,ppc", [(1.3, 300, 3, 0), (2.4, 77, 2, 3), (0.6, 520, 5, 2)])
+def test_packed_number_count_equals_fp32_map_and_oracle(band_hz, n_sft, n_sky, ppc):
+    """The packed byte hit map (ft_tile8, 8-bit SIMD counters folded every 224 SFTs) and the fp32
+    0/1 map give the same integer counts, equal to the oracle's; n_sft > 224 exercises the fold."""
+    from paper_2411_18370_b200 import binding as B
+    wl = W.config2(n_sft=n_sft, n_sky=n_sky, band_hz=band_hz, band_width=0.01, k=3)
+    _, oc, _, otie = fo.Oracle(wl).eval_range()
+    ctx = H.gpu_context(wl, kernel=2, ppc=ppc)
+    _, gc8 = H.gpu_full(ctx, wl, stat="hough")
+    assert "packed tile kernel" in ctx.describe()
+    ctx.set_option(B.FT_OPT_PACKED_COUNT, 0)
+    _, gc32 = H.gpu_full(ctx, wl, stat="hough")
+    assert "packed" not in ctx.describe()
+    assert np.array_equal(gc8, gc32)
+    ok = otie == 0
+    assert np.array_equal(gc8[ok], oc[ok])
+    ctx.set_option(B.FT_OPT_PACKED_COUNT, 1)
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    ctx.eval(wl.grid, "hough", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    op = fo.Oracle(wl).eval_range()[0]
+    H.assert_topk_parity(wl, cands, oc, op, oc, wl.k, bpb, by_count=True)
+    ctx.close()
