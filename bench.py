@@ -31,7 +31,7 @@ METRIC = "template_sft_evals_per_sec"
 UNIT = "evals/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per statistic launch (profiles/r01_k2_ncu_full.md: the
 # spectrogram is read from HBM once per launch, everything else is served from L2 / shared memory)
-NCU_TRAFFIC = {2: 31.19e6}
+NCU_TRAFFIC = {2: 31.23e6}
 SMEM_BYTES_PER_CLK_SM = 128.0   # B200_MICROARCH "smem crossbar BW 128 B/cyc/SM"
 N_SM = 148
 
