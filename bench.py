@@ -154,10 +154,15 @@ def run_gpu(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    local = local % torch.cuda.device_count()   # (one-GPU boxes: --dist-backend gloo runs every rank on cuda:0)
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    on_dev = args.dist_backend == "nccl"
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        if on_dev:
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group(args.dist_backend)
     wl, idx_off = make_workload(args, rank, world)
     from paper_2411_18370_b200 import sharding as S
     g = wl.grid
@@ -178,7 +183,7 @@ def run_gpu(args):
         c.eval(g, wl.stat, wl.rho_th)                      # bind grid (+ fold weights / threshold bit)
         cands = c.topk_per_band(wl.band_width, wl.k, n_bands)   # evaluate + fused selection; syncs
         if world > 1:  # KBs of records: all-gather + merge under the same total order
-            cands = S.merge_candidates(S.all_gather_candidates(S.to_global(cands, idx_off), dev), wl.k,
+            cands = S.merge_candidates(S.all_gather_candidates(S.to_global(cands, idx_off), dev if on_dev else None), wl.k,
                                        by_count=(wl.stat == "hough"))
         return cands
 
@@ -205,7 +210,7 @@ def run_gpu(args):
     clocks = sampler.stop()
     c1 = ctx.counters()
     ms = np.array([a.elapsed_time(b) for a, b in ev])
-    tot = torch.tensor([float(ms.sum())], device=dev)
+    tot = torch.tensor([float(ms.sum())], device=dev if on_dev else "cpu")
     if world > 1:
         dist.all_reduce(tot, op=dist.ReduceOp.MAX)
     total_ms = float(tot.item())
@@ -229,7 +234,7 @@ def run_gpu(args):
         if s > 0:
             e2e_ms.append(1e3 * (time.perf_counter() - t0))
         c2.close()
-    e2e_t = torch.tensor([float(np.mean(e2e_ms))], device=dev)
+    e2e_t = torch.tensor([float(np.mean(e2e_ms))], device=dev if on_dev else "cpu")
     if world > 1:
         dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
     h2d = P_host.numel() * 4 * (2 if wl.per_bin_weights else 1) + wl.n_sft * (8 + 24 + 4) + g.sky.size * 8
@@ -292,6 +297,8 @@ def main():
     ap.add_argument("--fused", type=int, default=1)
     ap.add_argument("--ppc", type=int, default=0, help="outer points per CTA (0 = library default)")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per launch (from profiles/)")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="gloo: exercise the N>1 path with every rank on one GPU (testing only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
