@@ -144,9 +144,10 @@ ft_tile_kernel(const __grid_constant__ FtDev d, const __grid_constant__ FtTileAr
 #pragma unroll
             for (int j = 0; j < J; ++j)
               if (j < J - 1 || last_ok) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v[j]) : "r"(ad + 128u * j));
+            if (!last_ok) v[J - 1] = 0.f;
 #pragma unroll
-            for (int j = 0; j < J; ++j)
-              if (j < J - 1 || last_ok) acc[j] += v[j];
+            for (int j = 0; j + 1 < J; j += 2) ft_add2(acc[j], acc[j + 1], v[j], v[j + 1]);
+            if (J & 1) acc[J - 1] += v[J - 1];
           } else {
             const uint32_t ad_lo = base + 4u * (e & 8191u);
             const uint32_t ad_hi = (e & (1u << 24)) ? ad_lo - 4u : ad_lo + 4u;

@@ -68,6 +68,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
+// (a0, a1) += (v0, v1) as ONE instruction: sm_100's packed fp32 add (SASS FADD2), round-to-nearest like FADD
+__device__ __forceinline__ void ft_add2(float& a0, float& a1, float v0, float v1) {
+  unsigned long long a2, v2;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(a2) : "f"(a0), "f"(a1));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(v2) : "f"(v0), "f"(v1));
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(a2) : "l"(a2), "l"(v2));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a0), "=f"(a1) : "l"(a2));
+}
+
 // Packed per-(warp, SFT) track entry: bits 0-12 strip offset of the warp's first output (floats),
 // bits 13-23 break position relative to the warp's first output (0 = no break in the warp's range),
 // bit 24 set when the shift decreases at the break.  No break <=> entry < 8192.
