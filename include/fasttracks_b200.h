@@ -70,6 +70,8 @@ typedef enum { FT_W_PER_SFT = 1, FT_W_PER_SFT_BIN = 2 } ft_wkind;
  *                        used as given (Eq. 4-5 are the caller's; no renormalisation).
  *   f_min, df            frequency of bin 0 and bin width (= 1/T_SFT, :248), Hz; df > 0.
  *   cuda_stream          a cudaStream_t (NULL = default stream); all work of the handle runs on it.
+ * ft_create also builds the library-owned gather array Q[a][k] = fl(fl(w P) - c_a), c_a the row mean
+ * (one pass over P on the stream), and synchronises the stream.
  */
 int ft_create(ft_ctx** out, const float* P_dev, int64_t n_sft, int64_t n_bins, int64_t ld_bins,
               const double* t_mid_host, const double* vel_host, const float* w, int wkind,
@@ -100,10 +102,11 @@ typedef struct {
  *   Both NULL: bind the grid only (for ft_topk_per_band); no statistic kernel is launched.
  * Validation before any launch: finite arguments, positive sizes, and a conservative bound on
  * every track of the grid must stay inside [0, n_bins) else FT_ERR_TRACK_RANGE (so kernels need
- * no per-evaluation bounds check).  Kernel choice: the tile kernel (TMA-staged strips, fp32
- * two-level accumulation, bins bit-identical to the canonical arithmetic except within 1e-9 bin of
- * a rounding tie) when df0 == df; otherwise the generic kernel (canonical arithmetic per
- * evaluation, fp64 accumulation).  Asynchronous on the handle's stream.
+ * no per-evaluation bounds check).  Kernel choice: the tile kernel (TMA-staged strips, fp32 accumulation
+ * of the folded, row-centred array Q = w P - c_row, bins bit-identical to the canonical arithmetic except
+ * within 1e-9 bin of a rounding tie; number count on a packed byte hit map, exact) when df0 == df;
+ * otherwise the generic kernel (canonical arithmetic per evaluation, fp64 accumulation).  Asynchronous
+ * on the handle's stream.
  */
 int ft_eval(ft_ctx* ctx, const ft_grid* grid, int stat, double rho_th, float* out_power_dev,
             int32_t* out_count_dev);

@@ -106,7 +106,6 @@ cudaError_t ft_launch_generic(const FtDev& d, int stat, uint64_t pt_begin, uint6
                               cudaStream_t s);
 cudaError_t ft_launch_refine(const FtDev& d, const uint64_t* idx_dev, const uint32_t* n_dev, int64_t n_max,
                              FtCandDev* out, unsigned long long* near_ties, cudaStream_t s);
-cudaError_t ft_launch_fold(const float* P, const float* w, float* Q, int64_t n, cudaStream_t s);
 // ctab[(i_porb*n_tasc + i_tasc)][a] = cos(Om (t_mid[a] - t_asc)), the same expression ft_doppler evaluates
 cudaError_t ft_launch_ctab(const FtDev& d, double* ctab, cudaStream_t s);
 // K1: explicit template list (records of 8 doubles: f0, f1, nx, ny, nz, a_p, P_orb, t_asc), device memory

@@ -110,13 +110,6 @@ ft_refine_kernel(const __grid_constant__ FtDev d, const uint64_t* __restrict__ i
   }
 }
 
-__global__ void ft_fold_kernel(const float* __restrict__ P, const float* __restrict__ w,
-                               float* __restrict__ Q, int64_t n) {
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-    Q[i] = __fmul_rn(w[i], P[i]);
-}
-
 // K1: an explicit list of templates (an unstructured bank: "no assumption on the properties of
 // lambda"; random banks :312-316).  One thread per template, the canonical fp64 track
 // per (template, SFT), gather through L1/L2, fp64 accumulation in ascending SFT order.  Nothing can
@@ -228,10 +221,6 @@ cudaError_t ft_launch_refine(const FtDev& d, const uint64_t* idx_dev, const uint
   return cudaGetLastError();
 }
 
-cudaError_t ft_launch_fold(const float* P, const float* w, float* Q, int64_t n, cudaStream_t s) {
-  ft_fold_kernel<<<148 * 8, 256, 0, s>>>(P, w, Q, n);
-  return cudaGetLastError();
-}
 
 cudaError_t ft_launch_list(const FtDev& d, int stat, const void* templates_dev, int64_t n, double t_ref,
                            float* out_power, int32_t* out_count, int32_t* err, unsigned long long* near_ties,
