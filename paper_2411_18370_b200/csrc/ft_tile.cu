@@ -323,8 +323,9 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   pl.mode = mode; pl.cw = cw;
   pl.tile_w = (int32_t)(((chunks + bT - 1) / bT) * cw);
   pl.n_tiles = (int32_t)((d.n_f0 + pl.tile_w - 1) / pl.tile_w);
-  // default: ~20 consumer warps per CTA (measured best on B200: R = 10 at wpp = 2, R = 23 at wpp = 1)
-  int R = in.points_per_cta > 0 ? in.points_per_cta : (pl.wpp == 1 ? 23 : 20 / pl.wpp);
+  // default: 24-27 consumer warps per CTA (measured best on B200 at 72 registers: R = 12 at wpp = 2,
+  // R = 6 at wpp = 4, R = 27 at wpp = 1); the packed kernel keeps 23 (80 registers)
+  int R = in.points_per_cta > 0 ? in.points_per_cta : (mode == 1 ? 23 : (pl.wpp == 1 ? 27 : 24 / pl.wpp));
   const int max_threads = mode == 1 ? ft_tile8_max_threads(pl.J) : ft_tile_max_threads(pl.J);
   R = std::min<int>(R, (max_threads / 32 - 1) / pl.wpp);  // + 1 producer warp
   R = (int)std::min<uint64_t>((uint64_t)R, d.n_points);

@@ -27,9 +27,9 @@ struct FtTileArgs {
 
 // Threads per CTA the kernel is compiled for: (consumer warps + 1 producer warp) * 32.  The
 // accumulators (J) and the loads in flight (J) set the register need, hence the bound.
-// (the register file is 4 x 16 384: 80 registers allow 6 warps per SM sub-partition, 64 allow 8)
-__host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : 80; }
-__host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 1024 : 768; }
+// (the register file is 4 x 16 384: 80 registers allow 6 warps per SM sub-partition, 72 allow 7, 64 allow 8)
+__host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : 72; }
+__host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 1024 : 896; }
 // packed number-count kernel: J registers of 8-bit counters + J loads in flight (16-bit levels in shared memory)
 __host__ __device__ constexpr int ft_tile8_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tile8_max_threads(int J) { return J <= 8 ? 1024 : 768; }
