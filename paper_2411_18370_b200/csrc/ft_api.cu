@@ -23,8 +23,11 @@ struct ft_ctx {
   float* H_dev = nullptr;       // hit map (tile kernel input for the number count)
   float H_rho = 0.f; bool H_valid = false;
   double add_back = 0.0;        // sum over SFTs of the per-row constant the fold removed from Q
-  double* axes_dev = nullptr;   // sky | a_p | P_orb | tasc
-  double* ctab_dev = nullptr;   // orbital cosine table of the bound grid (binary grids)
+  double* axes_dev = nullptr;   // sky | a_p | P_orb | tasc (grow-only buffer)
+  size_t axes_cap = 0;
+  double* ctab_dev = nullptr;   // orbital cosine table of the bound grid (binary grids; grow-only buffer)
+  size_t ctab_cap = 0;
+  std::vector<double> ctab_key; // (t_ref, P_orb[], tasc_frac[]) the table was built for
   // host copies used for validation
   std::vector<double> t_mid, vel;
   double vmax = 0.0, dt_min = 0.0, dt_max = 0.0;
@@ -313,8 +316,12 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   std::memcpy(ax.data() + o, g->P_orb, sizeof(double) * g->n_porb); o += g->n_porb;
   std::memcpy(ax.data() + o, g->tasc_frac, sizeof(double) * g->n_tasc);
   FT_CUDA(c, cudaStreamSynchronize(c->stream));  // previous work may still read the old axes
-  dfree(c->axes_dev);
-  FT_CUDA(c, cudaMalloc(&c->axes_dev, sizeof(double) * n_ax));
+  if (c->axes_cap < n_ax) {
+    dfree(c->axes_dev);
+    c->axes_cap = 0;
+    FT_CUDA(c, cudaMalloc(&c->axes_dev, sizeof(double) * n_ax));
+    c->axes_cap = n_ax;
+  }
   FT_CUDA(c, cudaMemcpyAsync(c->axes_dev, ax.data(), sizeof(double) * n_ax, cudaMemcpyHostToDevice, c->stream));
   FT_CUDA(c, cudaStreamSynchronize(c->stream));
   FtDev& d = c->d;
@@ -325,13 +332,25 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   d.n_points = (uint64_t)g->n_sky * g->n_ap * g->n_porb * g->n_tasc * g->n_f1;
   c->stat = stat;
   // binary grids: cos(Om (t - t_asc)) per (P_orb, t_asc, SFT) once, shared by every a_p (<= 1 GiB)
-  dfree(c->ctab_dev);
+  // (rebuilt only when t_ref, P_orb[] or tasc_frac[] change: the table does not depend on anything else)
   d.ctab = nullptr;
   const size_t ctab_elems = (size_t)g->n_porb * g->n_tasc * (size_t)d.n_sft;
   if (ap_max != 0.0 && g->n_porb * (int64_t)g->n_tasc <= 65535 && ctab_elems <= ((size_t)1 << 27)) {
-    FT_CUDA(c, cudaMalloc(&c->ctab_dev, sizeof(double) * ctab_elems));
-    FT_CUDA(c, ft_launch_ctab(d, c->ctab_dev, c->stream));
-    c->counters.kernel_launches += 1;
+    std::vector<double> key;
+    key.push_back(g->t_ref); key.push_back((double)g->n_porb); key.push_back((double)g->n_tasc);
+    key.insert(key.end(), g->P_orb, g->P_orb + g->n_porb);
+    key.insert(key.end(), g->tasc_frac, g->tasc_frac + g->n_tasc);
+    if (c->ctab_cap < ctab_elems) {
+      dfree(c->ctab_dev);
+      c->ctab_cap = 0; c->ctab_key.clear();
+      FT_CUDA(c, cudaMalloc(&c->ctab_dev, sizeof(double) * ctab_elems));
+      c->ctab_cap = ctab_elems;
+    }
+    if (key != c->ctab_key) {
+      FT_CUDA(c, ft_launch_ctab(d, c->ctab_dev, c->stream));
+      c->counters.kernel_launches += 1;
+      c->ctab_key = key;
+    }
     d.ctab = c->ctab_dev;
   }
   // tile-kernel eligibility and plan
@@ -348,7 +367,6 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   }
   // number count: the packed kernel when it is eligible (n_sft <= 65535), else the fp32 0/1 map
   c->tile8_ok = false;
-  ft_tile_plan_free(&c->plan8);
   if (c->tile_ok && stat != FT_STAT_POWER && c->opt_packed) {
     std::string why8;
     int launches = 0;

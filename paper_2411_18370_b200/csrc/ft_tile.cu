@@ -282,6 +282,7 @@ cudaError_t launch_any(int J, const FtDev& d, const FtTileArgs& a, unsigned grid
 void ft_tile_plan_free(FtTilePlan* p) {
   if (p->kst) cudaFree(p->kst);
   if (p->err) cudaFree(p->err);
+  if (p->vr) cudaFree(p->vr);
   *p = FtTilePlan{};
 }
 
@@ -289,7 +290,9 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
                          std::string* why, int* launches, int mode) {
   *launches = 0;
   why->clear();
-  ft_tile_plan_free(plan);
+  FtTilePlan pl;  // geometry starts from defaults; the device buffers of *plan are kept and reused
+  pl.kst = plan->kst; pl.kst_cap = plan->kst_cap; pl.err = plan->err; pl.vr = plan->vr; pl.vr_cap = plan->vr_cap;
+  *plan = pl;     // (an ineligible return leaves a plan with buffers only)
   if (d.df0 != in.df && d.n_f0 > 1) { *why = "f0 step differs from the bin width"; return cudaSuccess; }
   if (!d.Q) { *why = "no folded array"; return cudaSuccess; }
   if (d.n_f0 > (1 << 30)) { *why = "more than 2^30 f0 values"; return cudaSuccess; }
@@ -318,7 +321,6 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
     if (cpt == 1) break;
   }
   if (bJ == 0) { *why = "Doppler spread too large for a single break per warp range"; return cudaSuccess; }
-  FtTilePlan pl;
   pl.J = bJ; pl.wpp = bW;
   pl.mode = mode; pl.cw = cw;
   pl.tile_w = (int32_t)(((chunks + bT - 1) / bT) * cw);
@@ -331,15 +333,18 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   R = (int)std::min<uint64_t>((uint64_t)R, d.n_points);
   pl.R = std::max(R, 1);
   // --- point-independent strip bounds per (tile, SFT) -----------------------------------------------
-  double* vr_dev = nullptr;
-  cudaError_t e = cudaMalloc(&vr_dev, sizeof(double) * 2 * n_sft);
-  if (e != cudaSuccess) return e;
-  ft_vrange_kernel<<<(unsigned)n_sft, 256, 0, s>>>(d.vel, d.sky, d.n_sky, vr_dev);
+  if (pl.vr_cap < 2 * (size_t)n_sft) {
+    if (pl.vr) cudaFree(pl.vr);
+    pl.vr = nullptr; pl.vr_cap = 0; plan->vr = nullptr; plan->vr_cap = 0;
+    const cudaError_t ea = cudaMalloc(&pl.vr, sizeof(double) * 2 * n_sft);
+    if (ea != cudaSuccess) return ea;
+    pl.vr_cap = 2 * (size_t)n_sft; plan->vr = pl.vr; plan->vr_cap = pl.vr_cap;
+  }
+  ft_vrange_kernel<<<(unsigned)n_sft, 256, 0, s>>>(d.vel, d.sky, d.n_sky, pl.vr);
   *launches += 1;
   std::vector<double> vr(2 * (size_t)n_sft);
-  e = cudaMemcpyAsync(vr.data(), vr_dev, sizeof(double) * 2 * n_sft, cudaMemcpyDeviceToHost, s);
+  cudaError_t e = cudaMemcpyAsync(vr.data(), pl.vr, sizeof(double) * 2 * n_sft, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  cudaFree(vr_dev);
   if (e != cudaSuccess) return e;
   double bmax = 0.0;
   {
@@ -401,13 +406,22 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   pl.n_stages = (int32_t)(rows_fit / kRPS);
   pl.ctas_per_sm = ctas;
   pl.smem_bytes = (size_t)pl.n_stages * pl.rows_per_stage * row_bytes + 2 * 8 * (size_t)pl.n_stages + state_bytes;
-  e = cudaMalloc(&pl.kst, sizeof(int32_t) * kst.size());
-  if (e != cudaSuccess) return e;
-  e = cudaMalloc(&pl.err, sizeof(int32_t));
-  if (e == cudaSuccess) e = cudaMemcpyAsync(pl.kst, kst.data(), sizeof(int32_t) * kst.size(), cudaMemcpyHostToDevice, s);
+  if (pl.kst_cap < kst.size()) {
+    if (pl.kst) cudaFree(pl.kst);
+    pl.kst = nullptr; pl.kst_cap = 0; plan->kst = nullptr; plan->kst_cap = 0;
+    e = cudaMalloc(&pl.kst, sizeof(int32_t) * kst.size());
+    if (e != cudaSuccess) return e;
+    pl.kst_cap = kst.size(); plan->kst = pl.kst; plan->kst_cap = pl.kst_cap;
+  }
+  if (!pl.err) {
+    e = cudaMalloc(&pl.err, sizeof(int32_t));
+    if (e != cudaSuccess) return e;
+    plan->err = pl.err;
+  }
+  e = cudaMemcpyAsync(pl.kst, kst.data(), sizeof(int32_t) * kst.size(), cudaMemcpyHostToDevice, s);
   if (e == cudaSuccess) e = cudaMemsetAsync(pl.err, 0, sizeof(int32_t), s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);  // kst (host vector) goes out of scope
-  if (e != cudaSuccess) { ft_tile_plan_free(&pl); return e; }
+  if (e != cudaSuccess) return e;
   *plan = pl;
   return cudaSuccess;
 }

@@ -6,8 +6,12 @@
 #include "ft_select.cuh"
 
 struct FtTilePlan {
-  int32_t* kst = nullptr;       // device [n_tiles][n_sft] first staged bin of the strip (multiple of 4)
-  int32_t* err = nullptr;       // device [1] set by the kernel if a track left its staged strip (plan bug)
+  // device buffers, grow-only across ft_tile_plan calls on the same plan object (freed by ft_tile_plan_free)
+  int32_t* kst = nullptr;       // [n_tiles][n_sft] first staged bin of the strip (multiple of 4 / 16)
+  size_t kst_cap = 0;
+  int32_t* err = nullptr;       // [1] set by the kernel if a track left its staged strip (plan bug)
+  double* vr = nullptr;         // [n_sft][2] scratch of the sky-axis velocity range
+  size_t vr_cap = 0;
   int32_t mode = 0;             // 0: fp32 gather (ft_tile_kernel), 1: packed number count (ft_tile8_kernel)
   int32_t cw = 32;              // f0 per chunk (per warp load instruction): 32 or 128
   int32_t n_tiles = 0;          // f0 tiles
