@@ -176,6 +176,7 @@ def run_gpu(args):
     ctx.set_option(B.FT_OPT_KERNEL, args.kernel)
     ctx.set_option(B.FT_OPT_FUSED_TOPK, args.fused)
     ctx.set_option(B.FT_OPT_POINTS_PER_CTA, args.ppc)
+    ctx.set_option(B.FT_OPT_F0_TILES, args.tiles)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     evals = g.n_templates * wl.n_sft
 
@@ -228,7 +229,7 @@ def run_gpu(args):
             wa = torch.empty_like(w_arg); wa.copy_(w_host, non_blocking=True)
         c2 = B.Context(Pd, wl.t_mid, wl.vel, wa, wl.f_min, wl.df, stream)
         c2.set_option(B.FT_OPT_KERNEL, args.kernel); c2.set_option(B.FT_OPT_FUSED_TOPK, args.fused)
-        c2.set_option(B.FT_OPT_POINTS_PER_CTA, args.ppc)
+        c2.set_option(B.FT_OPT_POINTS_PER_CTA, args.ppc); c2.set_option(B.FT_OPT_F0_TILES, args.tiles)
         cands = step(c2)
         barrier()
         if s > 0:
@@ -295,6 +296,7 @@ def main():
     ap.add_argument("--n-sft", type=int, default=0)
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 tile")
     ap.add_argument("--fused", type=int, default=1)
+    ap.add_argument("--tiles", type=int, default=0, help="f0 tiles (0 = library default)")
     ap.add_argument("--ppc", type=int, default=0, help="outer points per CTA (0 = library default)")
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per launch (from profiles/)")
     ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],

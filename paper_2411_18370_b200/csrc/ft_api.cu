@@ -42,7 +42,7 @@ struct ft_ctx {
   uint8_t* H8_dev = nullptr;    // four byte-shifted hit maps
   float H8_rho = 0.f; bool H8_valid = false;
   // options
-  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1;
+  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0;
   // selection buffers
   FtSelectDev sel{};
   uint64_t* final_idx = nullptr;
@@ -265,6 +265,7 @@ int ft_set_option(ft_ctx* c, int option, int64_t value) {
     case FT_OPT_KERNEL: if (value < 0 || value > 2) return fail(c, FT_ERR_ARG, "FT_OPT_KERNEL: 0..2"); c->opt_kernel = value; break;
     case FT_OPT_FUSED_TOPK: c->opt_fused = value ? 1 : 0; break;
     case FT_OPT_PACKED_COUNT: c->opt_packed = value ? 1 : 0; break;
+    case FT_OPT_F0_TILES: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_F0_TILES >= 0"); c->opt_tiles = value; break;
     case FT_OPT_POINTS_PER_CTA: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_POINTS_PER_CTA >= 0"); c->opt_ppc = value; break;
     default: return fail(c, FT_ERR_ARG, "unknown option");
   }
@@ -358,7 +359,7 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   if (c->opt_kernel != 1) {
     std::string& why = c->why;
     int launches = 0;
-    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc};
+    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc, (int)c->opt_tiles};
     const cudaError_t e = ft_tile_plan(d, hin, c->stream, &c->plan, &why, &launches);
     c->counters.kernel_launches += launches;
     if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_tile_plan: ") + cudaGetErrorString(e));
@@ -370,7 +371,7 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   if (c->tile_ok && stat != FT_STAT_POWER && c->opt_packed) {
     std::string why8;
     int launches = 0;
-    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc};
+    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc, (int)c->opt_tiles};
     const cudaError_t e = ft_tile_plan(d, hin, c->stream, &c->plan8, &why8, &launches, 1);
     c->counters.kernel_launches += launches;
     if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_tile_plan (packed): ") + cudaGetErrorString(e));

@@ -307,8 +307,9 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   int bJ = 0, bW = 0; int64_t bT = 0;
   const int maxJ_eps = (int)std::floor(0.45 / ((double)cw * std::fmax(in.eps_bound, 1e-12)));
   for (int64_t nt = 1; nt <= chunks; ++nt) {
+    if (in.force_tiles > 0 && nt != in.force_tiles) continue;
     const int64_t cpt = (chunks + nt - 1) / nt;
-    if (nt > 1 && (chunks + nt - 2) / (nt - 1) == cpt) continue;  // same tile size as nt-1
+    if (nt > 1 && in.force_tiles <= 0 && (chunks + nt - 2) / (nt - 1) == cpt) continue;  // same tile size as nt-1
     for (int wpp = 1; wpp <= 4; ++wpp) {
       const int64_t Jn = (cpt + wpp - 1) / wpp;
       if (Jn > (mode == 1 ? 16 : 32)) continue;

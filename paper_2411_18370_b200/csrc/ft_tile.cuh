@@ -34,6 +34,7 @@ struct FtTileHostIn {
   const double* sky; const double* a_p; const double* P_orb;
   double df; double eps_bound;
   int points_per_cta;
+  int force_tiles;  // > 0: use exactly this many f0 tiles (FT_OPT_F0_TILES)
 };
 cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s, FtTilePlan* plan,
                          std::string* why, int* launches, int mode = 0);
