@@ -120,7 +120,7 @@ class Context:
                                 C.c_void_p(self.stream.cuda_stream))
         self._check(rc)
         self.n_templates = 0
-        self.k = 0
+        self._n_f0, self._df0 = 1, 0.0
 
     def _check(self, rc):
         if rc != 0:
@@ -137,13 +137,17 @@ class Context:
                    float(grid.df1), int(grid.n_f1), float(grid.t_ref), len(ax[0]), _hp(ax[0]),
                    len(ax[1]), _hp(ax[1]), len(ax[2]), _hp(ax[2]), len(ax[3]), _hp(ax[3]))
         self.n_templates = len(ax[0]) * len(ax[1]) * len(ax[2]) * len(ax[3]) * int(grid.n_f1) * int(grid.n_f0)
+        self._n_f0, self._df0 = int(grid.n_f0), float(grid.df0)
         for o in (out_power, out_count):
             assert o is None or (o.is_cuda and o.numel() == self.n_templates and o.is_contiguous())
         pp = C.c_void_p(out_power.data_ptr()) if out_power is not None else None
         pc = C.c_void_p(out_count.data_ptr()) if out_count is not None else None
         self._check(self.lib.ft_eval(self.h, C.byref(g), FT_STAT[stat], float(rho_th), pp, pc))
 
-    def topk_per_band(self, band_width_hz: float, k: int, n_bands_max: int):
+    def topk_per_band(self, band_width_hz: float, k: int, n_bands_max: int = 0):
+        # the C call writes n_bands * k records: size the buffer from the bound grid, not from the caller
+        bpb = max(1, int(round(band_width_hz / self._df0))) if self._df0 > 0 else 1
+        n_bands_max = max(int(n_bands_max), -(-self._n_f0 // bpb), 1)
         out = np.zeros((n_bands_max, k), dtype=CAND_DTYPE)
         nb = C.c_int32(0)
         self._check(self.lib.ft_topk_per_band(self.h, float(band_width_hz), int(k), _hp(out), C.byref(nb)))
