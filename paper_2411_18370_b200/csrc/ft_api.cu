@@ -42,7 +42,7 @@ struct ft_ctx {
   uint8_t* H8_dev = nullptr;    // four byte-shifted hit maps
   float H8_rho = 0.f; bool H8_valid = false;
   // options
-  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0;
+  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0, opt_cap = 0;
   // selection buffers
   FtSelectDev sel{};
   uint64_t* final_idx = nullptr;
@@ -101,6 +101,7 @@ void free_select(ft_ctx* c) {
 int ensure_select(ft_ctx* c, int32_t n_bands, int32_t k) {
   uint32_t cap = (uint32_t)((1u << 24) / (uint32_t)n_bands);
   cap = cap > 65536u ? 65536u : (cap < 4096u ? 4096u : cap);
+  if (c->opt_cap > 0) cap = (uint32_t)c->opt_cap;  // FT_OPT_SELECT_CAP (tests of the overflow recovery)
   const uint32_t final_cap = (uint32_t)n_bands * 2048u;
   if (c->sel.n_bands != n_bands || c->sel.cap != cap || c->out_cap < (size_t)n_bands * k) {
     free_select(c);
@@ -265,6 +266,7 @@ int ft_set_option(ft_ctx* c, int option, int64_t value) {
     case FT_OPT_KERNEL: if (value < 0 || value > 2) return fail(c, FT_ERR_ARG, "FT_OPT_KERNEL: 0..2"); c->opt_kernel = value; break;
     case FT_OPT_FUSED_TOPK: c->opt_fused = value ? 1 : 0; break;
     case FT_OPT_PACKED_COUNT: c->opt_packed = value ? 1 : 0; break;
+    case FT_OPT_SELECT_CAP: if (value < 0 || value > (1 << 20)) return fail(c, FT_ERR_ARG, "FT_OPT_SELECT_CAP: 0 .. 2^20"); c->opt_cap = value; break;
     case FT_OPT_F0_TILES: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_F0_TILES >= 0"); c->opt_tiles = value; break;
     case FT_OPT_POINTS_PER_CTA: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_POINTS_PER_CTA >= 0"); c->opt_ppc = value; break;
     default: return fail(c, FT_ERR_ARG, "unknown option");

@@ -164,3 +164,30 @@ def test_packed_number_count_equals_fp32_map_and_oracle(band_hz, n_sft, n_sky, p
     op = fo.Oracle(wl).eval_range()[0]
     H.assert_topk_parity(wl, cands, oc, op, oc, wl.k, bpb, by_count=True)
     ctx.close()
+
+
+def test_selection_overflow_recovery_and_forced_tiling():
+    """The threshold sample is the first 296 CTA groups here (the bank is barely larger than the
+    sample); 70 loud injections sit in the LAST a_p values, outside the sample, and flood the band's small append buffer (FT_OPT_SELECT_CAP) in the fused pass: the library tightens
+    the threshold from the entries it kept and repeats the pass (refine_fallbacks > 0); the candidates
+    still equal the oracle's.  Also forces 3 f0 tiles on a band one tile could hold."""
+    from paper_2411_18370_b200 import binding as B
+    wl = W.config3(n_sft=96, n_ap=24, n_porb=24, n_tasc=16, n_inj=0)
+    rng = np.random.Generator(np.random.PCG64(11))
+    wl.planned_injections = [((0, int(rng.integers(21, 24)), int(rng.integers(24)), int(rng.integers(16)), 0,
+                               198 + int(rng.integers(9))), 3.0) for _ in range(70)]   # 70 loud tracks, one band (22)
+    wl = H.apply_injections(wl)
+    g = wl.grid
+    o = fo.Oracle(wl)
+    op, oc, _, _ = o.eval_range()
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    ctx = H.gpu_context(wl, kernel=2)
+    ctx.set_option(B.FT_OPT_SELECT_CAP, 48)
+    ctx.set_option(B.FT_OPT_F0_TILES, 3)
+    ctx.eval(g, "power", wl.rho_th)
+    assert "n_tiles=3" in ctx.describe()
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    H.assert_topk_parity(wl, cands, op, op, oc, wl.k, bpb)
+    c = ctx.counters()
+    assert c["refine_fallbacks"] >= 1, c
+    ctx.close()
