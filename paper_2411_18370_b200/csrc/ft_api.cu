@@ -42,7 +42,7 @@ struct ft_ctx {
   uint8_t* H8_dev = nullptr;    // four byte-shifted hit maps
   float H8_rho = 0.f; bool H8_valid = false;
   // options
-  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0, opt_cap = 0;
+  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0, opt_cap = 0, opt_floor = 0;
   // selection buffers
   FtSelectDev sel{};
   uint64_t* final_idx = nullptr;
@@ -54,6 +54,8 @@ struct ft_ctx {
   size_t out_cap = 0;
   float* scratch_f = nullptr;
   int32_t* scratch_i = nullptr;
+  int32_t* veto_cnt = nullptr;  // number count of every template (FT_OPT_COUNT_FLOOR), grow-only
+  size_t veto_cap = 0;
   size_t scratch_elems = 0;
   unsigned long long* near_ties_dev = nullptr;
   // bookkeeping
@@ -267,6 +269,7 @@ int ft_set_option(ft_ctx* c, int option, int64_t value) {
     case FT_OPT_FUSED_TOPK: c->opt_fused = value ? 1 : 0; break;
     case FT_OPT_PACKED_COUNT: c->opt_packed = value ? 1 : 0; break;
     case FT_OPT_SELECT_CAP: if (value < 0 || value > (1 << 20)) return fail(c, FT_ERR_ARG, "FT_OPT_SELECT_CAP: 0 .. 2^20"); c->opt_cap = value; break;
+    case FT_OPT_COUNT_FLOOR: if (value < 0 || value > (1 << 24)) return fail(c, FT_ERR_ARG, "FT_OPT_COUNT_FLOOR: 0 .. 2^24"); c->opt_floor = value; break;
     case FT_OPT_F0_TILES: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_F0_TILES >= 0"); c->opt_tiles = value; break;
     case FT_OPT_POINTS_PER_CTA: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_POINTS_PER_CTA >= 0"); c->opt_ppc = value; break;
     default: return fail(c, FT_ERR_ARG, "unknown option");
@@ -447,6 +450,24 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
   FT_CUDA(c, ft_select_reset(c->sel, c->final_n, overflow, c->stream));
   c->counters.kernel_launches += 1;
   c->ev_used = 0; c->counters.stat_launches = 0;
+  // Number-count veto (the loudest normalized power "with the extra restriction of
+  // scoring at least a pre-established ... number count"): when both statistics are bound and a floor
+  // is set, one pass of the number count over the whole bank first; the power selection then skips
+  // every template below the floor.
+  const int32_t floor = (c->stat == FT_STAT_BOTH) ? (int32_t)c->opt_floor : 0;
+  c->sel.veto_cnt = nullptr; c->sel.veto_floor = 0;
+  if (floor > 0) {
+    const uint64_t n_templates = d.n_points * (uint64_t)d.n_f0;
+    if (n_templates > ((uint64_t)1 << 34)) return fail(c, FT_ERR_ALLOC, "ft_topk_per_band: count floor needs 4 B per template (bank too large)");
+    if (c->veto_cap < n_templates) {
+      dfree(c->veto_cnt); c->veto_cap = 0;
+      FT_CUDA(c, cudaMalloc(&c->veto_cnt, sizeof(int32_t) * n_templates));
+      c->veto_cap = n_templates;
+    }
+    rc = run_stat(c, FT_STAT_HOUGH, 0, d.n_points, nullptr, c->veto_cnt, 0, false, (int32_t)bpb);
+    if (rc != FT_OK) return rc;
+    c->sel.veto_cnt = c->veto_cnt; c->sel.veto_floor = floor;
+  }
   std::vector<uint32_t> cnt(n_bands);
   if (fused) {
     // Phase A: per-band thresholds from a strided sample of point groups (every stride-th CTA group
@@ -471,6 +492,10 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
                     by_count ? c->scratch_i : nullptr, 0, false, (int32_t)bpb);
     if (rc != FT_OK) return rc;
     if (by_count) { FT_CUDA(c, ft_count_to_key(c->scratch_i, c->scratch_f, rows * d.n_f0, c->stream)); c->counters.kernel_launches += 1; }
+    if (floor > 0) {
+      FT_CUDA(c, ft_select_mask_keys(c->scratch_f, rows, d.n_f0, 0, (uint32_t)R, (uint32_t)stride, d.n_points, c->veto_cnt, floor, c->stream));
+      c->counters.kernel_launches += 1;
+    }
     FT_CUDA(c, ft_select_threshold(c->scratch_f, rows, d.n_f0, (int32_t)bpb, (uint32_t)k, margin, c->sel, c->stream));
     c->counters.kernel_launches += 1;
     // Phase B: the sample's own survivors from the scratch array, the rest of the bank through the
@@ -508,6 +533,10 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
       if (rc != FT_OK) return rc;
       const int64_t rows = (int64_t)(pe - pt);
       if (by_count) { FT_CUDA(c, ft_count_to_key(c->scratch_i, c->scratch_f, rows * d.n_f0, c->stream)); c->counters.kernel_launches += 1; }
+      if (floor > 0) {
+        FT_CUDA(c, ft_select_mask_keys(c->scratch_f, rows, d.n_f0, pt, 1, 1, d.n_points, c->veto_cnt, floor, c->stream));
+        c->counters.kernel_launches += 1;
+      }
       FT_CUDA(c, ft_select_threshold(c->scratch_f, rows, d.n_f0, (int32_t)bpb, (uint32_t)k, margin, c->sel, c->stream));
       FT_CUDA(c, ft_select_append_keys(c->scratch_f, rows, d.n_f0, (int32_t)bpb, pt, c->sel, c->stream));
       c->counters.kernel_launches += 2;
@@ -614,7 +643,7 @@ void ft_destroy(ft_ctx* c) {
   ft_tile_plan_free(&c->plan8);
   dfree(c->H8_dev);
   dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->H_dev); dfree(c->ctab_dev); dfree(c->axes_dev);
-  dfree(c->scratch_f); dfree(c->scratch_i); dfree(c->near_ties_dev);
+  dfree(c->scratch_f); dfree(c->scratch_i); dfree(c->veto_cnt); dfree(c->near_ties_dev);
   for (cudaEvent_t e : c->evs) cudaEventDestroy(e);
   delete c;
 }

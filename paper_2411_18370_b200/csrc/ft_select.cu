@@ -181,6 +181,18 @@ ft_rank_kernel(const FtCandDev* __restrict__ cand, const int32_t* __restrict__ c
   }
 }
 
+__global__ void ft_mask_keys_kernel(float* __restrict__ keys, int64_t n_rows, int64_t n_f0, uint64_t pt_begin,
+                                    uint32_t R, uint32_t gstride, uint64_t pt_end,
+                                    const int32_t* __restrict__ veto_cnt, int32_t floor) {
+  const int64_t n = n_rows * n_f0;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
+    const uint64_t r = (uint64_t)(e / n_f0);
+    const uint64_t pt = pt_begin + (r / R) * (uint64_t)gstride * R + r % R;
+    if (pt < pt_end && veto_cnt[pt * (uint64_t)n_f0 + (uint64_t)(e % n_f0)] < floor) keys[e] = -INFINITY;
+  }
+}
+
 __global__ void ft_fill_f32_kernel(float* p, int64_t n, float v) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) p[i] = v;
@@ -247,5 +259,14 @@ cudaError_t ft_select_tighten(FtSelectDev sel, uint32_t k, float rel_margin, cud
 cudaError_t ft_fill_f32(float* p, int64_t n, float v, cudaStream_t s) {
   const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
   ft_fill_f32_kernel<<<grid, 256, 0, s>>>(p, n, v);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_select_mask_keys(float* keys, int64_t n_rows, int64_t n_f0, uint64_t pt_begin, uint32_t R,
+                                uint32_t stride, uint64_t pt_end, const int32_t* veto_cnt, int32_t floor,
+                                cudaStream_t s) {
+  const int64_t n = n_rows * n_f0;
+  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  ft_mask_keys_kernel<<<grid, 256, 0, s>>>(keys, n_rows, n_f0, pt_begin, R ? R : 1, stride ? stride : 1, pt_end, veto_cnt, floor);
   return cudaGetLastError();
 }

@@ -9,9 +9,13 @@ struct FtSelectDev {
   uint64_t* idx;   // [n_bands][cap]
   uint32_t cap;
   int32_t n_bands;
+  // number-count veto: templates with veto_cnt[idx] < veto_floor are not candidates
+  const int32_t* veto_cnt;  // [n_templates] integer number count, or nullptr
+  int32_t veto_floor;
 };
 
 __device__ __forceinline__ void ft_select_append(const FtSelectDev& sel, int band, float key, uint64_t idx) {
+  if (sel.veto_cnt && __ldg(sel.veto_cnt + idx) < sel.veto_floor) return;
   const uint32_t slot = atomicAdd(sel.cnt + band, 1u);
   if (slot < sel.cap) {
     sel.key[(size_t)band * sel.cap + slot] = key;
@@ -34,3 +38,8 @@ cudaError_t ft_select_rank(const FtCandDev* cand, const int32_t* cand_band, cons
 cudaError_t ft_count_to_key(const int32_t* c, float* k, int64_t n, cudaStream_t s);
 cudaError_t ft_select_tighten(FtSelectDev sel, uint32_t k, float rel_margin, cudaStream_t s);
 cudaError_t ft_fill_f32(float* p, int64_t n, float v, cudaStream_t s);
+// keys[r][c] = -inf where the template's number count is below the floor (rows mapped to points as in
+// ft_select_append_keys)
+cudaError_t ft_select_mask_keys(float* keys, int64_t n_rows, int64_t n_f0, uint64_t pt_begin, uint32_t R,
+                                uint32_t stride, uint64_t pt_end, const int32_t* veto_cnt, int32_t floor,
+                                cudaStream_t s);

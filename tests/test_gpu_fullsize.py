@@ -191,3 +191,45 @@ def test_selection_overflow_recovery_and_forced_tiling():
     c = ctx.counters()
     assert c["refine_fallbacks"] >= 1, c
     ctx.close()
+
+
+def test_config3_full_size_number_count_veto():
+    """Config 3 at full size with the paper's floor (three sigma above the Gaussian-noise mean count,
+    PAPER.md:502): every candidate re-evaluated by the oracle (count >= floor, power bit-identical,
+    ordered), and nothing louder with a passing count was missed (masked top-k of the full arrays)."""
+    import torch
+    from paper_2411_18370_b200 import binding as B
+    wl = _full(3)
+    g = wl.grid
+    o = fo.Oracle(wl)
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    p_hit = float(np.exp(-wl.rho_th))
+    floor = int(np.ceil(wl.n_sft * p_hit + 3.0 * np.sqrt(wl.n_sft * p_hit * (1 - p_hit))))
+    ctx = H.gpu_context(wl)
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    ctx.set_option(B.FT_OPT_COUNT_FLOOR, floor)
+    ctx.eval(g, "both", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    live = cands["idx"] != PAD
+    flat = cands[live]
+    cp, cc, _, _ = o.eval_list(flat["idx"])
+    assert np.array_equal(flat["power"], cp) and np.array_equal(flat["count"], cc) and np.all(cc >= floor)
+    full = torch.from_numpy(np.where(gc >= floor, gp, -np.inf).astype(np.float32)).cuda().view(-1, g.n_f0)
+    n_pass = 0
+    for b in range(n_bands):
+        c = cands[b][cands[b]["idx"] != PAD]
+        key = list(zip(-c["power"], c["idx"]))
+        assert key == sorted(key)
+        blk = full[:, b * bpb:(b + 1) * bpb].reshape(-1)
+        v, pos = torch.topk(blk, wl.k)
+        n_ok = int(torch.isfinite(v).sum())
+        assert len(c) == min(wl.k, int(torch.isfinite(blk).sum()))
+        n_pass += len(c)
+        if len(c):
+            kth = float(c["power"][-1])
+            w = bpb
+            tid = (pos // w) * g.n_f0 + b * bpb + (pos % w)
+            must = tid[:n_ok][v[:n_ok].double() > kth * (1 + 2e-5)].cpu().numpy().astype(np.uint64)
+            assert np.isin(must, c["idx"]).all(), f"band {b}: a louder passing template is missing"
+    assert n_pass > 0
+    ctx.close()

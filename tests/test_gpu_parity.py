@@ -122,3 +122,39 @@ def test_errors_and_edge_cases():
     op, oc, _, _ = fo.Oracle(wl1).eval_range()
     assert gc[0] == oc[0] and abs(gp[0] - op[0]) <= 1e-5 * op[0]
     ctx.close()
+
+
+@pytest.mark.parametrize("cfg,kernel,fused", [(3, 0, 1), (3, 0, 0), (1, 0, 1), (2, 1, 0), (4, 0, 1)])
+def test_number_count_veto(cfg, kernel, fused):
+    """per region, the loudest normalized power among templates scoring at least a
+    pre-established number count.  Oracle: mask the full arrays, then the plain per-band sort."""
+    from paper_2411_18370_b200 import binding as B
+    wl = H.apply_injections(_small(cfg))
+    o = fo.Oracle(wl)
+    op, oc, _, _ = o.eval_range()
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    p_hit = float(np.exp(-wl.rho_th))
+    floor = int(np.ceil(wl.n_sft * p_hit + 1.0 * np.sqrt(wl.n_sft * p_hit * (1 - p_hit))))   # mean + 1 sigma
+    masked = np.where(oc >= floor, op, -np.inf)
+    ref = fo.topk_per_band(masked, wl.grid.n_f0, bpb, wl.k)
+    ctx = H.gpu_context(wl, kernel=kernel, fused=fused)
+    ctx.set_option(B.FT_OPT_COUNT_FLOOR, floor)
+    ctx.eval(wl.grid, "both", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    vetoed_some = False
+    for b, (ridx, rval) in enumerate(ref):
+        keep = np.isfinite(rval)
+        ridx = ridx[keep]
+        vetoed_some |= len(ridx) < wl.k or bool((oc[b * bpb:(b + 1) * bpb] < floor).any())
+        got = cands[b]
+        assert np.array_equal(got["idx"][:len(ridx)], ridx), f"band {b}"
+        assert np.all(got["idx"][len(ridx):] == np.uint64(2 ** 64 - 1))
+        j = ridx.astype(np.int64)
+        assert np.array_equal(got["power"][:len(j)], op[j]) and np.array_equal(got["count"][:len(j)], oc[j])
+        assert np.all(got["count"][:len(j)] >= floor)
+    assert vetoed_some
+    # the floor only applies when both statistics are bound; power alone is unaffected
+    ctx.eval(wl.grid, "power", wl.rho_th)
+    plain = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    H.assert_topk_parity(wl, plain, op, op, oc, wl.k, bpb)
+    ctx.close()
