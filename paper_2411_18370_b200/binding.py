@@ -60,7 +60,10 @@ def load_library(path: str | None = None):
     """dlopen the in-tree shared library (fails loudly if it was not built)."""
     global _lib
     if _lib is None:
-        path = path or _build.SO
+        if path is None:
+            # in-tree library; compiled here with nvcc if it is missing or older than its sources
+            # (raises if that fails: there is no fallback path)
+            path = _build.build()
         if not os.path.exists(path):
             raise FileNotFoundError(f"{path} missing: run `python -m paper_2411_18370_b200.build`")
         lib = C.CDLL(path)
