@@ -23,15 +23,26 @@ def _stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale():
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-              [os.path.join(CSRC, s) for s in SOURCES] + ["-o", SO]
-        r = subprocess.run(cmd, capture_output=True, text=True)
-        if verbose or r.returncode != 0:
-            sys.stderr.write(r.stdout + r.stderr)
-        if r.returncode != 0:
-            raise RuntimeError("nvcc failed building libfasttracks_b200.so")
+    """Compile if missing or stale.  Safe under concurrent callers (one process per GPU): an exclusive
+    file lock serialises them and the library is written to a temporary name, then renamed."""
+    if not (force or _stale()):
+        return SO
+    import fcntl
+    with open(SO + ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if force or _stale():  # another process may have built it while we waited
+            nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+            tmp = f"{SO}.tmp.{os.getpid()}"
+            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+                  [os.path.join(CSRC, s) for s in SOURCES] + ["-o", tmp]
+            r = subprocess.run(cmd, capture_output=True, text=True)
+            if verbose or r.returncode != 0:
+                sys.stderr.write(r.stdout + r.stderr)
+            if r.returncode != 0:
+                if os.path.exists(tmp):
+                    os.remove(tmp)
+                raise RuntimeError("nvcc failed building libfasttracks_b200.so")
+            os.replace(tmp, SO)
     return SO
 
 
