@@ -233,3 +233,33 @@ def test_config3_full_size_number_count_veto():
             assert np.isin(must, c["idx"]).all(), f"band {b}: a louder passing template is missing"
     assert n_pass > 0
     ctx.close()
+
+
+def test_tight_orbit_limits_chunks_per_warp():
+    """a_p Omega = 3.6e-3 (10 lt-s at P_orb = 0.2 d): the shift drifts by a bin every ~270 f0, so the plan
+    must keep a warp's range short (32 J |D - 1| < 0.45) for the single-break model to hold; parity with
+    the oracle element by element, several breaks per tile."""
+    import math
+    T_sft, n_sft, n_f0, pad = 900.0, 61, 700, 700
+    df = 1.0 / T_sft
+    rng = np.random.Generator(np.random.PCG64(321))
+    t_mid = (np.arange(n_sft) * 7 + 0.5) * T_sft
+    vel = W.earth_velocity(t_mid, *W.DETECTORS["H1"])
+    n_bins = (n_f0 + 2 * pad + 3) // 4 * 4
+    P = (-np.log(1.0 - rng.random((n_sft, n_bins)))).astype(np.float32)
+    w = np.full(n_sft, 1.0 / n_sft, np.float32)
+    ra, dec = 2.0, -0.3
+    sky = np.array([[math.cos(dec) * math.cos(ra), math.cos(dec) * math.sin(ra), math.sin(dec)]])
+    g = W.Grid(f0_start=150.0, df0=df, n_f0=n_f0, sky=sky, a_p=np.array([5.0, 10.0]),
+               P_orb=np.array([0.2, 0.31]) * 86400.0, tasc_frac=np.array([0.0, 0.37, 0.8]))
+    wl = W.Workload("tight-orbit", 7, P, t_mid, vel, w, 150.0 - pad * df, df, g, "both", 1.6, 70 * df, 4, T_sft)
+    op, oc, _, otie = fo.Oracle(wl).eval_range()
+    ctx = H.gpu_context(wl, kernel=2)
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    desc = ctx.describe()
+    J = int(desc.split("J=")[1].split()[0])
+    assert J <= 3, desc
+    H.assert_full_parity(wl, gp, gc, op, oc, otie)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, 10)
+    H.assert_topk_parity(wl, cands, op, op, oc, wl.k, 70)
+    ctx.close()
