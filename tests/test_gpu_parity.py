@@ -158,3 +158,16 @@ def test_number_count_veto(cfg, kernel, fused):
     plain = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
     H.assert_topk_parity(wl, plain, op, op, oc, wl.k, bpb)
     ctx.close()
+
+
+@pytest.mark.parametrize("kernel,fused,k", [(0, 1, 300), (0, 0, 700), (1, 0, 1024)])
+def test_large_k(kernel, fused, k):
+    """k up to the documented limit (1024): trim / rank buffers hold k plus the fp32-margin ties."""
+    wl = _small(2)
+    op, oc, _, _ = fo.Oracle(wl).eval_range()
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    ctx = H.gpu_context(wl, kernel=kernel, fused=fused)
+    ctx.eval(wl.grid, "power", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, k, n_bands)
+    H.assert_topk_parity(wl, cands, op, op, oc, k, bpb)
+    ctx.close()
