@@ -57,3 +57,13 @@ def test_product_does_not_import_oracle():
                     s = line.strip()
                     if s.startswith(("import ", "from ", "#include")) or "CDLL" in s or "dlopen" in s:
                         assert "oracle" not in s, (f, s)
+
+
+def test_header_is_plain_c():
+    """The boundary is a C ABI: the header compiles as C99 with no C++ or torch types."""
+    import subprocess
+    hdr = os.path.join(ROOT, "include", "fasttracks_b200.h")
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-fsyntax-only", "-x", "c", hdr],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    assert "torch" not in open(hdr).read().lower().replace("pytorch allocates", "")
