@@ -263,3 +263,18 @@ def test_tight_orbit_limits_chunks_per_warp():
     cands = ctx.topk_per_band(wl.band_width, wl.k, 10)
     H.assert_topk_parity(wl, cands, op, op, oc, wl.k, 70)
     ctx.close()
+
+
+@pytest.mark.parametrize("n_sft,n_sky,band_hz", [(1, 2, 0.05), (3, 1, 0.3), (5, 3, 0.02)])
+def test_very_few_sfts(n_sft, n_sky, band_hz):
+    """Degenerate time axis: fewer SFTs than one ring stage (4 rows) or one 32-SFT block."""
+    wl = W.config2(n_sft=n_sft, n_sky=n_sky, band_hz=band_hz, band_width=0.01, k=2)
+    op, oc, _, otie = fo.Oracle(wl).eval_range()
+    ctx = H.gpu_context(wl, kernel=2)
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    H.assert_full_parity(wl, gp, gc, op, oc, otie)
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    ctx.eval(wl.grid, "power", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    H.assert_topk_parity(wl, cands, op, op, oc, wl.k, bpb)
+    ctx.close()
