@@ -475,7 +475,8 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
     const FtTilePlan& spl = (by_count && c->tile8_ok) ? c->plan8 : c->plan;  // the plan the statistic pass runs
     const uint64_t R = (uint64_t)spl.R;
     const uint64_t n_groups = (d.n_points + R - 1) / R;
-    uint64_t n_sg = ft_tile_sample_points(spl, d.n_points) / R;
+    // (a test override of the buffer capacity does not enlarge the sample: it is there to provoke overflow)
+    uint64_t n_sg = (ft_tile_sample_points(spl, d.n_points, (uint32_t)k, c->opt_cap > 0 ? 65536u : c->sel.cap) + R - 1) / R;
     n_sg = n_sg < 1 ? 1 : (n_sg > n_groups ? n_groups : n_sg);
     const uint64_t stride = n_groups / n_sg;
     const int64_t rows = (int64_t)(n_sg * R);

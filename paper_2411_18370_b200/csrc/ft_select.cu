@@ -50,23 +50,32 @@ __device__ __forceinline__ float apply_margin(float tau, float rel_margin) {
   return tau - rel_margin * fabsf(tau);
 }
 
-// k-th largest per band over a [n_rows][n_f0] key array -> thr[band] (with margin), one CTA per band.
+__device__ __forceinline__ void atomic_fmax(float* addr, float v) {
+  int* ai = reinterpret_cast<int*>(addr);
+  int old = *ai;
+  while (__int_as_float(old) < v) {
+    const int assumed = old;
+    old = atomicCAS(ai, assumed, __float_as_int(v));
+    if (old == assumed) break;
+  }
+}
+
+// k-th largest per band over a [n_rows][n_f0] key array -> thr[band] (with margin).  grid = (bands,
+// row slices): the k-th largest of a slice is a valid lower bound of the band's, so thr[band] is the
+// maximum over the slices (and over earlier calls: thresholds only ever tighten).
 __global__ void __launch_bounds__(SEL_THREADS)
 ft_band_threshold_kernel(const float* __restrict__ keys, int64_t n_rows, int64_t n_f0, int32_t bpb,
                          uint32_t k, float rel_margin, float* __restrict__ thr) {
   __shared__ uint32_t hist[256];
   __shared__ uint32_t bcast[2];
   const int b = blockIdx.x;
+  const int64_t r0 = n_rows * blockIdx.y / gridDim.y, r1 = n_rows * (blockIdx.y + 1) / gridDim.y;
   const int64_t c0 = (int64_t)b * bpb;
   const int64_t bw = min((int64_t)bpb, n_f0 - c0);
-  const int64_t n = n_rows * bw;
-  auto get = [&](int64_t e) { return keys[(e / bw) * n_f0 + c0 + (e % bw)]; };
+  const int64_t n = (r1 - r0) * bw;
+  auto get = [&](int64_t e) { return keys[(r0 + e / bw) * n_f0 + c0 + (e % bw)]; };
   const uint32_t kk = block_kth_largest(n, k, get, hist, bcast);
-  if (threadIdx.x == 0) {
-    const float prev = thr[b];
-    const float t = (n < (int64_t)k) ? -INFINITY : apply_margin(ft_unkey(kk), rel_margin);
-    thr[b] = fmaxf(prev, t);  // thresholds only ever tighten
-  }
+  if (threadIdx.x == 0 && n >= (int64_t)k) atomic_fmax(thr + b, apply_margin(ft_unkey(kk), rel_margin));
 }
 
 // Append every key >= thr[band] of a [n_rows][n_f0] key array (rows = points pt_begin + r).
@@ -218,7 +227,11 @@ cudaError_t ft_select_reset(FtSelectDev sel, uint32_t* final_n, uint32_t* overfl
 
 cudaError_t ft_select_threshold(const float* keys, int64_t n_rows, int64_t n_f0, int32_t bpb, uint32_t k,
                                 float rel_margin, FtSelectDev sel, cudaStream_t s) {
-  ft_band_threshold_kernel<<<sel.n_bands, SEL_THREADS, 0, s>>>(keys, n_rows, n_f0, bpb, k, rel_margin, sel.thr);
+  // slices of >= max(8 k, 32768) keys per band, at most 16 (more CTAs than bands on a 148-SM part)
+  const int64_t per_band = n_rows * std::min<int64_t>(bpb, n_f0);
+  const int64_t min_slice = std::max<int64_t>(8 * (int64_t)k, 32768);
+  const unsigned slices = (unsigned)std::max<int64_t>(1, std::min<int64_t>({(int64_t)16, per_band / min_slice, n_rows}));
+  ft_band_threshold_kernel<<<dim3((unsigned)sel.n_bands, slices), SEL_THREADS, 0, s>>>(keys, n_rows, n_f0, bpb, k, rel_margin, sel.thr);
   return cudaGetLastError();
 }
 

@@ -427,10 +427,14 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   return cudaSuccess;
 }
 
-uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points) {
-  uint64_t s = std::max<uint64_t>(n_points / 64, (uint64_t)plan.R * 296);
-  s = (s + plan.R - 1) / plan.R * plan.R;
-  return std::min(s, n_points);
+// Outer points of the threshold sample: one wave of CTA groups (148), more only when the bank is so large
+// that the fused pass would append more than cap / 8 entries per band (appended ~ k * groups / sample groups).
+uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points, uint32_t k, uint32_t cap) {
+  const uint64_t R = (uint64_t)plan.R;
+  const uint64_t n_groups = (n_points + R - 1) / R;
+  uint64_t n_sg = std::max<uint64_t>(148, (8ull * k * n_groups + cap - 1) / std::max<uint32_t>(cap, 1u));
+  n_sg = std::min(n_sg, n_groups);
+  return std::min(n_sg * R, n_points);
 }
 
 cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* A, double add_back, uint64_t pt_begin,

@@ -38,7 +38,7 @@ struct FtTileHostIn {
 };
 cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s, FtTilePlan* plan,
                          std::string* why, int* launches, int mode = 0);
-uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points);
+uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points, uint32_t k, uint32_t cap);
 // One pass of the gather-reduce over array A (folded w*P for the power statistic, the 0/1 hit map
 // for the number count); add_back is the constant the fold removed from A, summed over SFTs.
 // Writes out_f (fp32) and/or out_i (int32) indexed from out_base, and/or
