@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libfasttracks_b200.so")
-SOURCES = ["ft_api.cu", "ft_generic.cu", "ft_select.cu", "ft_tile.cu", "ft_tile8.cu"]
+SOURCES = ["ft_api.cu", "ft_generic.cu", "ft_select.cu", "ft_tile.cu", "ft_tile8.cu", "ft_tileb.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--extended-lambda", "-Xcompiler", "-fPIC", "-shared"]
 

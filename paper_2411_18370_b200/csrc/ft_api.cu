@@ -39,10 +39,14 @@ struct ft_ctx {
   FtTilePlan plan{};            // fp32 gather (power; number count when the packed kernel is not eligible)
   FtTilePlan plan8{};           // packed number-count kernel (ft_tile8.cu)
   bool tile8_ok = false;
+  FtTilePlan planb{};           // both statistics in one pass (ft_tileb.cu), narrow bands
+  bool tileb_ok = false;
+  float* QB_dev = nullptr;      // Q with the hit bit in the LSB
+  float QB_rho = 0.f; bool QB_valid = false;
   uint8_t* H8_dev = nullptr;    // four byte-shifted hit maps
   float H8_rho = 0.f; bool H8_valid = false;
   // options
-  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0, opt_cap = 0, opt_floor = 0;
+  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0, opt_cap = 0, opt_floor = 0, opt_onepass = 1;
   // selection buffers
   FtSelectDev sel{};
   uint64_t* final_idx = nullptr;
@@ -159,6 +163,14 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
     // one gather-reduce pass per statistic: power over Q, number count over the hit map
     const FtSelectDev* sel = filter ? &c->sel : nullptr;
     int launches = 0;
+    if (stat == FT_STAT_BOTH && c->tileb_ok && ((out_power && out_count) || filter)) {
+      // narrow bands: both statistics (and the count veto of the fused filter) from one gather
+      tick(c);
+      FT_CUDA(c, ft_launch_tile(c->d, c->planb, c->QB_dev, c->add_back, pt_begin, pt_end, out_power, out_count, out_base,
+                                sel, bpb, c->near_ties_dev, c->stream, &launches, stride, n_strided, complement));
+      tock(c, launches);
+      return FT_OK;
+    }
     if (stat != FT_STAT_HOUGH && (out_power || (filter && stat == FT_STAT_POWER))) {
       tick(c);
       FT_CUDA(c, ft_launch_tile(c->d, c->plan, c->d.Q, c->add_back, pt_begin, pt_end, out_power, nullptr, out_base,
@@ -183,7 +195,7 @@ int run_stat(ft_ctx* c, int stat, uint64_t pt_begin, uint64_t pt_end, float* out
 // The tile kernel raises plan.err if a track left its staged strip (a planning bug, never data):
 // surfaced at the next synchronising call instead of silently wrong sums.
 int check_tile_err(ft_ctx* c) {
-  for (const FtTilePlan* pl : {&c->plan, &c->plan8}) {
+  for (const FtTilePlan* pl : {&c->plan, &c->plan8, &c->planb}) {
     if (!pl->err) continue;
     int32_t e = 0;
     FT_CUDA(c, cudaMemcpy(&e, pl->err, sizeof e, cudaMemcpyDeviceToHost));
@@ -270,6 +282,7 @@ int ft_set_option(ft_ctx* c, int option, int64_t value) {
     case FT_OPT_PACKED_COUNT: c->opt_packed = value ? 1 : 0; break;
     case FT_OPT_SELECT_CAP: if (value < 0 || value > (1 << 20)) return fail(c, FT_ERR_ARG, "FT_OPT_SELECT_CAP: 0 .. 2^20"); c->opt_cap = value; break;
     case FT_OPT_COUNT_FLOOR: if (value < 0 || value > (1 << 24)) return fail(c, FT_ERR_ARG, "FT_OPT_COUNT_FLOOR: 0 .. 2^24"); c->opt_floor = value; break;
+    case FT_OPT_ONE_PASS_BOTH: c->opt_onepass = value ? 1 : 0; break;
     case FT_OPT_F0_TILES: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_F0_TILES >= 0"); c->opt_tiles = value; break;
     case FT_OPT_POINTS_PER_CTA: if (value < 0) return fail(c, FT_ERR_ARG, "FT_OPT_POINTS_PER_CTA >= 0"); c->opt_ppc = value; break;
     default: return fail(c, FT_ERR_ARG, "unknown option");
@@ -401,6 +414,24 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
     c->H_rho = d.rho; c->H_valid = true;
   }
   d.H = c->H_dev;
+  // both statistics bound on a narrow band: one-pass kernel on QB (Q with the hit bit in the LSB)
+  c->tileb_ok = false;
+  if (c->tile_ok && stat == FT_STAT_BOTH && c->opt_onepass) {
+    std::string whyb;
+    int launches = 0;
+    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc, (int)c->opt_tiles};
+    const cudaError_t e = ft_tile_plan(d, hin, c->stream, &c->planb, &whyb, &launches, 2);
+    c->counters.kernel_launches += launches;
+    if (e != cudaSuccess) return fail(c, FT_ERR_CUDA, std::string("ft_tile_plan (both): ") + cudaGetErrorString(e));
+    // only where the fp32 plan itself is narrow (J <= 16): wide bands run power on K2 and the count packed
+    c->tileb_ok = whyb.empty() && c->plan.J <= 16 && c->planb.n_tiles == c->plan.n_tiles;
+    if (c->tileb_ok && !(c->QB_valid && c->QB_rho == d.rho)) {
+      if (!c->QB_dev) FT_CUDA(c, cudaMalloc(&c->QB_dev, sizeof(float) * (size_t)d.n_sft * d.ld));
+      FT_CUDA(c, ft_launch_qb(d.Q, d.P, d.rho, c->QB_dev, d.n_sft * d.ld, c->stream));
+      c->counters.kernel_launches += 1;
+      c->QB_rho = d.rho; c->QB_valid = true;
+    }
+  }
   {
     char buf[320];
     if (c->tile_ok && c->opt_kernel != 1)
@@ -410,6 +441,11 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
     else
       std::snprintf(buf, sizeof buf, "K0 generic kernel (%s)", c->opt_kernel == 1 ? "forced" : c->why.c_str());
     c->desc = buf;
+    if (c->tileb_ok) {
+      std::snprintf(buf, sizeof buf, "; both statistics: one-pass tile kernel J=%d wpp=%d R=%d threads=%d",
+                    c->planb.J, c->planb.wpp, c->planb.R, (c->planb.R * c->planb.wpp + 1) * 32);
+      c->desc += buf;
+    }
     if (c->tile8_ok) {
       std::snprintf(buf, sizeof buf, "; number count: packed tile kernel J=%d wpp=%d R=%d n_tiles=%d tile_w=%d threads=%d pitch=%d copy=%d stages=%dx%d",
                     c->plan8.J, c->plan8.wpp, c->plan8.R, c->plan8.n_tiles, c->plan8.tile_w, (c->plan8.R * c->plan8.wpp + 1) * 32,
@@ -456,7 +492,10 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
   // every template below the floor.
   const int32_t floor = (c->stat == FT_STAT_BOTH) ? (int32_t)c->opt_floor : 0;
   c->sel.veto_cnt = nullptr; c->sel.veto_floor = 0;
-  if (floor > 0) {
+  // narrow bands with the one-pass kernel: the count is in registers when the filter runs, no bank-wide pass
+  const bool onepass_veto = floor > 0 && fused && c->tileb_ok;
+  if (onepass_veto) c->sel.veto_floor = floor;
+  if (floor > 0 && !onepass_veto) {
     const uint64_t n_templates = d.n_points * (uint64_t)d.n_f0;
     if (n_templates > ((uint64_t)1 << 34)) return fail(c, FT_ERR_ALLOC, "ft_topk_per_band: count floor needs 4 B per template (bank too large)");
     if (c->veto_cap < n_templates) {
@@ -472,7 +511,9 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
   if (fused) {
     // Phase A: per-band thresholds from a strided sample of point groups (every stride-th CTA group
     // of the bank, so the sample sees every region of parameter space), written out in full.
-    const FtTilePlan& spl = (by_count && c->tile8_ok) ? c->plan8 : c->plan;  // the plan the statistic pass runs
+    const FtTilePlan& spl = onepass_veto ? c->planb : ((by_count && c->tile8_ok) ? c->plan8 : c->plan);  // the plan the statistic pass runs
+    const int pass_stat = onepass_veto ? (int)FT_STAT_BOTH : sel_stat;
+    const bool want_i = by_count || onepass_veto, want_f = !by_count;
     const uint64_t R = (uint64_t)spl.R;
     const uint64_t n_groups = (d.n_points + R - 1) / R;
     // (a test override of the buffer capacity does not enlarge the sample: it is there to provoke overflow)
@@ -480,20 +521,23 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
     n_sg = n_sg < 1 ? 1 : (n_sg > n_groups ? n_groups : n_sg);
     const uint64_t stride = n_groups / n_sg;
     const int64_t rows = (int64_t)(n_sg * R);
-    rc = ensure_scratch(c, (size_t)rows * d.n_f0, by_count);
+    rc = ensure_scratch(c, (size_t)rows * d.n_f0, want_i);
     if (rc != FT_OK) return rc;
     // rows of a ragged last group are never written: make them lose every comparison
-    if (by_count) FT_CUDA(c, cudaMemsetAsync(c->scratch_i, 0x80, sizeof(int32_t) * (size_t)rows * d.n_f0, c->stream));
-    else { FT_CUDA(c, ft_fill_f32(c->scratch_f, rows * d.n_f0, -INFINITY, c->stream)); c->counters.kernel_launches += 1; }
+    if (want_i) FT_CUDA(c, cudaMemsetAsync(c->scratch_i, 0x80, sizeof(int32_t) * (size_t)rows * d.n_f0, c->stream));
+    if (want_f) { FT_CUDA(c, ft_fill_f32(c->scratch_f, rows * d.n_f0, -INFINITY, c->stream)); c->counters.kernel_launches += 1; }
     if (stride > 1)
-      rc = run_stat(c, sel_stat, 0, d.n_points, by_count ? nullptr : c->scratch_f, by_count ? c->scratch_i : nullptr,
+      rc = run_stat(c, pass_stat, 0, d.n_points, want_f ? c->scratch_f : nullptr, want_i ? c->scratch_i : nullptr,
                     0, false, (int32_t)bpb, (uint32_t)stride, n_sg);
     else
-      rc = run_stat(c, sel_stat, 0, std::min<uint64_t>(d.n_points, (uint64_t)rows), by_count ? nullptr : c->scratch_f,
-                    by_count ? c->scratch_i : nullptr, 0, false, (int32_t)bpb);
+      rc = run_stat(c, pass_stat, 0, std::min<uint64_t>(d.n_points, (uint64_t)rows), want_f ? c->scratch_f : nullptr,
+                    want_i ? c->scratch_i : nullptr, 0, false, (int32_t)bpb);
     if (rc != FT_OK) return rc;
     if (by_count) { FT_CUDA(c, ft_count_to_key(c->scratch_i, c->scratch_f, rows * d.n_f0, c->stream)); c->counters.kernel_launches += 1; }
-    if (floor > 0) {
+    if (onepass_veto) {
+      FT_CUDA(c, ft_select_mask_keys_local(c->scratch_f, c->scratch_i, rows * d.n_f0, floor, c->stream));
+      c->counters.kernel_launches += 1;
+    } else if (floor > 0) {
       FT_CUDA(c, ft_select_mask_keys(c->scratch_f, rows, d.n_f0, 0, (uint32_t)R, (uint32_t)stride, d.n_points, c->veto_cnt, floor, c->stream));
       c->counters.kernel_launches += 1;
     }
@@ -506,8 +550,8 @@ int ft_topk_per_band(ft_ctx* c, double band_width_hz, int32_t k, ft_cand* out_ho
       FT_CUDA(c, ft_select_append_keys(c->scratch_f, rows, d.n_f0, (int32_t)bpb, 0, c->sel, c->stream, (uint32_t)R,
                                        (uint32_t)stride, d.n_points));
       c->counters.kernel_launches += 1;
-      if (stride > 1) rc = run_stat(c, sel_stat, 0, d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb, (uint32_t)stride, n_sg, true);
-      else rc = run_stat(c, sel_stat, std::min<uint64_t>(d.n_points, (uint64_t)rows), d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb);
+      if (stride > 1) rc = run_stat(c, pass_stat, 0, d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb, (uint32_t)stride, n_sg, true);
+      else rc = run_stat(c, pass_stat, std::min<uint64_t>(d.n_points, (uint64_t)rows), d.n_points, nullptr, nullptr, 0, true, (int32_t)bpb);
       if (rc != FT_OK) return rc;
       FT_CUDA(c, cudaMemcpyAsync(cnt.data(), c->sel.cnt, sizeof(uint32_t) * n_bands, cudaMemcpyDeviceToHost, c->stream));
       FT_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -642,7 +686,8 @@ void ft_destroy(ft_ctx* c) {
   free_select(c);
   ft_tile_plan_free(&c->plan);
   ft_tile_plan_free(&c->plan8);
-  dfree(c->H8_dev);
+  ft_tile_plan_free(&c->planb);
+  dfree(c->H8_dev); dfree(c->QB_dev);
   dfree(c->t_mid_dev); dfree(c->vel_dev); dfree(c->w_dev); dfree(c->Q_dev); dfree(c->H_dev); dfree(c->ctab_dev); dfree(c->axes_dev);
   dfree(c->scratch_f); dfree(c->scratch_i); dfree(c->veto_cnt); dfree(c->near_ties_dev);
   for (cudaEvent_t e : c->evs) cudaEventDestroy(e);

@@ -91,7 +91,7 @@ __global__ void ft_append_from_keys_kernel(const float* __restrict__ keys, int64
     const float v = keys[e];
     const uint64_t r = (uint64_t)(e / n_f0);
     const uint64_t pt = pt_begin + (r / R) * (uint64_t)gstride * R + r % R;
-    if (pt < pt_end && v >= sel.thr[b]) ft_select_append(sel, b, v, pt * (uint64_t)n_f0 + (uint64_t)c);
+    if (pt < pt_end && v > -INFINITY && v >= sel.thr[b]) ft_select_append(sel, b, v, pt * (uint64_t)n_f0 + (uint64_t)c);
   }
 }
 
@@ -202,6 +202,13 @@ __global__ void ft_mask_keys_kernel(float* __restrict__ keys, int64_t n_rows, in
   }
 }
 
+// keys[e] = -inf where the element's own number count (same layout) is below the floor
+__global__ void ft_mask_keys_local_kernel(float* __restrict__ keys, const int32_t* __restrict__ counts, int64_t n, int32_t floor) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride)
+    if (counts[e] < floor) keys[e] = -INFINITY;
+}
+
 __global__ void ft_fill_f32_kernel(float* p, int64_t n, float v) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) p[i] = v;
@@ -281,5 +288,11 @@ cudaError_t ft_select_mask_keys(float* keys, int64_t n_rows, int64_t n_f0, uint6
   const int64_t n = n_rows * n_f0;
   const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
   ft_mask_keys_kernel<<<grid, 256, 0, s>>>(keys, n_rows, n_f0, pt_begin, R ? R : 1, stride ? stride : 1, pt_end, veto_cnt, floor);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_select_mask_keys_local(float* keys, const int32_t* counts, int64_t n, int32_t floor, cudaStream_t s) {
+  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  ft_mask_keys_local_kernel<<<grid, 256, 0, s>>>(keys, counts, n, floor);
   return cudaGetLastError();
 }

@@ -43,3 +43,4 @@ cudaError_t ft_fill_f32(float* p, int64_t n, float v, cudaStream_t s);
 cudaError_t ft_select_mask_keys(float* keys, int64_t n_rows, int64_t n_f0, uint64_t pt_begin, uint32_t R,
                                 uint32_t stride, uint64_t pt_end, const int32_t* veto_cnt, int32_t floor,
                                 cudaStream_t s);
+cudaError_t ft_select_mask_keys_local(float* keys, const int32_t* counts, int64_t n, int32_t floor, cudaStream_t s);

@@ -312,7 +312,7 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
     if (nt > 1 && in.force_tiles <= 0 && (chunks + nt - 2) / (nt - 1) == cpt) continue;  // same tile size as nt-1
     for (int wpp = 1; wpp <= 4; ++wpp) {
       const int64_t Jn = (cpt + wpp - 1) / wpp;
-      if (Jn > (mode == 1 ? 16 : 32)) continue;
+      if (Jn > (mode == 0 ? 32 : 16)) continue;
       int J = 0;
       for (int c : kJList) if (c >= Jn) { J = c; break; }
       if (J == 0 || J > maxJ_eps) continue;
@@ -328,8 +328,8 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   pl.n_tiles = (int32_t)((d.n_f0 + pl.tile_w - 1) / pl.tile_w);
   // default: 24-27 consumer warps per CTA (measured best on B200 at 72 registers: R = 12 at wpp = 2,
   // R = 6 at wpp = 4, R = 27 at wpp = 1); the packed kernel keeps 23 (80 registers)
-  int R = in.points_per_cta > 0 ? in.points_per_cta : (mode == 1 ? 23 : (pl.wpp == 1 ? 27 : 24 / pl.wpp));
-  const int max_threads = mode == 1 ? ft_tile8_max_threads(pl.J) : ft_tile_max_threads(pl.J);
+  int R = in.points_per_cta > 0 ? in.points_per_cta : (mode != 0 ? 23 / pl.wpp : (pl.wpp == 1 ? 27 : 24 / pl.wpp));
+  const int max_threads = mode == 1 ? ft_tile8_max_threads(pl.J) : (mode == 2 ? ft_tileb_max_threads(pl.J) : ft_tile_max_threads(pl.J));
   R = std::min<int>(R, (max_threads / 32 - 1) / pl.wpp);  // + 1 producer warp
   R = (int)std::min<uint64_t>((uint64_t)R, d.n_points);
   pl.R = std::max(R, 1);
@@ -388,7 +388,7 @@ cudaError_t ft_tile_plan(const FtDev& d, const FtTileHostIn& in, cudaStream_t s,
   if (pl.copy_floats > kMaxPitch + 1) { *why = "strip too wide for the packed track entry"; return cudaSuccess; }
   // --- shared-memory ring ---------------------------------------------------------------------------
   const int threads = (pl.R * pl.wpp + 1) * 32;
-  const int regs_est = 2 * pl.J + 30;
+  const int regs_est = (mode == 2 ? 3 : 2) * pl.J + 30;
   int ctas = std::min(4, std::min(2048 / threads, 65536 / (threads * regs_est)));
   ctas = std::max(ctas, 1);
   const size_t row_bytes = (size_t)pl.pitch * 4;
@@ -464,6 +464,7 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* 
     if (n_launch == 0) return cudaSuccess;
     a.pt_begin = pt_begin; a.pt_end = pt_end;
     const cudaError_t e = plan.mode == 1 ? ft_tile8_launch(plan.J, d, a, (unsigned)(n_launch * plan.n_tiles), block, plan.smem_bytes, s)
+                        : plan.mode == 2 ? ft_tileb_launch(plan.J, d, a, (unsigned)(n_launch * plan.n_tiles), block, plan.smem_bytes, s)
                                          : launch_any(plan.J, d, a, (unsigned)(n_launch * plan.n_tiles), block, plan.smem_bytes, s);
     if (e == cudaSuccess) *launches = 1;
     return e;
@@ -475,6 +476,7 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const float* 
     a.pt_begin = pt;
     a.pt_end = std::min<uint64_t>(pt_end, pt + groups * plan.R);
     const cudaError_t e = plan.mode == 1 ? ft_tile8_launch(plan.J, d, a, (unsigned)(groups * plan.n_tiles), block, plan.smem_bytes, s)
+                        : plan.mode == 2 ? ft_tileb_launch(plan.J, d, a, (unsigned)(groups * plan.n_tiles), block, plan.smem_bytes, s)
                                          : launch_any(plan.J, d, a, (unsigned)(groups * plan.n_tiles), block, plan.smem_bytes, s);
     if (e != cudaSuccess) return e;
     *launches += 1;

@@ -12,7 +12,8 @@ struct FtTilePlan {
   int32_t* err = nullptr;       // [1] set by the kernel if a track left its staged strip (plan bug)
   double* vr = nullptr;         // [n_sft][2] scratch of the sky-axis velocity range
   size_t vr_cap = 0;
-  int32_t mode = 0;             // 0: fp32 gather (ft_tile_kernel), 1: packed number count (ft_tile8_kernel)
+  int32_t mode = 0;             // 0: fp32 gather (ft_tile_kernel), 1: packed number count (ft_tile8_kernel),
+                                // 2: both statistics in one pass (ft_tileb_kernel, J <= 16)
   int32_t cw = 32;              // f0 per chunk (per warp load instruction): 32 or 128
   int32_t n_tiles = 0;          // f0 tiles
   int32_t tile_w = 0;           // f0 per tile (multiple of 32; the last tile may hold fewer)
@@ -56,4 +57,6 @@ cudaError_t ft_launch_hitmap8(const float* P, float rho, uint8_t* H8, int64_t n_
 // Q[a][k] = fl(fl(w P) - c_a) with c_a = fl(mean_k fl(w P)) per row; w_sft (per-SFT) or w_bin (per-bin).
 cudaError_t ft_launch_fold_centered(const float* P, const float* w_sft, const float* w_bin, float* Q, float* c_row,
                                     int64_t n_sft, int64_t n_bins, int64_t ld, cudaStream_t s);
+// QB = Q with the least significant bit replaced by the hit (P > rho): gather array of ft_tileb_kernel
+cudaError_t ft_launch_qb(const float* Q, const float* P, float rho, float* QB, int64_t n, cudaStream_t s);
 void ft_tile_plan_free(FtTilePlan* plan);

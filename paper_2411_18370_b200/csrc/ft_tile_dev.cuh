@@ -34,6 +34,12 @@ __host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 
 __host__ __device__ constexpr int ft_tile8_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tile8_max_threads(int J) { return J <= 8 ? 1024 : 768; }
 
+// both statistics in one pass (ft_tileb.cu): J accumulators + J counters + J loads in flight
+__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : 80; }
+__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : 768; }
+cudaError_t ft_tileb_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem,
+                            cudaStream_t s);
+
 // packed number-count kernels (ft_tile8.cu); A = the 4 byte-shifted hit maps d.H8
 cudaError_t ft_tile8_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem,
                             cudaStream_t s);
