@@ -174,13 +174,13 @@ typedef enum {
   FT_OPT_POINTS_PER_CTA = 2, /* 0 auto; else number of outer points a CTA shares one staged strip among */
   FT_OPT_PACKED_COUNT = 3,  /* 1 (default) number count on the packed byte hit map when n_sft <= 65535; 0 fp32 0/1 map */
   FT_OPT_F0_TILES = 4,      /* 0 auto; else split the f0 axis into exactly this many tiles (tuning / tests) */
+  FT_OPT_SELECT_CAP = 5,    /* 0 auto; else entries per band of the fused selection's append buffers (tests of the
+                               overflow recovery: a band that overflows tightens its threshold and the pass repeats) */
   FT_OPT_COUNT_FLOOR = 6,   /* 0 off (default); n > 0: with FT_STAT_BOTH bound, ft_topk_per_band keeps the loudest
                                normalized power among templates whose integer number count is >= n (the number-count
                                veto of :496-502; for uniform weights the paper's weighted-count floor times n_sft) */
-  FT_OPT_ONE_PASS_BOTH = 7, /* 1 (default): narrow bands compute both statistics in one gather (hit bit in the LSB of
+  FT_OPT_ONE_PASS_BOTH = 7  /* 1 (default): narrow bands compute both statistics in one gather (hit bit in the LSB of
                                the folded pixel); 0: one pass per statistic */
-  FT_OPT_SELECT_CAP = 5     /* 0 auto; else entries per band of the fused selection's append buffers (tests of the
-                               overflow recovery: a band that overflows tightens its threshold and the pass repeats) */
 } ft_option;
 int ft_set_option(ft_ctx* ctx, int option, int64_t value);
 
