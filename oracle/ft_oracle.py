@@ -44,7 +44,13 @@ class _Problem(C.Structure):
         ("n_porb", C.c_int64), ("P_orb", C.c_void_p),
         ("n_tasc", C.c_int64), ("tasc_frac", C.c_void_p),
         ("rho_th", C.c_double),
+        ("det_lat", C.c_void_p), ("det_gamma", C.c_void_p), ("lst", C.c_void_p),
     ]
+
+
+class _BankBox(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("f0_lo", "f0_hi", "f1_lo", "f1_hi", "ra_lo", "ra_hi", "sd_lo", "sd_hi",
+                                           "ap_lo", "ap_hi", "porb_lo", "porb_hi", "t_ref")]
 
 
 _lib = None
@@ -59,6 +65,13 @@ def _load():
         _lib.fto_eval_list.restype = C.c_int
         _lib.fto_eval_templates.restype = C.c_int
         _lib.fto_num_threads.restype = C.c_int
+        _lib.fto_eval_range_z.restype = C.c_int
+        _lib.fto_track_template.restype = C.c_int
+        _lib.fto_uniform.restype = C.c_double
+        _lib.fto_uniform.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32]
+        _lib.fto_antenna_ab.restype = None
+        _lib.fto_antenna_ab.argtypes = [C.c_double] * 5 + [C.POINTER(C.c_double)] * 2
+        _lib.fto_bank_draw.restype = None
     return _lib
 
 
@@ -69,7 +82,9 @@ def num_threads() -> int:
 class Oracle:
     """Binds one workload (spectrogram + tables + grid) and evaluates templates on the CPU."""
 
-    def __init__(self, wl, rho_th=None):
+    def __init__(self, wl, rho_th=None, antenna=None):
+        """antenna: None (weights used as given) or (lat[n_sft], gamma[n_sft], lst[n_sft]) in radians:
+        sky-dependent weights w_a(n) ∝ (a^2 + b^2) w_a normalised to sum 1 (Eq. 4-5)."""
         self.lib = _load()
         g = wl.grid
         self._keep = dict(
@@ -82,6 +97,10 @@ class Oracle:
             P_orb=np.ascontiguousarray(g.P_orb, dtype=np.float64),
             tasc=np.ascontiguousarray(g.tasc_frac, dtype=np.float64),
         )
+        if antenna is not None:
+            for name, arr in zip(("det_lat", "det_gamma", "lst"), antenna):
+                self._keep[name] = np.ascontiguousarray(arr, dtype=np.float64)
+                assert self._keep[name].shape == (len(self._keep["t_mid"]),)
         k = self._keep
         n_sft, n_bins = k["P"].shape
         assert k["t_mid"].shape == (n_sft,) and k["vel"].shape == (n_sft, 3)
@@ -95,7 +114,10 @@ class Oracle:
             float(g.f1_start), float(g.df1), int(g.n_f1), float(g.t_ref),
             len(k["sky"]), p(k["sky"]), len(k["a_p"]), p(k["a_p"]),
             len(k["P_orb"]), p(k["P_orb"]), len(k["tasc"]), p(k["tasc"]),
-            float(wl.rho_th if rho_th is None else rho_th))
+            float(wl.rho_th if rho_th is None else rho_th),
+            p(k["det_lat"]) if antenna is not None else None,
+            p(k["det_gamma"]) if antenna is not None else None,
+            p(k["lst"]) if antenna is not None else None)
         self.n_sft, self.n_bins = n_sft, n_bins
         self.dims = (len(k["sky"]), len(k["a_p"]), len(k["P_orb"]), len(k["tasc"]), int(g.n_f1),
                      int(g.n_f0))
@@ -122,6 +144,25 @@ class Oracle:
         if rc != 0:
             raise ValueError(f"oracle: a track left the spectrogram (rc={rc})")
         return o
+
+    def eval_range_z(self, begin: int = 0, end=None):
+        """(power, count, wcount, near_tie, z, sigma_G): eval_range plus the standardised statistic (Eq. 36)."""
+        end = self.n_templates if end is None else end
+        o = self._outs(end - begin) + (np.empty(end - begin, np.float64), np.empty(end - begin, np.float64))
+        rc = self.lib.fto_eval_range_z(C.byref(self.pb), C.c_uint64(begin), C.c_uint64(end),
+                                       *[a.ctypes.data_as(C.c_void_p) for a in o])
+        if rc != 0:
+            raise ValueError(f"oracle: a track left the spectrogram (rc={rc})")
+        return o
+
+    def track_template(self, template, t_ref: float):
+        """bins and positions of one explicit template (a TEMPLATE_DTYPE record)."""
+        tl = np.ascontiguousarray(np.atleast_1d(template), dtype=TEMPLATE_DTYPE)
+        k = np.empty(self.n_sft, dtype=np.int64)
+        x = np.empty(self.n_sft, dtype=np.float64)
+        rc = self.lib.fto_track_template(C.byref(self.pb), tl.ctypes.data_as(C.c_void_p), C.c_double(float(t_ref)),
+                                         k.ctypes.data_as(C.c_void_p), x.ctypes.data_as(C.c_void_p))
+        return k, x, rc
 
     def eval_list(self, idx):
         idx = np.ascontiguousarray(idx, dtype=np.uint64)
@@ -165,3 +206,57 @@ def topk_per_band(values, n_f0: int, bins_per_band: int, k: int, idx_begin: int 
         order = np.lexsort((idx[sel], -values[sel].astype(np.float64)))[:k]
         out.append((idx[sel][order], values[sel][order]))
     return out
+
+
+def topk_per_region(values, n_f0: int, bins_per_band: int, k: int, pbox=None, keep=None):
+    """Plain definition of the per-region top-k over a FULL array (disjoint regions, the
+    loudest candidates of each).  Region of canonical index idx = pbox[idx // n_f0] * n_bands +
+    (idx % n_f0) // bins_per_band (pbox None: one box of points, i.e. frequency sub-bands).  keep: boolean
+    mask of the templates that pass the number-count veto, None = all.  Returns a list
+    over regions of (idx[k'], value[k']) sorted by (value desc, idx asc)."""
+    values = np.asarray(values, dtype=np.float64)
+    idx = np.arange(values.size, dtype=np.uint64)
+    n_bands = (n_f0 + bins_per_band - 1) // bins_per_band
+    band = (idx % np.uint64(n_f0)).astype(np.int64) // bins_per_band
+    pt = (idx // np.uint64(n_f0)).astype(np.int64)
+    pb = np.zeros(values.size, dtype=np.int64) if pbox is None else np.asarray(pbox, dtype=np.int64)[pt]
+    region = pb * n_bands + band
+    n_regions = (1 if pbox is None else int(np.max(pbox)) + 1) * n_bands
+    ok = np.ones(values.size, dtype=bool) if keep is None else np.asarray(keep, dtype=bool)
+    out = []
+    for r in range(n_regions):
+        sel = np.flatnonzero((region == r) & ok)
+        order = np.lexsort((idx[sel], -values[sel]))[:k]
+        out.append((idx[sel][order], values[sel][order]))
+    return out
+
+
+def mismatch(s_signal, s_template, mu_G):
+    """Eq. (24) PAPER.md:190: m(lambda'; lambda) = (s(lambda) - s(lambda')) / (s(lambda) - mu_G)."""
+    return (np.asarray(s_signal, dtype=np.float64) - np.asarray(s_template, dtype=np.float64)) / \
+        (np.asarray(s_signal, dtype=np.float64) - mu_G)
+
+
+BANK_FIELDS = ("f0_lo", "f0_hi", "f1_lo", "f1_hi", "ra_lo", "ra_hi", "sd_lo", "sd_hi", "ap_lo", "ap_hi",
+               "porb_lo", "porb_hi", "t_ref")
+
+
+def bank_draw(box: dict, seed: int, first: int, n: int):
+    """n templates drawn uniformly in the xi coordinates of Eq. (A11) over the lambda-box `box` (keys BANK_FIELDS),
+    template i = first .. first + n - 1 of the counter-based stream `seed`."""
+    lib = _load()
+    bx = _BankBox(*[float(box[f]) for f in BANK_FIELDS])
+    out = np.zeros(n, dtype=TEMPLATE_DTYPE)
+    lib.fto_bank_draw(C.byref(bx), C.c_uint64(int(seed)), C.c_uint64(int(first)), C.c_int64(int(n)),
+                      out.ctypes.data_as(C.c_void_p))
+    return out
+
+
+def uniform(seed: int, i: int, d: int) -> float:
+    return float(_load().fto_uniform(int(seed), int(i), int(d)))
+
+
+def antenna_ab(lat, gamma, lst, ra, dec):
+    a, b = C.c_double(), C.c_double()
+    _load().fto_antenna_ab(float(lat), float(gamma), float(lst), float(ra), float(dec), C.byref(a), C.byref(b))
+    return a.value, b.value

@@ -166,6 +166,25 @@ class Workload:
         return self.grid.n_templates * self.n_sft
 
 
+# arm-bisector orientation gamma (deg, counter-clockwise from East) of the two LIGO sites, as tabulated with
+# the antenna-pattern formulas of the paper's ref. [20]
+DETECTOR_GAMMA = {"H1": 171.8, "L1": 243.0, "cfg1": 171.8}
+
+
+def antenna_geometry(wl: "Workload"):
+    """Per-SFT detector geometry for sky-dependent weights (Eq. 4): latitude, arm orientation gamma
+    and local sidereal angle at the SFT mid-time (the same rotation phase as earth_velocity), radians.  Rows are
+    detector-major (first half H1, second half L1) for the two-detector configs, config 1 is one detector.
+    Inputs only: no antenna function is evaluated here."""
+    n = wl.n_sft
+    names = ["cfg1"] * n if wl.config_id == 1 else ["H1"] * (n - n // 2) + ["L1"] * (n // 2)
+    lat = np.array([math.radians(DETECTORS[d][0]) for d in names])
+    gam = np.array([math.radians(DETECTOR_GAMMA[d]) for d in names])
+    lon = np.array([math.radians(DETECTORS[d][1]) for d in names])
+    lst = np.mod(2.0 * math.pi * np.asarray(wl.t_mid, dtype=np.float64) / 86164.0905 + lon, 2.0 * math.pi)
+    return lat, gam, lst
+
+
 def inject(P: np.ndarray, bins: np.ndarray, amplitude: float) -> None:
     """Add `amplitude` at P[alpha][bins[alpha]] for every row (in place).  The bins come from
     the caller (tests: the oracle's track); nothing of the track is computed here."""

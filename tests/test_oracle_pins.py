@@ -458,3 +458,209 @@ def test_template_list_straight_line_is_a_column_sum():
     for q, col in enumerate([12, 13, 40]):
         assert abs(pw[q] - colsum[:, col].sum()) <= 1e-12 * pw[q]
         assert ct[q] == int((wl.P[:, col] > np.float32(1.6)).sum())
+
+
+# ---------------------------------------------------------------- near-tie window WIDTH (north_star: 1e-9 bin)
+def test_near_tie_window_width():
+    """Catches: a window wider or narrower than 1e-9 bin (a 1e-4 window would silently exempt templates from
+    parity).  df = 1, f_min = 0, v = 0: x = f0 exactly, so x = k + 0.5 + delta is built by hand."""
+    n_sft, n_bins = 3, 256
+    P = np.ones((n_sft, n_bins), np.float32)
+    t_mid = np.arange(n_sft) + 0.5
+    for k in (2, 100, 201):
+        for delta, flagged in ((5e-10, 1), (-5e-10, 1), (9e-10, 1), (-9e-10, 1), (2e-9, 0), (-2e-9, 0),
+                               (1.1e-9, 0), (-1.1e-9, 0), (1e-4, 0), (-1e-4, 0), (0.25, 0)):
+            f0 = k + 0.5 + delta
+            wl = W.Workload("w", 99, P, t_mid, np.zeros((n_sft, 3)), np.ones(n_sft, np.float32), 0.0, 1.0,
+                            W.Grid(f0_start=f0, df0=1.0, n_f0=1), "both", 1.6, 1.0, 1, 1.0)
+            o = fo.Oracle(wl)
+            x = o.track(0)[1]
+            assert np.all(x == f0)
+            assert o.eval_range()[3][0] == flagged, (k, delta)
+
+
+# ---------------------------------------------------------------- Eq. (4)-(5): antenna-pattern weights
+def _detector_tensor_response(lat, gamma, lst, ra, dec):
+    """F+^2 + Fx^2 from the geometry alone: detector tensor d = (n1 n1 - n2 n2)/2 of two perpendicular arms at
+    gamma -+ 45 deg counter-clockwise from East at (lat, local sidereal angle lst), contracted with the
+    polarisation tensors of a wave from (ra, dec).  No formula shared with the oracle."""
+    e_east = np.array([-math.sin(lst), math.cos(lst), 0.0])
+    e_north = np.array([-math.sin(lat) * math.cos(lst), -math.sin(lat) * math.sin(lst), math.cos(lat)])
+    arms = [math.cos(gamma + s * math.pi / 4) * e_east + math.sin(gamma + s * math.pi / 4) * e_north for s in (-1, 1)]
+    d = 0.5 * (np.outer(arms[0], arms[0]) - np.outer(arms[1], arms[1]))
+    xi = np.array([math.sin(ra), -math.cos(ra), 0.0])
+    eta = np.array([-math.sin(dec) * math.cos(ra), -math.sin(dec) * math.sin(ra), math.cos(dec)])
+    fp = np.sum(d * (np.outer(xi, xi) - np.outer(eta, eta)))
+    fc = np.sum(d * (np.outer(xi, eta) + np.outer(eta, xi)))
+    return fp * fp + fc * fc
+
+
+def test_antenna_functions_against_detector_tensor_and_sky_average(golden):
+    """Catches: a wrong coefficient, sign or angle in a(t), b(t) (ref. [20] Eq. 12-13): a^2 + b^2 must equal
+    F+^2 + Fx^2 of the detector tensor for perpendicular arms, for any detector, time and source."""
+    rng = np.random.Generator(np.random.PCG64(42))
+    for _ in range(300):
+        lat, gamma, lst = rng.uniform(-1.5, 1.5), rng.uniform(0, 2 * math.pi), rng.uniform(0, 2 * math.pi)
+        ra, dec = rng.uniform(0, 2 * math.pi), math.asin(rng.uniform(-1, 1))
+        a, b = fo.antenna_ab(lat, gamma, lst, ra, dec)
+        assert abs((a * a + b * b) - _detector_tensor_response(lat, gamma, lst, ra, dec)) < 1e-12
+    # sky average 2/5 (Gauss-Legendre in sin(dec), uniform in ra: exact for the degree-4 polynomial integrand)
+    xs, ws = np.polynomial.legendre.leggauss(8)
+    ras = (np.arange(16) + 0.5) * 2 * math.pi / 16
+    for lat, gamma, lst in ((0.81, 2.99, 0.3), (0.53, 4.24, 5.0), (-0.2, 0.0, 1.0)):
+        tot = 0.0
+        for x, wq in zip(xs, ws):
+            for ra in ras:
+                a, b = fo.antenna_ab(lat, gamma, lst, ra, math.asin(x))
+                tot += wq * (a * a + b * b) / (2 * len(ras))
+        assert abs(tot - golden["antenna_sky_average_a2_plus_b2"]) < 1e-12
+    # a source on the rotation axis sees a time-independent a^2 + b^2
+    vals = [sum(v * v for v in fo.antenna_ab(0.7, 1.1, lst, 0.4, math.pi / 2)) for lst in np.linspace(0, 6, 13)]
+    assert np.ptp(vals) < 1e-13
+
+
+def _antenna_tables(wl):
+    """Per-SFT detector geometry of the synthetic two-detector network (inputs: workloads.antenna_geometry)."""
+    return W.antenna_geometry(wl)
+
+
+def test_sky_dependent_weights_sum_to_one_and_reduce_to_given_weights():
+    """Eq. (5): the weights of every sky point sum to 1, so on a constant spectrogram P = c the statistic is c
+    for every template; the weighted count of an all-hit spectrogram is 1; z is (s - 1)/sigma_G with
+    sigma_G^2 = sum w^2 recomputed here from the antenna functions.  Catches: missing normalisation, weights
+    taken at the wrong SFT / sky point, sigma_G from the wrong weights."""
+    wl = W.config2(n_sft=96, n_sky=6, band_hz=0.05)
+    wl.P[:] = np.float32(3.0)
+    ant = _antenna_tables(wl)
+    o = fo.Oracle(wl, antenna=ant)
+    power, count, wcount, _, z, sigma = o.eval_range_z()
+    assert np.allclose(power, 3.0, rtol=1e-12) and np.all(count == wl.n_sft) and np.allclose(wcount, 1.0, rtol=1e-12)
+    g = wl.grid
+    for i_sky in range(len(g.sky)):
+        n = g.sky[i_sky]
+        ra, dec = math.atan2(n[1], n[0]), math.asin(n[2])
+        u = np.array([sum(v * v for v in fo.antenna_ab(ant[0][a], ant[1][a], ant[2][a], ra, dec)) for a in range(wl.n_sft)])
+        w = u * wl.w.astype(np.float64)
+        w /= w.sum()
+        j = int(g.ravel(i_sky, 0, 0, 0, 0, 0))
+        assert abs(sigma[j] - math.sqrt((w ** 2).sum())) < 1e-12 * sigma[j]
+        assert abs(z[j] - (3.0 - 1.0) / sigma[j]) < 1e-8
+    # weights vary across the sky (otherwise the feature is vacuous)
+    assert np.ptp(sigma) > 1e-3 * sigma.mean()
+    # an isotropic antenna factor (u = const) must give back the weights as given: emulate with P = hits only at one SFT
+    wl2 = W.config2(n_sft=96, n_sky=6, band_hz=0.05)
+    wl2.P[:] = 0.0
+    wl2.P[17, :] = 1.0
+    p2 = fo.Oracle(wl2, antenna=ant).eval_range()[0]
+    n = g.sky[2]
+    ra, dec = math.atan2(n[1], n[0]), math.asin(n[2])
+    u = np.array([sum(v * v for v in fo.antenna_ab(ant[0][a], ant[1][a], ant[2][a], ra, dec)) for a in range(wl.n_sft)])
+    w = u * wl2.w.astype(np.float64)
+    assert abs(p2[int(g.ravel(2, 0, 0, 0, 0, 5))] - w[17] / w.sum()) < 1e-15
+
+
+def test_standardised_statistic_is_zero_mean_unit_variance_in_noise(golden):
+    """Eq. (36) with Eq. (13)-(14): z ~ N(0, 1) on an Exponential(1) spectrogram.  Catches: sigma_G from sum w
+    instead of sum w^2, mu_G off by the chi^2 factor 2, z not using the template's own weights."""
+    wl = W.config2(n_sft=400, n_sky=3)
+    for ant in (None, _antenna_tables(wl)):
+        o = fo.Oracle(wl, antenna=ant)
+        n_f0 = wl.grid.n_f0
+        power, _, _, _, z, sigma = o.eval_range_z(0, n_f0)
+        assert abs(z.mean() - golden["z_noise_mean"]) < 4 / math.sqrt(n_f0)
+        assert abs(z.var() - golden["z_noise_var"]) < 4 * math.sqrt(2.0 / n_f0) + 0.05
+        if ant is None:   # fixed weights: mu_G = sum w, sigma_G = sqrt(sum w^2), recomputed here
+            w = wl.w.astype(np.float64)
+            assert np.allclose(z, (power - w.sum()) / math.sqrt((w ** 2).sum()), rtol=0, atol=1e-9)
+            assert np.allclose(sigma, math.sqrt((w ** 2).sum()), rtol=1e-12)
+
+
+# ---------------------------------------------------------------- boxes (PAPER.md:338-342) and the veto (:496-502)
+def test_topk_per_region_against_python_sorted():
+    """Catches: wrong region index, veto applied after instead of before the selection, tie order."""
+    rng = np.random.Generator(np.random.PCG64(3))
+    n_pt, n_f0, bpb, k = 12, 10, 4, 3
+    vals = rng.integers(0, 6, n_pt * n_f0).astype(np.float64)      # many exact ties
+    pbox = np.array([0, 0, 1, 1, 1, 2, 2, 0, 3, 3, 3, 3])
+    keep = rng.random(n_pt * n_f0) < 0.7
+    got = fo.topk_per_region(vals, n_f0, bpb, k, pbox=pbox, keep=keep)
+    n_bands = 3
+    assert len(got) == 4 * n_bands
+    for r, (gi, gv) in enumerate(got):
+        pb, band = divmod(r, n_bands)
+        members = [(-(vals[i]), i) for i in range(vals.size)
+                   if pbox[i // n_f0] == pb and (i % n_f0) // bpb == band and keep[i]]
+        ref = sorted(members)[:k]
+        assert [int(i) for i in gi] == [i for _, i in ref]
+        assert list(gv) == [-v for v, _ in ref]
+    # one box of points and no veto = the per-band top-k
+    a = fo.topk_per_region(vals, n_f0, bpb, k)
+    b = fo.topk_per_band(vals, n_f0, bpb, k)
+    assert all(np.array_equal(x[0], y[0]) for x, y in zip(a, b))
+
+
+def test_mismatch_definition_eq24():
+    """Eq. (24): m = 0 at the matched template, m = 1 for a template that recovers only the noise mean."""
+    assert fo.mismatch(3.0, 3.0, 1.0) == 0.0 and fo.mismatch(3.0, 1.0, 1.0) == 1.0
+    assert abs(fo.mismatch(3.0, 2.5, 1.0) - 0.25) < 1e-15
+
+
+# ---------------------------------------------------------------- Eq. (A11): xi-uniform random banks
+BOX = dict(f0_lo=100.0, f0_hi=200.0, f1_lo=-1e-9, f1_hi=0.0, ra_lo=0.0, ra_hi=2 * math.pi, sd_lo=-1.0, sd_hi=1.0,
+           ap_lo=1.0, ap_hi=10.0, porb_lo=10 * 86400.0, porb_hi=60 * 86400.0, t_ref=1000.0)
+
+
+def test_counter_generator_is_uniform_and_order_independent():
+    """Catches: correlated coordinates, a stream that depends on the batch boundaries."""
+    a = fo.bank_draw(BOX, 5, 0, 1000)
+    b = np.concatenate([fo.bank_draw(BOX, 5, 0, 300), fo.bank_draw(BOX, 5, 300, 700)])
+    assert a.tobytes() == b.tobytes()
+    u = np.array([[fo.uniform(9, i, d) for d in range(7)] for i in range(20000)])
+    assert np.all((u > 0) & (u < 1))
+    assert np.all(np.abs(u.mean(axis=0) - 0.5) < 4 / math.sqrt(12 * 20000))
+    assert np.all(np.abs(u.var(axis=0) - 1 / 12) < 0.003)
+    assert np.all(np.abs(np.corrcoef(u.T) - np.eye(7)) < 0.04)
+    assert np.all(np.abs(np.corrcoef(u[:-1, 0], u[1:, 0])[0, 1]) < 0.04)
+
+
+def test_xi_bank_marginal_densities_follow_eq_a9(golden):
+    """The marginals of a xi-uniform bank follow rho ∝ f0^5 a_p^2 Omega^3 (Eq. A9), uniform in (alpha, sin delta,
+    phi_b).  The expected bin counts come from numerical quadrature of the density, not from the inverse map.
+    Catches: a wrong exponent, Omega drawn as P_orb, phi_b not spanning one orbit, non-unit sky vectors."""
+    n = 200000
+    tl = fo.bank_draw(BOX, 11, 0, n)
+
+    def check(x, lo, hi, p):
+        edges = np.linspace(lo, hi, 9)
+        got = np.histogram(x, edges)[0]
+        grid = np.linspace(lo, hi, 8001)
+        dens = grid ** p
+        cum = np.concatenate([[0.0], np.cumsum(0.5 * (dens[1:] + dens[:-1]) * np.diff(grid))])
+        exp = n * np.diff(np.interp(edges, grid, cum)) / cum[-1]
+        assert np.all(np.abs(got - exp) < 5 * np.sqrt(exp) + 1), (p, got, exp)
+
+    check(tl["f0"], BOX["f0_lo"], BOX["f0_hi"], golden["xi_exponent_f0"])
+    check(tl["a_p"], BOX["ap_lo"], BOX["ap_hi"], golden["xi_exponent_ap"])
+    Om = 2 * math.pi / tl["P_orb"]
+    check(Om, 2 * math.pi / BOX["porb_hi"], 2 * math.pi / BOX["porb_lo"], golden["xi_exponent_omega"])
+    check(np.mod(np.arctan2(tl["ny"], tl["nx"]), 2 * math.pi), 0.0, 2 * math.pi, 0)
+    check(tl["nz"], -1.0, 1.0, 0)
+    phi_b = (tl["t_asc"] - BOX["t_ref"]) * Om
+    check(phi_b, 0.0, 2 * math.pi, 0)
+    check(tl["f1"], BOX["f1_lo"], BOX["f1_hi"], 0)
+    assert np.allclose(tl["nx"] ** 2 + tl["ny"] ** 2 + tl["nz"] ** 2, 1.0, atol=1e-14)
+    # isolated bank: a_p = 0 exactly
+    iso = dict(BOX, ap_lo=0.0, ap_hi=0.0)
+    assert np.all(fo.bank_draw(iso, 11, 0, 100)["a_p"] == 0.0)
+
+
+def test_xi_round_trip():
+    """lambda -> xi (Eq. A11) -> lambda: the drawn template, pushed forward through xi = lambda^(p+1)/(p+1), lands
+    at xi_min + u (xi_max - xi_min) with the generator's own u.  Catches: a wrong inverse map."""
+    tl = fo.bank_draw(BOX, 3, 40, 50)
+    for j, t in enumerate(tl):
+        i = 40 + j
+        for val, lo, hi, p1, d in ((t["f0"], BOX["f0_lo"], BOX["f0_hi"], 6, 0), (t["a_p"], BOX["ap_lo"], BOX["ap_hi"], 3, 3),
+                                   (2 * math.pi / t["P_orb"], 2 * math.pi / BOX["porb_hi"], 2 * math.pi / BOX["porb_lo"], 4, 4)):
+            xi, xl, xh = val ** p1 / p1, lo ** p1 / p1, hi ** p1 / p1
+            assert abs((xi - xl) / (xh - xl) - fo.uniform(3, i, d)) < 1e-12
