@@ -10,7 +10,13 @@
  *   spectrogram      s[t;f] = 4 |x~|^2 / (T_SFT S_n)                                    Eq. (6)  :88
  *   number count     nc = 1 if s > 3.2 else 0; weighted count "akin to Eq. (3)"         Eq. (7)  :95-97
  *   batching         vmap s : {lambda_i} -> {s(lambda_i)}                                Sec. III :213
- *   post-processing  loudest candidate per parameter-space region                        Sec. IV.B :330-351
+ *   post-processing  loudest candidate per parameter-space region (hyperboxes)           Sec. IV.B :330-351
+ *   standardisation  z(lambda; b) = (s(lambda) - mu_G(b)) / sigma_G(b)                    Eq. (36) :346
+ *   noise moments    mu_G = 2 sum w, sigma_G^2 = 4 sum w^2 (chi^2_2 scale)                Eq. (13)-(14) :130-132
+ *   number-count veto  loudest power subject to a minimal weighted number count           Sec. VI.B :496-502
+ *   random banks     templates drawn uniformly in xi = (f0^6/6, alpha, sin delta, a_p^3/3, Omega^4/4, phi_b)
+ *                                                                                        :312-316, Eq. (A11) :602-614
+ *   mismatch         m = (s(lambda) - s(lambda')) / (s(lambda) - mu_G)                    Eq. (24) :190
  * Extensions fixed by BASELINE.json north_star: spindown f1 with reference time t_ref, SFT
  * mid-times, regions = frequency sub-bands, loudest -> top-k.  DESIGN.md lists every reading.
  *
@@ -53,7 +59,8 @@ typedef enum {
   FT_ERR_UNSUPPORTED = -7  /* option combination the selected kernel cannot run */
 } ft_status;
 
-typedef enum { FT_STAT_POWER = 0, FT_STAT_HOUGH = 1, FT_STAT_BOTH = 2 } ft_stat;
+/* FT_STAT_WHOUGH: the weighted number count sum_a w_a [P > rho_th] (:97) as the statistic (fp32 array, ranking). */
+typedef enum { FT_STAT_POWER = 0, FT_STAT_HOUGH = 1, FT_STAT_BOTH = 2, FT_STAT_WHOUGH = 3 } ft_stat;
 typedef enum { FT_W_PER_SFT = 1, FT_W_PER_SFT_BIN = 2 } ft_wkind;
 
 /*
@@ -97,7 +104,8 @@ typedef struct {
  * (vmap s, :213).
  *   stat        ft_stat.  rho_th: number-count threshold on the scale of P (1.6 <-> the paper's
  *               3.2, Eq. 7), compared in fp32 with strict '>'.
- *   out_power_dev [device] fp32 [n_templates] or NULL: Eq. (3) for every canonical index.
+ *   out_power_dev [device] fp32 [n_templates] or NULL: Eq. (3) for every canonical index (FT_STAT_WHOUGH: the
+ *               weighted number count sum_a w_a [P > rho_th] instead).
  *   out_count_dev [device] int32 [n_templates] or NULL: Eq. (7) summed along the track (integer).
  *   Both NULL: bind the grid only (for ft_topk_per_band); no statistic kernel is launched.
  * Validation before any launch: finite arguments, positive sizes, and a conservative bound on
@@ -137,6 +145,49 @@ int ft_topk_per_band(ft_ctx* ctx, double band_width_hz, int32_t k, ft_cand* out_
                      int32_t* n_bands_out);
 
 /*
+ * One candidate of ft_topk_per_box: ft_cand plus the standardised statistic of Eq. (36).
+ * z = (power - mu_G) / sigma_G with the noise moments of the template's own weights on the scale of P
+ * (Eq. 13-14 / footnote 2: mu_G = sum_a w_a, sigma_G^2 = sum_a w_a^2; per-bin weights: the row means of w,
+ * DESIGN.md reading R21; sky-dependent weights: those of the template's sky point, mu_G = 1).
+ */
+typedef struct {
+  double power, wcount;
+  uint64_t idx;
+  int32_t count;
+  int32_t box;     /* region: pbox[point] * n_bands + i_f0 / bins_per_band */
+  double z, sigma; /* Eq. (36); sigma_G */
+} ft_cand_box;
+
+/*
+ * ft_topk_per_box — the paper's post-processing (:338-347): the parameter space is divided into disjoint
+ * regions and the k loudest templates of every region are kept (the paper keeps k = 1, :476).  A region is
+ * (box of outer points) x (frequency sub-band):
+ *     region = pbox[point] * n_bands + i_f0 / round(band_width_hz/df0),   point = canonical idx / n_f0,
+ * i.e. any partition of the outer axes (sky, a_p, P_orb, t_asc, f1 -- regular hyperboxes in the xi coordinates
+ * are blocks of those axes) times the sub-bands of ft_topk_per_band.
+ *   pbox_host   [host] int32 [n_points], values in [0, n_pbox), or NULL (one box: regions = sub-bands).
+ *   rank_by_z   0: rank inside a region by the bound statistic (as ft_topk_per_band);
+ *               1: rank by z (Eq. 36) -- with sky-dependent weights (ft_set_antenna) sigma_G differs between
+ *               the sky points of a box, so the order differs from the order by power.  Needs FT_STAT_POWER/BOTH.
+ *   out_host    [host] ft_cand_box [n_regions][k], padded with idx = UINT64_MAX.
+ *   n_regions_out [host] receives n_pbox * n_bands.
+ * Errors as ft_topk_per_band; FT_ERR_ARG for a pbox value out of range.  Synchronises the stream.
+ */
+int ft_topk_per_box(ft_ctx* ctx, const int32_t* pbox_host, int32_t n_pbox, double band_width_hz, int32_t k,
+                    int rank_by_z, ft_cand_box* out_host, int32_t* n_regions_out);
+
+/*
+ * ft_set_antenna — sky-dependent weights (Eq. 4-5, :67-84): w_a(n) = u_a(n) w_a / sum_b u_b(n) w_b with
+ * u_a(n) = a^2(t_a; n) + b^2(t_a; n), a and b the amplitude-modulation functions of the paper's ref. [20]
+ * (Jaranowski, Krolak & Schutz 1998, Eq. 12-13) for perpendicular arms, and w_a the per-SFT weights given to
+ * ft_create (∝ 1/S_a).  Per SFT (host arrays [n_sft], radians, copied): detector latitude, orientation
+ * gamma of the arm bisector counter-clockwise from East, local sidereal angle at the SFT mid-time.
+ * All three NULL: back to the weights as given.  Needs FT_W_PER_SFT weights (else FT_ERR_UNSUPPORTED) and a
+ * grid the tile kernel accepts (checked at ft_eval).  Unbinds the grid.
+ */
+int ft_set_antenna(ft_ctx* ctx, const double* det_lat_host, const double* det_gamma_host, const double* lst_host);
+
+/*
  * ft_eval_list — canonical fp64 evaluation of an explicit list of templates of the bound grid
  * (the refinement step of the selection, exposed for spot checks of full-size runs).
  *   idx_host [host] uint64 [n]; out_host [host] ft_cand [n] (band = -1).  Synchronises.
@@ -167,6 +218,41 @@ typedef struct {
 int ft_eval_templates(ft_ctx* ctx, const ft_template* templates_dev, int64_t n, double t_ref, int stat,
                       double rho_th, float* out_power_dev, int32_t* out_count_dev);
 
+/*
+ * ft_bank_draw — a random template bank drawn uniformly in the xi coordinates of Eq. (A11) (:602-614) over a
+ * box of the physical parameters ("draw n templates uniformly in xi, map them to lambda", :312-316, :627):
+ *   f0 ~ f0^5, (alpha, sin delta) uniform, a_p ~ a_p^2, Omega = 2 pi / P_orb ~ Omega^3, phi_b = Omega (t_asc - t_ref)
+ *   uniform in [0, 2 pi); f1 uniform (reading R22).  ap_hi == 0 draws an isolated bank (a_p = 0).
+ * Template i of stream `seed` is a pure function of (seed, i): u(seed, i, d) = splitmix64 finaliser of
+ * seed + 0x9E3779B97F4A7C15 (8 i + d + 1), top 53 bits; so banks can be drawn in batches of any size.
+ *   out_dev [device] ft_template [n]: templates first .. first + n - 1.  Asynchronous on the handle's stream.
+ */
+typedef struct {
+  double f0_lo, f0_hi, f1_lo, f1_hi, ra_lo, ra_hi, sd_lo, sd_hi, ap_lo, ap_hi, porb_lo, porb_hi, t_ref;
+} ft_bank_box;
+int ft_bank_draw(ft_ctx* ctx, const ft_bank_box* box, uint64_t seed, uint64_t first, int64_t n, ft_template* out_dev);
+
+/*
+ * ft_eval_bank — draw (ft_bank_draw) AND evaluate templates first .. first + n - 1 of a xi-uniform bank in one
+ * call (the paper's benchmark counts "generating random templates, computing the frequency indices,
+ * gathering, reducing", :228): the templates are generated in registers and never stored.  Returns the
+ * loudest template of the batch under (statistic desc, index asc) -- the per-box loudest of :476 -- re-evaluated
+ * in fp64, and optionally every statistic.
+ *   stat: FT_STAT_POWER or FT_STAT_HOUGH (ranking value).  out_power_dev / out_count_dev as ft_eval_templates, or NULL.
+ *   best_host [host] ft_cand (idx = position in the stream; band = -1) and best_template_host [host] ft_template, or NULL.
+ * Synchronises the stream.
+ */
+int ft_eval_bank(ft_ctx* ctx, const ft_bank_box* box, uint64_t seed, uint64_t first, int64_t n, int stat,
+                 double rho_th, float* out_power_dev, int32_t* out_count_dev, ft_cand* best_host,
+                 ft_template* best_template_host);
+
+/*
+ * ft_track — the track of ONE explicit template: bin k_a (Eq. 2 rounded to the bin grid, :248) for every SFT.
+ *   template_host [host]; k_out_host [host] int64 [n_sft].  For building injections (a "data stream containing a
+ *   CW signal", :322) without leaving the library.  Synchronises.  FT_ERR_TRACK_RANGE if a bin is outside.
+ */
+int ft_track(ft_ctx* ctx, const ft_template* template_host, double t_ref, int64_t* k_out_host);
+
 /* Options (ft_set_option): */
 typedef enum {
   FT_OPT_KERNEL = 0,        /* 0 auto (default), 1 force generic kernel, 2 force tile kernel (FT_ERR_UNSUPPORTED if ineligible) */
@@ -179,10 +265,16 @@ typedef enum {
   FT_OPT_COUNT_FLOOR = 6,   /* 0 off (default); n > 0: with FT_STAT_BOTH bound, ft_topk_per_band keeps the loudest
                                normalized power among templates whose integer number count is >= n (the number-count
                                veto of :496-502; for uniform weights the paper's weighted-count floor times n_sft) */
-  FT_OPT_ONE_PASS_BOTH = 7  /* 1 (default): narrow bands compute both statistics in one gather (hit bit in the LSB of
+  FT_OPT_ONE_PASS_BOTH = 7, /* 1 (default): narrow bands compute both statistics in one gather (hit bit in the LSB of
                                the folded pixel); 0: one pass per statistic */
+  FT_OPT_WCOUNT_FLOOR = 8   /* ft_set_option_f64: 0 off (default); x > 0: with FT_STAT_BOTH bound, the selection keeps the
+                               loudest normalized power among templates whose WEIGHTED number count sum_a w_a [P > rho_th]
+                               is >= x -- the veto as the paper states it (:496-502; "three standard deviations above
+                               the average number count in Gaussian noise": x = p sum w + 3 sqrt(p (1 - p) sum w^2),
+                               p = exp(-rho_th)).  Costs one weighted-count pass over the bank. */
 } ft_option;
 int ft_set_option(ft_ctx* ctx, int option, int64_t value);
+int ft_set_option_f64(ft_ctx* ctx, int option, double value);
 
 typedef struct {
   uint64_t near_ties;        /* canonical track evaluations that fell within 1e-9 bin of a rounding tie, since ft_create */
@@ -194,6 +286,29 @@ typedef struct {
   double last_kernel_ms;     /* summed device time of those launches (CUDA events on the handle's stream) */
 } ft_counters;
 int ft_get_counters(ft_ctx* ctx, ft_counters* out);
+
+/*
+ * ft_measure_peaks — micro-benchmarks of the units that bound the kernels of this library, on the handle's
+ * device and stream (the roofline denominators MEASURED_PEAKS.json does not hold):
+ *   smem_gbs       shared-memory read bandwidth, conflict-free LDS.32 from every SM (the bound of the tile kernel)
+ *   fp64_gflops    DFMA throughput x 2 (the bound of the per-evaluation track arithmetic, kernel K1)
+ *   fp64_cvt_gops  F2I.F64 + I2F.F64 pairs per second (conversions share the fp64 pipe at a lower rate)
+ *   l2_gbs         read bandwidth of a 32 MiB buffer resident in L2
+ *   sm_clock_mhz   SM clock during the shared-memory run (cycles counted on the device / event time)
+ * Synchronises the stream.
+ */
+typedef struct { double smem_gbs, fp64_gflops, fp64_cvt_gops, l2_gbs, sm_clock_mhz; } ft_peaks;
+int ft_measure_peaks(ft_ctx* ctx, ft_peaks* out);
+
+/*
+ * ft_selftest — device-side checks of arithmetic identities the kernels rely on; *n_fail_out receives the
+ * number of failures among n random cases of stream `seed`.
+ *   which = 0: the unstructured-bank kernel divides v.n by c with a reciprocal multiply and one fused
+ *              correction; every quotient must equal the IEEE division __ddiv_rn(dot, c) bit for bit (up to the sign of a zero)
+ *              (dot drawn over the range of |v.n| <= 5e4 m/s, every binade from 2^-300 to 2^300, exact multiples of c, +-0).
+ *   which = 1: the integer-arithmetic fp32 -> fp64 conversion of K1 equals (double)x for every finite input.
+ */
+int ft_selftest(ft_ctx* ctx, int which, int64_t n, uint64_t seed, uint64_t* n_fail_out);
 
 const char* ft_last_error(const ft_ctx* ctx); /* never NULL; valid until the next call on ctx */
 /* Which kernel the bound grid runs and its launch geometry (diagnostics; never NULL; valid until the next ft_eval). */

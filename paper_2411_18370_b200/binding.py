@@ -10,11 +10,12 @@ import numpy as np
 
 from . import build as _build
 
-FT_STAT = {"power": 0, "hough": 1, "both": 2}
+FT_STAT = {"power": 0, "hough": 1, "both": 2, "whough": 3}
 FT_OPT_KERNEL, FT_OPT_FUSED_TOPK, FT_OPT_POINTS_PER_CTA, FT_OPT_PACKED_COUNT, FT_OPT_F0_TILES = 0, 1, 2, 3, 4
-FT_OPT_SELECT_CAP, FT_OPT_COUNT_FLOOR, FT_OPT_ONE_PASS_BOTH = 5, 6, 7
-SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_eval_list", "ft_eval_templates", "ft_set_option",
-           "ft_get_counters", "ft_last_error", "ft_describe", "ft_destroy"]
+FT_OPT_SELECT_CAP, FT_OPT_COUNT_FLOOR, FT_OPT_ONE_PASS_BOTH, FT_OPT_WCOUNT_FLOOR = 5, 6, 7, 8
+SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_topk_per_box", "ft_set_antenna", "ft_eval_list",
+           "ft_eval_templates", "ft_bank_draw", "ft_eval_bank", "ft_track", "ft_set_option", "ft_set_option_f64",
+           "ft_get_counters", "ft_measure_peaks", "ft_selftest", "ft_last_error", "ft_describe", "ft_destroy"]
 
 
 class FtGrid(C.Structure):
@@ -34,6 +35,21 @@ class FtCand(C.Structure):
 
 CAND_DTYPE = np.dtype([("power", "<f8"), ("wcount", "<f8"), ("idx", "<u8"), ("count", "<i4"),
                        ("band", "<i4")])
+
+
+CAND_BOX_DTYPE = np.dtype([("power", "<f8"), ("wcount", "<f8"), ("idx", "<u8"), ("count", "<i4"), ("box", "<i4"),
+                           ("z", "<f8"), ("sigma", "<f8")])   # ft_cand_box
+
+BANK_FIELDS = ("f0_lo", "f0_hi", "f1_lo", "f1_hi", "ra_lo", "ra_hi", "sd_lo", "sd_hi", "ap_lo", "ap_hi",
+               "porb_lo", "porb_hi", "t_ref")
+
+
+class FtBankBox(C.Structure):
+    _fields_ = [(n, C.c_double) for n in BANK_FIELDS]
+
+
+class FtPeaks(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("smem_gbs", "fp64_gflops", "fp64_cvt_gops", "l2_gbs", "sm_clock_mhz")]
 
 
 TEMPLATE_DTYPE = np.dtype([("f0", "<f8"), ("f1", "<f8"), ("nx", "<f8"), ("ny", "<f8"), ("nz", "<f8"),
@@ -80,6 +96,24 @@ def load_library(path: str | None = None):
         lib.ft_eval_templates.restype = C.c_int
         lib.ft_eval_templates.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int, C.c_double,
                                           C.c_void_p, C.c_void_p]
+        lib.ft_topk_per_box.restype = C.c_int
+        lib.ft_topk_per_box.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_double, C.c_int32, C.c_int, C.c_void_p,
+                                        C.POINTER(C.c_int32)]
+        lib.ft_set_antenna.restype = C.c_int
+        lib.ft_set_antenna.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.ft_bank_draw.restype = C.c_int
+        lib.ft_bank_draw.argtypes = [C.c_void_p, C.POINTER(FtBankBox), C.c_uint64, C.c_uint64, C.c_int64, C.c_void_p]
+        lib.ft_eval_bank.restype = C.c_int
+        lib.ft_eval_bank.argtypes = [C.c_void_p, C.POINTER(FtBankBox), C.c_uint64, C.c_uint64, C.c_int64, C.c_int,
+                                     C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.ft_track.restype = C.c_int
+        lib.ft_track.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
+        lib.ft_set_option_f64.restype = C.c_int
+        lib.ft_set_option_f64.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        lib.ft_measure_peaks.restype = C.c_int
+        lib.ft_measure_peaks.argtypes = [C.c_void_p, C.POINTER(FtPeaks)]
+        lib.ft_selftest.restype = C.c_int
+        lib.ft_selftest.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.c_uint64, C.POINTER(C.c_uint64)]
         lib.ft_set_option.restype = C.c_int
         lib.ft_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         lib.ft_get_counters.restype = C.c_int
@@ -156,6 +190,73 @@ class Context:
         nb = C.c_int32(0)
         self._check(self.lib.ft_topk_per_band(self.h, float(band_width_hz), int(k), _hp(out), C.byref(nb)))
         return out.reshape(-1)[: nb.value * k].reshape(nb.value, k)
+
+    def set_option_f64(self, option: int, value: float):
+        self._check(self.lib.ft_set_option_f64(self.h, option, float(value)))
+
+    def set_antenna(self, lat=None, gamma=None, lst=None):
+        """Per-SFT detector latitude, arm orientation and local sidereal angle (radians): sky-dependent weights."""
+        if lat is None:
+            self._check(self.lib.ft_set_antenna(self.h, None, None, None))
+            return
+        a = [np.ascontiguousarray(x, dtype=np.float64) for x in (lat, gamma, lst)]
+        assert all(x.shape == (self.n_sft,) for x in a)
+        self._check(self.lib.ft_set_antenna(self.h, _hp(a[0]), _hp(a[1]), _hp(a[2])))
+
+    def topk_per_box(self, pbox, n_pbox: int, band_width_hz: float, k: int, rank_by_z: bool = False):
+        """pbox: int32 [n_points] (or None).  Returns ft_cand_box records [n_regions][k]."""
+        bpb = max(1, int(round(band_width_hz / self._df0))) if self._df0 > 0 else 1
+        n_bands = max(-(-self._n_f0 // bpb), 1)
+        n_pbox = int(n_pbox) if pbox is not None else 1
+        out = np.zeros((n_pbox * n_bands, k), dtype=CAND_BOX_DTYPE)
+        nr = C.c_int32(0)
+        pb = None
+        if pbox is not None:
+            pb = np.ascontiguousarray(pbox, dtype=np.int32)
+            assert pb.size * self._n_f0 == self.n_templates
+        self._check(self.lib.ft_topk_per_box(self.h, _hp(pb) if pb is not None else None, n_pbox, float(band_width_hz),
+                                             int(k), 1 if rank_by_z else 0, _hp(out), C.byref(nr)))
+        return out.reshape(-1)[: nr.value * k].reshape(nr.value, k)
+
+    @staticmethod
+    def _box(box) -> "FtBankBox":
+        return FtBankBox(*[float(box[f]) for f in BANK_FIELDS])
+
+    def bank_draw(self, box: dict, seed: int, first: int, out_dev):
+        """Fill a torch device tensor of n x 8 float64 with templates first .. first + n - 1 of a xi-uniform bank."""
+        assert out_dev.is_cuda and out_dev.is_contiguous() and out_dev.numel() * out_dev.element_size() % 64 == 0
+        n = out_dev.numel() * out_dev.element_size() // 64
+        bx = self._box(box)
+        self._check(self.lib.ft_bank_draw(self.h, C.byref(bx), int(seed), int(first), n, C.c_void_p(out_dev.data_ptr())))
+
+    def eval_bank(self, box: dict, seed: int, first: int, n: int, stat: str, rho_th: float, out_power=None, out_count=None):
+        """Draw + evaluate n templates of a xi-uniform bank; returns (best candidate record, best template record)."""
+        for o in (out_power, out_count):
+            assert o is None or (o.is_cuda and o.numel() == n and o.is_contiguous())
+        pp = C.c_void_p(out_power.data_ptr()) if out_power is not None else None
+        pc = C.c_void_p(out_count.data_ptr()) if out_count is not None else None
+        best = np.zeros(1, dtype=CAND_DTYPE)
+        tp = np.zeros(1, dtype=TEMPLATE_DTYPE)
+        bx = self._box(box)
+        self._check(self.lib.ft_eval_bank(self.h, C.byref(bx), int(seed), int(first), int(n), FT_STAT[stat], float(rho_th),
+                                          pp, pc, _hp(best), _hp(tp)))
+        return best[0], tp[0]
+
+    def track(self, template, t_ref: float):
+        tp = np.ascontiguousarray(np.atleast_1d(template), dtype=TEMPLATE_DTYPE)
+        k = np.zeros(self.n_sft, dtype=np.int64)
+        self._check(self.lib.ft_track(self.h, _hp(tp), float(t_ref), _hp(k)))
+        return k
+
+    def measure_peaks(self) -> dict:
+        p = FtPeaks()
+        self._check(self.lib.ft_measure_peaks(self.h, C.byref(p)))
+        return {f: getattr(p, f) for f, _ in FtPeaks._fields_}
+
+    def selftest(self, which: int, n: int, seed: int = 1) -> int:
+        nf = C.c_uint64(0)
+        self._check(self.lib.ft_selftest(self.h, int(which), int(n), int(seed), C.byref(nf)))
+        return int(nf.value)
 
     def eval_list(self, idx):
         idx = np.ascontiguousarray(idx, dtype=np.uint64)

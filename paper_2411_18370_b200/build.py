@@ -37,7 +37,8 @@ def _stale() -> bool:
 
 def _compile_one(nvcc, src, verbose):
     obj = os.path.join(OBJ, src[:-3] + ".o")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
+    extra = os.environ.get("FT_NVCC_EXTRA", "").split()   # e.g. -DFT_K1_INT_CVT=0 (tuning experiments)
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     return src, obj, r
 

@@ -22,13 +22,18 @@ struct FtDev {
   const double* P_orb;  // [n_porb]
   const double* tasc;   // [n_tasc]
   const double* ctab;   // [n_porb*n_tasc][n_sft] cos(Om (t_mid - t_asc)) or nullptr (binary grids, bind time)
+  const double* ant;    // [n_sft][9] antenna-pattern coefficients A[5], B[4] of the SFT's detector and sidereal
+                        // angle (ft_set_antenna), or nullptr: weights w are used as given
+  const float* c_row;   // [n_sft] per-row constant the fold removed from Q (row-weighted gather add-back)
   int64_t n_sft, n_bins, ld;
   int64_t n_f0, n_sky;
   int32_t n_f1, n_ap, n_porb, n_tasc;
   int32_t wkind;
+  int32_t skyw;         // 1: sky-dependent weights w_a(n) = u_a(n) w_a / sum_b u_b(n) w_b, u = a^2 + b^2 (Eq. 4-5)
   float rho;
   double f_min, inv_df, f0_start, df0, f1_start, df1, t_ref;
   uint64_t n_points;  // n_sky*n_ap*n_porb*n_tasc*n_f1 ; canonical idx = point*n_f0 + i_f0
+  double mu_G, sigma_G; // sum_a w_a and sqrt(sum_a w_a^2) of the fixed weights (Eq. 13-14 on the P = s/2 scale)
 };
 
 // Parameters of one "outer point" = everything of a template but f0.
@@ -80,6 +85,31 @@ __device__ __forceinline__ bool ft_near_tie(double x) {
   return fabs((x - floor(x)) - 0.5) < 1e-9;
 }
 
+// Antenna-pattern weights (Eq. 4; a, b of Jaranowski, Krolak & Schutz 1998, the paper's ref. [20],
+// Eq. (12)-(13) there), written as a(t; n) = sum_m A_m(t) Y_m(n), b(t; n) = sum_m B_m(t) Z_m(n): the detector
+// and time dependence A[5], B[4] sits in a per-SFT table built at ft_set_antenna, the sky dependence below
+// (no trigonometric call: cos/sin of the right ascension and declination come from the unit vector n).
+struct FtSkyPoint { double Y[5], Z[4]; };
+
+__device__ __forceinline__ FtSkyPoint ft_sky_point(double nx, double ny, double nz) {
+  const double rho2 = nx * nx + ny * ny;
+  const double rho = sqrt(rho2), r = sqrt(rho2 + nz * nz);
+  const double ca = rho > 0.0 ? nx / rho : 1.0, sa = rho > 0.0 ? ny / rho : 0.0;   // at the poles a^2 + b^2 does not depend on alpha
+  const double sd = nz / r, cd = rho / r;
+  const double c2a = ca * ca - sa * sa, s2a = 2.0 * sa * ca;
+  const double s2d = 2.0 * sd * cd, c2d = cd * cd - sd * sd;
+  FtSkyPoint p;
+  p.Y[0] = (3.0 - c2d) * c2a; p.Y[1] = (3.0 - c2d) * s2a; p.Y[2] = s2d * ca; p.Y[3] = s2d * sa; p.Y[4] = cd * cd;
+  p.Z[0] = sd * c2a; p.Z[1] = sd * s2a; p.Z[2] = cd * ca; p.Z[3] = cd * sa;
+  return p;
+}
+// u = a^2 + b^2 at one SFT (ant = that SFT's row of FtDev::ant)
+__device__ __forceinline__ double ft_antenna_u(const double* __restrict__ ant, const FtSkyPoint& p) {
+  const double a = ant[0] * p.Y[0] + ant[1] * p.Y[1] + ant[2] * p.Y[2] + ant[3] * p.Y[3] + ant[4] * p.Y[4];
+  const double b = ant[5] * p.Z[0] + ant[6] * p.Z[1] + ant[7] * p.Z[2] + ant[8] * p.Z[3];
+  return a * a + b * b;
+}
+
 // order-preserving float <-> uint32 key (larger float -> larger key)
 __device__ __forceinline__ uint32_t ft_key(float v) {
   const uint32_t u = __float_as_uint(v);
@@ -89,13 +119,15 @@ __device__ __forceinline__ float ft_unkey(uint32_t k) {
   return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
 }
 
-// Candidate record as it sits in device buffers.
+// Candidate record as it sits in device buffers (ft_cand: the first 32 bytes; ft_cand_box: all 48).
 struct FtCandDev {
   double power;
   double wcount;
   uint64_t idx;
   int32_t count;
-  int32_t band;
+  int32_t band;    // region of the selection (frequency sub-band, or box)
+  double z;        // (power - mu_G) / sigma_G of the template's weights (Eq. 36)
+  double sigma;    // sigma_G
 };
 
 // ---- host-visible launchers (defined in the .cu files) ---------------------------------------
@@ -108,7 +140,6 @@ cudaError_t ft_launch_refine(const FtDev& d, const uint64_t* idx_dev, const uint
                              FtCandDev* out, unsigned long long* near_ties, cudaStream_t s);
 // ctab[(i_porb*n_tasc + i_tasc)][a] = cos(Om (t_mid[a] - t_asc)), the same expression ft_doppler evaluates
 cudaError_t ft_launch_ctab(const FtDev& d, double* ctab, cudaStream_t s);
-// K1: explicit template list (records of 8 doubles: f0, f1, nx, ny, nz, a_p, P_orb, t_asc), device memory
-cudaError_t ft_launch_list(const FtDev& d, int stat, const void* templates_dev, int64_t n, double t_ref,
-                           float* out_power, int32_t* out_count, int32_t* err, unsigned long long* near_ties,
-                           cudaStream_t s);
+// one explicit template (record of 8 doubles: f0, f1, nx, ny, nz, a_p, P_orb, t_asc) in fp64; optional bins k_out[n_sft]
+cudaError_t ft_launch_refine_template(const FtDev& d, const double* template_dev, double t_ref, FtCandDev* out,
+                                      int64_t* k_out, int32_t* err, cudaStream_t s);

@@ -1,6 +1,10 @@
-// Device-side pieces shared by the tile kernels (ft_tile.cu: fp32 gather; ft_tile8.cu: packed
-// number-count gather): mbarrier / TMA bulk-copy wrappers, kernel arguments, the packed track entry
-// and the canonical (shift, break) computation of one (outer point, SFT, warp range).
+// Device side of the tile kernels: ONE kernel body (prologue, TMA producer ring, canonical track entries,
+// row loop, epilogue with the fused selection) templated on a gather policy:
+//   GatherF32   (ft_tile.cu)   fp32 pixels, packed fp32 add             Eq. (3) on Q, Eq. (7) on the 0/1 map
+//   GatherF32W  (ft_tilew.cu)  fp32 pixels x per-(point, SFT) weight    Eq. (3)-(5) with sky-dependent weights
+//   GatherBoth  (ft_tileb.cu)  fp32 pixels with the hit bit in the LSB  Eq. (3) and Eq. (7) from one gather
+//   GatherHit8  (ft_tile8.cu)  packed byte hit map, 8-bit SIMD counters Eq. (7)
+// DESIGN.md "Kernels".  PAPER.md:53 (Eq. 2), :64 (Eq. 3), :69-84 (Eq. 4-5), :95 (Eq. 7), :330-351 (selection).
 #pragma once
 #include "ft_common.cuh"
 #include "ft_select.cuh"
@@ -14,36 +18,48 @@ struct FtTileArgs {
   int32_t tile_w, n_tiles, R, wpp, pitch, copy_floats, n_stages;
   uint64_t pt_begin, pt_end;
   double add_back;  // sum over SFTs of the per-row constant removed from A at fold time
+  const float* c_row;   // [n_sft] that per-row constant (row-weighted gather: add-back = sum_a u_a c_a)
   float* out_f;
   int32_t* out_i;
   uint64_t out_base;
   FtSelectDev sel;
   int32_t has_sel, bpb;
+  // regions of the selection: box = pbox[pt] * n_bands + i_f0 / bpb (pbox == nullptr: frequency sub-bands only)
+  const int32_t* pbox;
+  int32_t n_bands;
+  // standardised keys z = (s - mu) / sigma (Eq. 36): fixed weights use (z_mu, z_inv_sigma); the
+  // row-weighted gather computes mu = 1 and sigma per point itself
+  int32_t zmode;
+  int32_t out_key;      // out_f receives the selection key (z in zmode) instead of the statistic
+  double z_mu, z_inv_sigma;
+  float* out_sigma;     // row-weighted gather: sigma_G of every outer point, [n_points] (or nullptr)
   unsigned long long* near_ties;
-  uint32_t group_stride;  // > 1: every stride-th group only (threshold sample), outputs packed by launch-local row
-  uint32_t skip_stride;   // > 1: every group EXCEPT the first skip_n multiples of skip_stride (the rest of the bank)
-  uint64_t skip_n;
+  const uint32_t* glist;  // != nullptr: the launch runs the CTA groups glist[0 .. grid / n_tiles) (the threshold
+                          // sample), outputs packed by launch-local row (group_local * R + r) * n_f0 + i_f0
+  const uint32_t* gskip;  // != nullptr: bit g set = group g was in the sample; its CTAs exit at once (the rest of the bank)
 };
 
-// Threads per CTA the kernel is compiled for: (consumer warps + 1 producer warp) * 32.  The
-// accumulators (J) and the loads in flight (J) set the register need, hence the bound.
+// Threads per CTA the kernels are compiled for: (consumer warps + 1 producer warp) * 32.  The accumulators
+// (J) and the loads in flight (J) set the register need, hence the bound.
 // (the register file is 4 x 16 384: 80 registers allow 6 warps per SM sub-partition, 72 allow 7, 64 allow 8)
 __host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : 72; }
 __host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 1024 : 896; }
 // packed number-count kernel: J registers of 8-bit counters + J loads in flight (16-bit levels in shared memory)
 __host__ __device__ constexpr int ft_tile8_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tile8_max_threads(int J) { return J <= 8 ? 1024 : 768; }
-
-// both statistics in one pass (ft_tileb.cu): J accumulators + J counters + J loads in flight
+// both statistics in one pass: J accumulators + J counters + J loads in flight
 __host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : 768; }
-cudaError_t ft_tileb_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem,
-                            cudaStream_t s);
+// row-weighted gather: J accumulators + J loads in flight + the fp64 weight sums
+__host__ __device__ constexpr int ft_tilew_max_regs(int J) { return J <= 8 ? 64 : 80; }
+__host__ __device__ constexpr int ft_tilew_max_threads(int J) { return J <= 8 ? 1024 : 768; }
 
-// packed number-count kernels (ft_tile8.cu); A = the 4 byte-shifted hit maps d.H8
-cudaError_t ft_tile8_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem,
-                            cudaStream_t s);
+cudaError_t ft_tile_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
+cudaError_t ft_tilew_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
+cudaError_t ft_tileb_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
+cudaError_t ft_tile8_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
 
+#ifdef __CUDACC__
 namespace {
 
 constexpr int kMaxPitch = 8191;  // packed entry: 13 bits of strip offset
@@ -73,6 +89,19 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ float lds_f32(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
 
 // (a0, a1) += (v0, v1) as ONE instruction: sm_100's packed fp32 add (SASS FADD2), round-to-nearest like FADD
 __device__ __forceinline__ void ft_add2(float& a0, float& a1, float v0, float v1) {
@@ -80,6 +109,15 @@ __device__ __forceinline__ void ft_add2(float& a0, float& a1, float v0, float v1
   asm("mov.b64 %0, {%1, %2};" : "=l"(a2) : "f"(a0), "f"(a1));
   asm("mov.b64 %0, {%1, %2};" : "=l"(v2) : "f"(v0), "f"(v1));
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(a2) : "l"(a2), "l"(v2));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a0), "=f"(a1) : "l"(a2));
+}
+// (a0, a1) += w * (v0, v1): packed fp32 fused multiply-add (SASS FFMA2)
+__device__ __forceinline__ void ft_fma2(float& a0, float& a1, float v0, float v1, float w) {
+  unsigned long long a2, v2, w2;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(a2) : "f"(a0), "f"(a1));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(v2) : "f"(v0), "f"(v1));
+  asm("mov.b64 %0, {%1, %1};" : "=l"(w2) : "f"(w));
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(a2) : "l"(v2), "l"(w2), "l"(a2));
   asm("mov.b64 {%0, %1}, %2;" : "=f"(a0), "=f"(a1) : "l"(a2));
 }
 
@@ -144,4 +182,397 @@ __device__ __forceinline__ uint32_t ft_tile_entry(const FtDev& d, const FtPoint&
   return pack_entry(off, rel, neg);
 }
 
+// ---- gather policies ---------------------------------------------------------------------------------
+// A policy provides: CW (f0 per chunk = per warp load instruction), PER (f0 per lane per chunk), ROWW (a
+// per-(point, SFT) weight multiplies the row), VETO (the fused filter applies the number-count floor from
+// registers), the accumulator state, the producer's copies of one row, the two row bodies (no break / one
+// break inside the warp's range), a hook after every block of 32 SFTs, and the final value of one output.
+
+// fp32 pixels: J conflict-free LDS.32 + J/2 packed adds per row
+struct GatherF32 {
+  static constexpr int CW = 32, PER = 1;
+  static constexpr bool ROWW = false, VETO = false, HASCNT = false;
+  template <int J> struct State { float acc[J]; };
+  static __device__ __forceinline__ size_t extra_smem(int, int) { return 0; }
+  template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t, uint32_t) {
+#pragma unroll
+    for (int j = 0; j < J; ++j) st.acc[j] = 0.f;
+  }
+  static __device__ __forceinline__ void produce_row(const FtDev& d, const FtTileArgs& a, uint32_t dst, int row, int k0,
+                                                     uint32_t bar) {
+    const int64_t src = (int64_t)row * d.ld + k0;
+    const uint32_t nb = 4u * (uint32_t)min((int64_t)a.copy_floats, d.n_sft * d.ld - src);
+    bulk_g2s(dst, a.A + src, nb, bar);
+  }
+  static __device__ __forceinline__ uint32_t row_tx_bytes(const FtDev& d, const FtTileArgs& a, int row, int k0) {
+    const int64_t src = (int64_t)row * d.ld + k0;
+    return 4u * (uint32_t)min((int64_t)a.copy_floats, d.n_sft * d.ld - src);
+  }
+  template <int J> static __device__ __forceinline__ void row_fast(State<J>& st, uint32_t e, uint32_t base, uint32_t,
+                                                                   bool last_ok, float) {
+    const uint32_t ad = base + 4u * e;
+    float v[J];
+#pragma unroll
+    for (int j = 0; j < J; ++j)
+      if (j < J - 1 || last_ok) v[j] = lds_f32(ad + 128u * j);
+    if (!last_ok) v[J - 1] = 0.f;
+#pragma unroll
+    for (int j = 0; j + 1 < J; j += 2) ft_add2(st.acc[j], st.acc[j + 1], v[j], v[j + 1]);
+    if (J & 1) st.acc[J - 1] += v[J - 1];
+  }
+  template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t,
+                                                                    int lane, float) {
+    const uint32_t ad_lo = base + 4u * (e & 8191u);
+    const uint32_t ad_hi = (e & (1u << 24)) ? ad_lo - 4u : ad_lo + 4u;
+    const int t_lane = (int)((e >> 13) & 2047u) - lane;
+#pragma unroll
+    for (int j = 0; j < J; ++j) st.acc[j] += lds_f32(((32 * j >= t_lane) ? ad_hi : ad_lo) + 128u * j);
+  }
+  template <int J, class S> static __device__ __forceinline__ void block_end(S&, int) {}
+  template <int J, class S> static __device__ __forceinline__ void finalize(S&) {}
+  // value of output (chunk j, sub-position c) before the final scale, and its integer count (HASCNT policies)
+  template <int J> static __device__ __forceinline__ void result(State<J>& st, int j, int, double add_back, double* v, int32_t* c) {
+    *v = (double)st.acc[j] + add_back;
+    *c = 0;
+  }
+};
+
+// fp32 pixels times a per-(point, SFT) weight u (sky-dependent weights, Eq. 4): packed FFMA
+struct GatherF32W : GatherF32 {
+  static constexpr bool ROWW = true;
+  template <int J> static __device__ __forceinline__ void row_fast(State<J>& st, uint32_t e, uint32_t base, uint32_t,
+                                                                   bool last_ok, float u) {
+    const uint32_t ad = base + 4u * e;
+    float v[J];
+#pragma unroll
+    for (int j = 0; j < J; ++j)
+      if (j < J - 1 || last_ok) v[j] = lds_f32(ad + 128u * j);
+    if (!last_ok) v[J - 1] = 0.f;
+#pragma unroll
+    for (int j = 0; j + 1 < J; j += 2) ft_fma2(st.acc[j], st.acc[j + 1], v[j], v[j + 1], u);
+    if (J & 1) st.acc[J - 1] = fmaf(u, v[J - 1], st.acc[J - 1]);
+  }
+  template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t,
+                                                                    int lane, float u) {
+    const uint32_t ad_lo = base + 4u * (e & 8191u);
+    const uint32_t ad_hi = (e & (1u << 24)) ? ad_lo - 4u : ad_lo + 4u;
+    const int t_lane = (int)((e >> 13) & 2047u) - lane;
+#pragma unroll
+    for (int j = 0; j < J; ++j) st.acc[j] = fmaf(u, lds_f32(((32 * j >= t_lane) ? ad_hi : ad_lo) + 128u * j), st.acc[j]);
+  }
+};
+
+// fp32 pixels of QB (Q with the hit bit (P > rho_th) in the mantissa LSB): power and count from one LDS
+struct GatherBoth : GatherF32 {
+  static constexpr bool VETO = true, HASCNT = true;
+  template <int J> struct State { float acc[J]; uint32_t cnt[J]; };
+  template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t, uint32_t) {
+#pragma unroll
+    for (int j = 0; j < J; ++j) { st.acc[j] = 0.f; st.cnt[j] = 0u; }
+  }
+  template <int J> static __device__ __forceinline__ void row_fast(State<J>& st, uint32_t e, uint32_t base, uint32_t,
+                                                                   bool last_ok, float) {
+    const uint32_t ad = base + 4u * e;
+    float v[J];
+#pragma unroll
+    for (int j = 0; j < J; ++j)
+      if (j < J - 1 || last_ok) v[j] = lds_f32(ad + 128u * j);
+    if (!last_ok) v[J - 1] = 0.f;
+#pragma unroll
+    for (int j = 0; j + 1 < J; j += 2) ft_add2(st.acc[j], st.acc[j + 1], v[j], v[j + 1]);
+    if (J & 1) st.acc[J - 1] += v[J - 1];
+#pragma unroll
+    for (int j = 0; j < J; ++j) st.cnt[j] += __float_as_uint(v[j]) & 1u;  // the hit bit rides in the LSB
+  }
+  template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t,
+                                                                    int lane, float) {
+    const uint32_t ad_lo = base + 4u * (e & 8191u);
+    const uint32_t ad_hi = (e & (1u << 24)) ? ad_lo - 4u : ad_lo + 4u;
+    const int t_lane = (int)((e >> 13) & 2047u) - lane;
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const float v = lds_f32(((32 * j >= t_lane) ? ad_hi : ad_lo) + 128u * j);
+      st.acc[j] += v;
+      st.cnt[j] += __float_as_uint(v) & 1u;
+    }
+  }
+  template <int J> static __device__ __forceinline__ void result(State<J>& st, int j, int, double add_back, double* v, int32_t* c) {
+    *v = (double)st.acc[j] + add_back;
+    *c = (int32_t)st.cnt[j];
+  }
+};
+
+// packed byte hit map in four byte-shifted copies: H8[m][a][b] = (P[a][b + m] > rho_th), so the 4 hits of 4
+// consecutive f0 starting at any bin are ONE aligned 32-bit word of copy (bin mod 4).  A lane owns 4
+// consecutive f0 per 128-wide chunk: 1 LDS.32 + 1 IADD into four 8-bit counters per 4 evaluations; every 224
+// SFTs the counters are folded into 16-bit levels in shared memory (n_sft <= 65535 is a plan condition).
+struct GatherHit8 {
+  static constexpr int CW = 128, PER = 4;
+  static constexpr bool ROWW = false, VETO = false, HASCNT = true;
+  static constexpr int kFlushBlocks = 7;  // 7 blocks of 32 SFTs = 224 <= 255 increments per 8-bit counter
+  template <int J> struct State { uint32_t c8[J]; uint32_t c16, n_ct; };
+  template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t extra0, uint32_t n_ct) {
+    st.c16 = extra0 + 4u * threadIdx.x;
+    st.n_ct = n_ct;
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      st.c8[j] = 0u;
+      sts_u32(st.c16 + 4u * n_ct * (2 * j), 0u);
+      sts_u32(st.c16 + 4u * n_ct * (2 * j + 1), 0u);
+    }
+  }
+  static __device__ __forceinline__ void produce_row(const FtDev& d, const FtTileArgs& a, uint32_t dst, int row, int k0,
+                                                     uint32_t bar) {
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+      bulk_g2s(dst + (uint32_t)m * (uint32_t)a.pitch, d.H8 + ((int64_t)m * d.n_sft + row) * d.ld8 + k0,
+               (uint32_t)a.copy_floats, bar);
+  }
+  static __device__ __forceinline__ uint32_t row_tx_bytes(const FtDev&, const FtTileArgs& a, int, int) {
+    return 4u * (uint32_t)a.copy_floats;
+  }
+  template <int J> static __device__ __forceinline__ void row_fast(State<J>& st, uint32_t e, uint32_t base, uint32_t copy_pitch,
+                                                                   bool last_ok, float) {
+    // word of copy (off mod 4) that holds bins off .. off+3 of this lane's first 4 outputs
+    const uint32_t ad = base + (e & 3u) * copy_pitch + (e & ~3u);
+    uint32_t v[J];
+#pragma unroll
+    for (int j = 0; j < J; ++j)
+      if (j < J - 1 || last_ok) v[j] = lds_u32(ad + 128u * j);
+#pragma unroll
+    for (int j = 0; j < J; ++j)
+      if (j < J - 1 || last_ok) st.c8[j] += v[j];
+  }
+  template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t copy_pitch,
+                                                                    int lane, float) {
+    const uint32_t off = e & 8191u;
+    const uint32_t ad_lo = base + (off & 3u) * copy_pitch + (off & ~3u);
+    const uint32_t off_hi = (e & (1u << 24)) ? off - 1u : off + 1u;
+    const uint32_t ad_hi = base + (off_hi & 3u) * copy_pitch + (off_hi & ~3u);
+    const int t_lane = (int)((e >> 13) & 2047u) - 4 * lane;  // outputs of this lane's chunk 0 before the break
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const int cut = t_lane - 128 * j;  // >= 4: all before the break, <= 0: all after
+      const uint32_t va = lds_u32(ad_lo + 128u * j), vb = lds_u32(ad_hi + 128u * j);
+      const uint32_t mask = cut >= 4 ? 0xffffffffu : (cut <= 0 ? 0u : ((1u << (8 * cut)) - 1u));
+      st.c8[j] += (va & mask) | (vb & ~mask);
+    }
+  }
+  template <int J> static __device__ __forceinline__ void flush(State<J>& st) {
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const uint32_t aa = st.c16 + 4u * st.n_ct * (2 * j), ab = st.c16 + 4u * st.n_ct * (2 * j + 1);
+      sts_u32(aa, lds_u32(aa) + (st.c8[j] & 0x00ff00ffu));
+      sts_u32(ab, lds_u32(ab) + ((st.c8[j] >> 8) & 0x00ff00ffu));
+      st.c8[j] = 0u;
+    }
+  }
+  template <int J> static __device__ __forceinline__ void block_end(State<J>& st, int blocks_done) {
+    if (blocks_done % kFlushBlocks == 0) flush<J>(st);
+  }
+  template <int J> static __device__ __forceinline__ void finalize(State<J>& st) { flush<J>(st); }
+  template <int J> static __device__ __forceinline__ void result(State<J>& st, int j, int c, double, double* v, int32_t* cnt) {
+    const uint32_t ta = lds_u32(st.c16 + 4u * st.n_ct * (2 * j)), tb = lds_u32(st.c16 + 4u * st.n_ct * (2 * j + 1));
+    const uint32_t r = (c == 0) ? (ta & 0xffffu) : (c == 1) ? (tb & 0xffffu) : (c == 2) ? (ta >> 16) : (tb >> 16);
+    *cnt = (int32_t)r;
+    *v = (double)r;
+  }
+};
+
+// Shared-memory layout (bytes): ring [NS][kRPS][row_bytes] | full[NS] empty[NS] mbarriers | FtPoint[n_cw] |
+// entry table [n_cw][32] u32 | (ROWW: weight table [n_cw][32] f32) | policy extra.
+template <class G>
+__host__ __device__ inline size_t ft_tile_state_bytes(int J, int n_cw) {
+  return (sizeof(FtPoint) + 128 + (G::ROWW ? 128 : 0)) * (size_t)n_cw + 16 +
+         (G::PER == 4 ? (size_t)8 * J * 32 * n_cw : 0);
+}
+
+template <int J, class G>
+__device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_cw = a.R * a.wpp;
+  const int tile = (int)(blockIdx.x % (unsigned)a.n_tiles);
+  const uint64_t group_l = blockIdx.x / (unsigned)a.n_tiles;  // launch-local group
+  const uint64_t group = a.glist ? (uint64_t)__ldg(a.glist + group_l) : group_l;
+  if (a.gskip && ((__ldg(a.gskip + (group >> 5)) >> (group & 31)) & 1u)) return;   // (whole CTA: before any barrier)
+  const int n_sft = (int)d.n_sft;
+  const int NS = a.n_stages;
+  const uint32_t copy_pitch = (uint32_t)a.pitch;                 // elements per staged (copy of a) row
+  const uint32_t row_bytes = 4u * copy_pitch;                    // fp32: pitch floats; packed: four byte copies
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NS * kRPS * row_bytes);
+  const uint32_t ring0 = smem_u32(smem_raw);
+  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + NS);
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < NS; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, n_cw);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const int32_t* kst = a.kst + (size_t)tile * n_sft;
+
+  if (warp == n_cw) {
+    // ---- producer: streams the strips (A3).  The whole warp fetches the 32 strip starts of a block
+    // with one coalesced load; lane 0 issues the bulk copies.
+    int s = 0;
+    uint32_t lap = 0;  // how many times the ring has wrapped
+    for (int a0 = 0; a0 < n_sft; a0 += 32) {
+      const int kk = (a0 + lane < n_sft) ? kst[a0 + lane] : 0;
+      const int n_rows = min(32, n_sft - a0);
+      for (int q = 0; q < n_rows; q += kRPS) {
+        if (lap > 0) mbar_wait(empty0 + 8 * s, (lap - 1u) & 1u);  // consumers released the previous use
+        const int rows = min(kRPS, n_rows - q);
+        int kr[kRPS];
+#pragma unroll
+        for (int r = 0; r < kRPS; ++r) kr[r] = __shfl_sync(0xffffffffu, kk, (q + r) & 31);
+        if (lane == 0) {
+          uint32_t bytes = 0;
+#pragma unroll
+          for (int r = 0; r < kRPS; ++r)
+            if (r < rows) bytes += G::row_tx_bytes(d, a, a0 + q + r, kr[r]);
+          mbar_expect_tx(full0 + 8 * s, bytes);
+          const uint32_t dst = ring0 + (uint32_t)(s * kRPS) * row_bytes;
+#pragma unroll
+          for (int r = 0; r < kRPS; ++r)
+            if (r < rows) G::produce_row(d, a, dst + (uint32_t)r * row_bytes, a0 + q + r, kr[r], full0 + 8 * s);
+        }
+        __syncwarp();
+        if (++s == NS) { s = 0; ++lap; }
+      }
+    }
+    return;
+  }
+  if (warp > n_cw) return;
+
+  // ---- consumers -------------------------------------------------------------------------------
+  const int r_pt = warp / a.wpp, sub = warp % a.wpp;
+  uint64_t pt = a.pt_begin + group * (uint64_t)a.R + (uint64_t)r_pt;
+  const bool pt_active = pt < a.pt_end;
+  if (!pt_active) pt = a.pt_end - 1;  // keep the barrier protocol; results are discarded
+  // the point's parameters live in shared memory (17 registers less across the main loop)
+  FtPoint* sp = reinterpret_cast<FtPoint*>(bars + 2 * NS) + warp;
+  if (lane == 0) *sp = ft_decode_point(d, pt);
+  __syncwarp();
+  // per-warp table of the 32 packed track entries of the current SFT block: one broadcast LDS.128
+  // per ring stage instead of one shuffle per row (and, row-weighted, a second table of the 32 weights)
+  const uint32_t etab0 = smem_u32(reinterpret_cast<FtPoint*>(bars + 2 * NS) + n_cw);
+  const uint32_t etab = etab0 + 128u * (uint32_t)warp;
+  const uint32_t wtab = etab0 + 128u * (uint32_t)n_cw + 128u * (uint32_t)warp;
+  const uint32_t extra0 = etab0 + (G::ROWW ? 256u : 128u) * (uint32_t)n_cw;
+  const int tile_i0 = tile * a.tile_w;
+  const int wlo = sub * J * G::CW;                                     // warp's first output, tile-relative
+  const int tile_n = min(a.tile_w, (int)d.n_f0 - tile_i0);             // valid f0 in this tile
+  const int warp_n = max(0, min(J * G::CW, tile_n - wlo));             // valid outputs of this warp
+  const int i_first = tile_i0 + wlo;
+  const bool last_ok = warp_n > G::CW * (J - 1);  // the warp's last chunk holds valid outputs (else: skipped)
+  typename G::template State<J> st;
+  G::template init<J>(st, extra0, 32u * (uint32_t)n_cw);
+  unsigned ties = 0;
+  // row-weighted gather: this lane's share of  sum_a u_a r_a,  sum_a (u_a r_a)^2,  sum_a u_a c_a  (fp64)
+  double w_sum = 0.0, w_sq = 0.0, w_cb = 0.0;
+  FtSkyPoint skyp;
+  if (G::ROWW) skyp = ft_sky_point(sp->nx, sp->ny, sp->nz);
+  const uint32_t lane_bytes = ring0 + 4u * (uint32_t)lane;
+  uint32_t stage_addr = lane_bytes;
+  int s = 0;
+  uint32_t ph = 0;
+
+  for (int a0 = 0; a0 < n_sft; a0 += 32) {
+    // -- A1/A2: this lane's SFT ---------------------------------------------------------------------
+    uint32_t entry = 0;
+    if (a0 + lane < n_sft && warp_n > 0)
+      entry = ft_tile_entry(d, *sp, a0 + lane, kst[a0 + lane], i_first, warp_n, a.copy_floats, &ties, a.err);
+    sts_u32(etab + 4u * (uint32_t)lane, entry);
+    if (G::ROWW) {
+      float uf = 0.f;
+      if (a0 + lane < n_sft) {
+        const double u = ft_antenna_u(d.ant + 9 * (size_t)(a0 + lane), skyp);   // a^2 + b^2 (Eq. 4)
+        uf = (float)u;
+        const double ur = __dmul_rn((double)uf, (double)d.w[a0 + lane]);
+        w_sum = __dadd_rn(w_sum, ur);
+        w_sq = __dadd_rn(w_sq, __dmul_rn(ur, ur));
+        w_cb = __dadd_rn(w_cb, __dmul_rn((double)uf, (double)a.c_row[a0 + lane]));
+      }
+      sts_u32(wtab + 4u * (uint32_t)lane, __float_as_uint(uf));
+    }
+    __syncwarp();
+    // -- A4: gather + reduce over the block's SFTs -----------------------------------------------
+    const int n_rows = min(32, n_sft - a0);
+    for (int q = 0; q < n_rows; q += kRPS) {
+      uint32_t e4[kRPS], u4[kRPS];
+      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                   : "=r"(e4[0]), "=r"(e4[1]), "=r"(e4[2]), "=r"(e4[3]) : "r"(etab + 4u * (uint32_t)q));
+      if (G::ROWW)
+        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(u4[0]), "=r"(u4[1]), "=r"(u4[2]), "=r"(u4[3]) : "r"(wtab + 4u * (uint32_t)q));
+      mbar_wait(full0 + 8 * s, ph);
+#pragma unroll
+      for (int r = 0; r < kRPS; ++r) {
+        if (q + r < n_rows) {
+          const uint32_t e = e4[r];
+          const uint32_t base = stage_addr + (uint32_t)r * row_bytes;
+          const float u = G::ROWW ? __uint_as_float(u4[r]) : 1.f;
+          if (e < 8192u) G::template row_fast<J>(st, e, base, copy_pitch, last_ok, u);   // no break in this warp's range
+          else G::template row_break<J>(st, e, base, copy_pitch, lane, u);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty0 + 8 * s);
+      if (++s == NS) { s = 0; ph ^= 1u; stage_addr = lane_bytes; } else { stage_addr += kRPS * row_bytes; }
+    }
+    G::template block_end<J>(st, a0 / 32 + 1);
+  }
+
+  // ---- A5/A6: epilogue ---------------------------------------------------------------------------
+  if (a.near_ties) {
+    for (int o = 16; o > 0; o >>= 1) ties += __shfl_xor_sync(0xffffffffu, ties, o);
+    if (lane == 0 && pt_active && ties) atomicAdd(a.near_ties, (unsigned long long)ties);
+  }
+  double add_back = a.add_back, scale = 1.0, z_mu = a.z_mu, z_is = a.z_inv_sigma;
+  if (G::ROWW) {
+    // Eq. (5): the weights of this point are u_a r_a / sum_b u_b r_b; sigma_G^2 = sum w^2 (Eq. 14 on the P = s/2 scale)
+    for (int o = 16; o > 0; o >>= 1) {
+      w_sum += __shfl_xor_sync(0xffffffffu, w_sum, o);
+      w_sq += __shfl_xor_sync(0xffffffffu, w_sq, o);
+      w_cb += __shfl_xor_sync(0xffffffffu, w_cb, o);
+    }
+    add_back = w_cb;
+    scale = 1.0 / w_sum;
+    const double sigma = sqrt(w_sq) * scale;
+    z_mu = 1.0; z_is = 1.0 / sigma;
+    if (a.out_sigma && lane == 0 && sub == 0 && tile == 0 && pt_active) a.out_sigma[pt] = (float)sigma;
+  }
+  if (!pt_active) return;
+  G::template finalize<J>(st);
+  const int64_t box0 = a.pbox ? (int64_t)__ldg(a.pbox + pt) * a.n_bands : 0;
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+#pragma unroll
+    for (int c = 0; c < G::PER; ++c) {
+      const int ii = G::CW * j + G::PER * lane + c;
+      if (ii < warp_n) {
+        const int64_t i = i_first + ii;
+        const uint64_t idx = pt * (uint64_t)d.n_f0 + (uint64_t)i;
+        const uint64_t o = a.glist ? (group_l * (uint64_t)a.R + (uint64_t)r_pt) * (uint64_t)d.n_f0 + (uint64_t)i
+                                              : idx - a.out_base;
+        double vd; int32_t cnt;
+        G::template result<J>(st, j, c, add_back, &vd, &cnt);
+        if (G::ROWW) vd *= scale;
+        const float v = (float)vd;
+        if (!G::HASCNT) cnt = __float2int_rn(v);   // (the 0/1 hit map gathered as fp32: the sum is the integer count)
+        const float key = a.zmode ? (float)((vd - z_mu) * z_is) : v;
+        if (a.out_f) a.out_f[o] = a.out_key ? key : v;
+        if (a.out_i) a.out_i[o] = cnt;
+        if (a.has_sel && (!G::VETO || cnt >= a.sel.veto_floor)) {   // (VETO: number-count floor from the count in registers)
+          const int box = (int)(box0 + i / a.bpb);
+          if (key >= __ldg(a.sel.thr + box)) ft_select_append(a.sel, box, key, idx);
+        }
+      }
+    }
+  }
+}
+
 }  // namespace
+#endif  // __CUDACC__

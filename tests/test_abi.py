@@ -13,7 +13,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def _declared():
     src = open(os.path.join(ROOT, "include", "fasttracks_b200.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(ft_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(ft_[a-z_0-9]+)\s*\(", src)))
 
 
 def test_library_exports_every_declared_symbol():
@@ -26,7 +26,8 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_struct_layouts():
-    assert C.sizeof(B.FtCand) == 32 and B.CAND_DTYPE.itemsize == 32
+    assert C.sizeof(B.FtCand) == 32 and B.CAND_DTYPE.itemsize == 32 and B.CAND_BOX_DTYPE.itemsize == 48
+    assert C.sizeof(B.FtBankBox) == 104 and C.sizeof(B.FtPeaks) == 40
     assert C.sizeof(B.FtCounters) == 56
     assert B.FtGrid.n_f0.offset == 16 and B.FtGrid.t_ref.offset == 48
     assert C.sizeof(B.FtGrid) == 120

@@ -54,7 +54,25 @@ def test_full_size_sampled_outputs_and_candidates(cfg):
         assert np.all((c["idx"] % np.uint64(g.n_f0)).astype(np.int64) // bpb == b)
         key = list(zip(-c["power"], c["idx"]))
         assert key == sorted(key), f"band {b} not in (value desc, idx asc) order"
-    # (c) nothing louder was missed: exact per-band top-k of the GPU's own full fp32 array
+    # (c) nothing louder was missed.  Whole bands against the ORACLE: every template of the band evaluated by the
+    # oracle, its plain sort must give exactly the library's candidates, and the library's full fp32 array must
+    # agree with it element by element (config 2: 9e6 templates x 4000 SFTs per band)
+    for b in {2: (7,), 3: (0, 31), 4: (11,)}[cfg]:
+        n_pt = g.n_templates // g.n_f0
+        cols = np.arange(b * bpb, min(g.n_f0, (b + 1) * bpb), dtype=np.uint64)
+        bidx = (np.arange(n_pt, dtype=np.uint64)[:, None] * np.uint64(g.n_f0) + cols[None, :]).reshape(-1)
+        bp, bc, _, btie = o.eval_list(bidx)
+        order = np.lexsort((bidx, -bp))[:wl.k]
+        assert np.array_equal(cands[b]["idx"], bidx[order]), f"band {b}: candidates differ from the oracle's sort of the whole band"
+        assert np.array_equal(cands[b]["power"], bp[order])
+        okb = btie == 0
+        relb = np.abs(gp[bidx.astype(np.int64)].astype(np.float64) - bp) / bp
+        assert relb[okb].max() <= H.POWER_RTOL
+        if gc is not None:
+            assert np.array_equal(gc[bidx.astype(np.int64)][okb], bc[okb])
+        assert int((~okb).sum()) <= H.near_tie_bound(wl, bidx.size * wl.n_sft)
+    # ... and every other band against the library's own full array (a property, not parity: the fused
+    # selection and the write-out agree)
     full = torch.from_numpy(gp).cuda().view(-1, g.n_f0)
     for b in range(n_bands):
         blk = full[:, b * bpb:(b + 1) * bpb]
@@ -278,3 +296,120 @@ def test_very_few_sfts(n_sft, n_sky, band_hz):
     cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
     H.assert_topk_parity(wl, cands, op, op, oc, wl.k, bpb)
     ctx.close()
+
+
+# ---------------------------------------------------------------- BASELINE.json configs[4]: the scaling sweep
+@pytest.mark.parametrize("size", [0, 1])
+def test_config5_sweep_sizes_exhaustive(size):
+    """Sweep sizes A1 (1e6 templates x 500 SFTs) and A2 (1e7 x 2000): every template against the oracle (full
+    array, top-k fused and through the full write-out)."""
+    from paper_2411_18370_b200 import binding as B
+    n_sft, band_hz, n_sky = W.SWEEP_A[size]
+    wl = W.config5(n_sft, band_hz, n_sky)
+    g = wl.grid
+    op, oc, _, otie = fo.Oracle(wl).eval_range()
+    ctx = H.gpu_context(wl)
+    gp, _ = H.gpu_full(ctx, wl, stat="power")
+    assert "K2 tile kernel" in ctx.describe()
+    flagged = H.assert_full_parity(wl, gp, None, op, oc, otie)
+    assert flagged <= H.near_tie_bound(wl)
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    for fused in (1, 0):
+        ctx.set_option(B.FT_OPT_FUSED_TOPK, fused)
+        ctx.eval(g, "power", wl.rho_th)
+        cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+        H.assert_topk_parity(wl, cands, op, op, oc, wl.k, bpb)
+    ctx.close()
+
+
+def test_config5_16000_sfts_and_4hz_band_geometry():
+    """n_sft = 16 000 (the longest accumulation of the sweep: fp32 sums over the centred array must hold 1e-5) at a
+    reduced sky grid, and the 4 Hz band of the largest sweep size, which plans 4 warps per point over 2 f0 tiles."""
+    wl = W.config5(16000, 1.0, 8)
+    op, oc, _, otie = fo.Oracle(wl).eval_range()
+    ctx = H.gpu_context(wl)
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    H.assert_full_parity(wl, gp, gc, op, oc, otie)
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    ctx.eval(wl.grid, "power", wl.rho_th)
+    H.assert_topk_parity(wl, ctx.topk_per_band(wl.band_width, wl.k, n_bands), op, op, oc, wl.k, bpb)
+    ctx.close()
+    wl = W.config5(64, 4.0, 6)
+    op, oc, _, otie = fo.Oracle(wl).eval_range()
+    ctx = H.gpu_context(wl)
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    desc = ctx.describe().split(";")[0]
+    assert "wpp=4" in desc and "n_tiles=2" in desc, desc
+    H.assert_full_parity(wl, gp, gc, op, oc, otie)
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    ctx.eval(wl.grid, "power", wl.rho_th)
+    H.assert_topk_parity(wl, ctx.topk_per_band(wl.band_width, wl.k, n_bands), op, op, oc, wl.k, bpb)
+    ctx.close()
+
+
+def test_zero_velocity_straight_line_runs_the_tile_kernel():
+    """v = 0, a_p = 0: D = 1 exactly, eps_bound = 0 (the J bound must not overflow).  The statistic
+    is the weighted column sum of the spectrogram."""
+    wl = W.config2(n_sft=200, n_sky=3, band_hz=0.5)
+    wl.vel = np.zeros_like(wl.vel)
+    wl.grid.n_f1, wl.grid.f1_start, wl.grid.df1 = 1, 0.0, 0.0
+    ctx = H.gpu_context(wl, kernel=2)
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    assert "K2 tile kernel" in ctx.describe()
+    k0 = int(round((wl.grid.f0_start - wl.f_min) / wl.df))
+    col = (wl.w.astype(np.float64)[:, None] * wl.P.astype(np.float64)).sum(axis=0)[k0:k0 + wl.grid.n_f0]
+    hits = (wl.P > np.float32(wl.rho_th)).sum(axis=0)[k0:k0 + wl.grid.n_f0]
+    for i_sky in range(3):
+        sl = slice(i_sky * wl.grid.n_f0, (i_sky + 1) * wl.grid.n_f0)
+        assert np.allclose(gp[sl], col, rtol=1e-5) and np.array_equal(gc[sl], hits)
+    ctx.close()
+
+
+def test_config3_full_size_boxes_ranked_by_z():
+    """Config 3 at full size, the paper's post-processing: 64 boxes of (a_p, P_orb, t_asc) points x 50 sub-bands,
+    the loudest of each ranked by z (Eq. 36).  Every candidate re-evaluated by the oracle; the regions of two whole
+    boxes of points against the oracle's exhaustive sort."""
+    wl = _full(3)
+    g = wl.grid
+    o = fo.Oracle(wl)
+    n_pt = g.n_templates // g.n_f0
+    n_pbox = 64
+    pbox = (np.arange(n_pt) * n_pbox // n_pt).astype(np.int32)
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    ctx = H.gpu_context(wl)
+    ctx.eval(g, "both", wl.rho_th)
+    cands = ctx.topk_per_box(pbox, n_pbox, wl.band_width, 1, rank_by_z=True)
+    assert cands.shape == (n_pbox * n_bands, 1) and np.all(cands["idx"] != PAD)
+    flat = cands.reshape(-1)
+    cp, cc, cw, _ = o.eval_list(flat["idx"])
+    assert np.array_equal(flat["power"], cp) and np.array_equal(flat["count"], cc) and np.array_equal(flat["wcount"], cw)
+    w = wl.w.astype(np.float64)
+    assert np.allclose(flat["z"], (cp - w.sum()) / np.sqrt((w ** 2).sum()), rtol=0, atol=1e-9)
+    for pb in (0, 37):
+        pts = np.flatnonzero(pbox == pb).astype(np.uint64)
+        idx = (pts[:, None] * np.uint64(g.n_f0) + np.arange(g.n_f0, dtype=np.uint64)[None, :]).reshape(-1)
+        bp = o.eval_list(idx)[0]
+        band = (idx % np.uint64(g.n_f0)).astype(np.int64) // bpb
+        for b in range(n_bands):
+            m = band == b
+            best = np.lexsort((idx[m], -bp[m]))[0]
+            assert int(cands[pb * n_bands + b, 0]["idx"]) == int(idx[m][best]), (pb, b)
+    ctx.close()
+
+
+def test_bench_two_ranks_on_one_gpu_through_its_own_launcher():
+    """`python bench.py --gpus 2 --dist-backend gloo`: bench.py starts both ranks itself; they share cuda:0, run
+    independent shards (no kernel waits on another rank) and all-gather their candidates over gloo."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--dist-backend", "gloo", "--n-sky", "600",
+                        "--steps", "1", "--warmup", "3", "--no-peaks"], capture_output=True, text=True, env=env, timeout=600)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["value"] > 0 and out["config"]["n_templates_per_gpu"] == 600 * 5 * 1800

@@ -41,7 +41,7 @@ def test_full_arrays_match_oracle(case, kernel):
     ctx = H.gpu_context(wl, kernel=kernel)
     gp, gc = H.gpu_full(ctx, wl, stat="both")
     flagged = H.assert_full_parity(wl, gp, gc, o_power, o_count, o_tie)
-    assert flagged <= max(2, int(1e-6 * wl.n_evals))
+    assert flagged <= H.near_tie_bound(wl)      # a few times the expected 2e-9 per evaluation
     # single-statistic launches give the same arrays
     gp1, _ = H.gpu_full(ctx, wl, stat="power")
     _, gc1 = H.gpu_full(ctx, wl, stat="hough")
@@ -177,4 +177,182 @@ def test_large_k(kernel, fused, k):
     ctx.eval(wl.grid, "power", wl.rho_th)
     cands = ctx.topk_per_band(wl.band_width, k, n_bands)
     H.assert_topk_parity(wl, cands, op, op, oc, k, bpb)
+    ctx.close()
+
+
+# ---------------------------------------------------------------- weighted number count and its veto (:496-502)
+@pytest.mark.parametrize("cfg", [2, 4, 3])
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_weighted_count_statistic(cfg, kernel):
+    """sum_a w_a [P > rho] as a full-array statistic and as the ranking value: fp32 array within 1e-5 of the
+    oracle's fp64 weighted count, integer count bit-exact, candidate sets identical, refined values bit-identical."""
+    wl = H.apply_injections(_small(cfg))
+    o = fo.Oracle(wl)
+    op, oc, owc, otie = o.eval_range()
+    ctx = H.gpu_context(wl, kernel=kernel)
+    gw, gc = H.gpu_full(ctx, wl, stat="whough")
+    ok = otie == 0
+    assert np.array_equal(gc[ok], oc[ok])
+    rel = np.abs(gw.astype(np.float64) - owc) / np.maximum(owc, 1e-300)
+    assert rel[ok].max() <= H.POWER_RTOL, rel[ok].max()
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    for fused in (1, 0):
+        ctx.set_option(__import__("paper_2411_18370_b200.binding", fromlist=["x"]).FT_OPT_FUSED_TOPK, fused)
+        ctx.eval(wl.grid, "whough", wl.rho_th)
+        cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+        ref = fo.topk_per_region(owc, wl.grid.n_f0, bpb, wl.k)
+        H.assert_region_parity(cands, ref, owc, {"wcount": owc, "power": op, "count": oc})
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg,kernel,fused", [(2, 0, 1), (2, 0, 0), (2, 1, 0), (4, 0, 1), (3, 0, 1), (1, 0, 1)])
+def test_weighted_count_veto(cfg, kernel, fused):
+    """The veto as the paper states it: loudest normalized power among templates whose WEIGHTED number count is at
+    least a floor (mean + sigma of the weighted count in Gaussian noise here, so that a good fraction is vetoed).
+    The floor is then set EXACTLY on a template's own fp64 weighted count: the fp32 array cannot decide that
+    template, the fp64 refinement must."""
+    from paper_2411_18370_b200 import binding as B
+    wl = H.apply_injections(_small(cfg))
+    o = fo.Oracle(wl)
+    op, oc, owc, _ = o.eval_range()
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    p_hit = float(np.exp(-wl.rho_th))
+    w = wl.w.astype(np.float64)
+    wbar = w.mean(axis=1) if w.ndim == 2 else w
+    floor0 = p_hit * wbar.sum() + 1.0 * np.sqrt(p_hit * (1 - p_hit) * (wbar ** 2).sum())
+    ctx = H.gpu_context(wl, kernel=kernel, fused=fused)
+    plain_ref = fo.topk_per_region(op, wl.grid.n_f0, bpb, wl.k)
+    top_unvetoed = int(plain_ref[0][0][0])                      # the loudest template of band 0
+    for floor in (floor0, float(owc[top_unvetoed]), float(np.nextafter(owc[top_unvetoed], 1.0))):
+        keep = owc >= floor
+        ref = fo.topk_per_region(op, wl.grid.n_f0, bpb, wl.k, keep=keep)
+        ctx.set_option_f64(B.FT_OPT_WCOUNT_FLOOR, floor)
+        ctx.eval(wl.grid, "both", wl.rho_th)
+        cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+        H.assert_region_parity(cands, ref, op, {"power": op, "count": oc, "wcount": owc})
+        live = cands["idx"] != np.uint64(2 ** 64 - 1)
+        assert np.all(cands["wcount"][live] >= floor)
+    assert (owc < floor0).mean() > 0.3                          # the veto did something
+    ctx.close()
+
+
+# ---------------------------------------------------------------- boxes of points x sub-bands, z (PAPER.md:338-347)
+def _pbox(n_points, n_pbox, kind):
+    pt = np.arange(n_points)
+    if kind == "blocks":
+        return (pt * n_pbox // n_points).astype(np.int32)
+    if kind == "interleaved":
+        return (pt % n_pbox).astype(np.int32)
+    rng = np.random.Generator(np.random.PCG64(77))
+    return rng.integers(0, n_pbox, n_points).astype(np.int32)
+
+
+@pytest.mark.parametrize("cfg,n_pbox,kind,k,by_z", [(2, 3, "blocks", 1, True), (2, 5, "interleaved", 3, False),
+                                                    (3, 4, "blocks", 1, True), (3, 7, "random", 2, True),
+                                                    (4, 3, "blocks", 2, True), (1, 4, "random", 1, False)])
+@pytest.mark.parametrize("kernel,fused", [(0, 1), (0, 0), (1, 0)])
+def test_topk_per_box_and_z(cfg, n_pbox, kind, k, by_z, kernel, fused):
+    """Regions = (box of outer points) x (sub-band); the k loudest of each, ranked by the statistic or by z
+    (Eq. 36).  Oracle: the plain sort of the full array per region."""
+    wl = H.apply_injections(_small(cfg))
+    g = wl.grid
+    o = fo.Oracle(wl)
+    op, oc, owc, _, oz, osig = o.eval_range_z()
+    n_points = g.n_templates // g.n_f0
+    pbox = _pbox(n_points, n_pbox, kind)
+    bpb = int(round(wl.band_width / g.df0))
+    ctx = H.gpu_context(wl, kernel=kernel, fused=fused)
+    ctx.eval(g, "both", wl.rho_th)
+    cands = ctx.topk_per_box(pbox, n_pbox, wl.band_width, k, rank_by_z=by_z)
+    ref = fo.topk_per_region(oz if by_z else op, g.n_f0, bpb, k, pbox=pbox)
+    H.assert_region_parity(cands, ref, op, {"power": op, "count": oc, "wcount": owc}, tol_fields=(("z", oz), ("sigma", osig)))
+    n_bands = -(-g.n_f0 // bpb)
+    assert cands.shape == (n_pbox * n_bands, k)
+    live = cands["idx"] != np.uint64(2 ** 64 - 1)
+    assert np.array_equal(cands["box"][live], (pbox[(cands["idx"][live] // np.uint64(g.n_f0)).astype(np.int64)] * n_bands
+                                               + (cands["idx"][live] % np.uint64(g.n_f0)).astype(np.int64) // bpb))
+    # pbox = None is ft_topk_per_band
+    a = ctx.topk_per_box(None, 1, wl.band_width, k)
+    b = ctx.topk_per_band(wl.band_width, k, n_bands)
+    assert np.array_equal(a["idx"], b["idx"]) and np.array_equal(a["power"], b["power"])
+    ctx.close()
+
+
+def test_topk_per_box_errors():
+    from paper_2411_18370_b200 import binding as B
+    wl = W.config1()
+    ctx = H.gpu_context(wl)
+    ctx.eval(wl.grid, "hough", 1.6)
+    with pytest.raises(B.FtError) as e:      # z needs the power statistic
+        ctx.topk_per_box(None, 1, 0.01, 1, rank_by_z=True)
+    assert e.value.code == -1
+    ctx.eval(wl.grid, "power", 1.6)
+    bad = np.zeros(10, np.int32); bad[3] = 5
+    with pytest.raises(B.FtError) as e:      # pbox value out of range
+        ctx.topk_per_box(bad, 2, 0.01, 1)
+    assert e.value.code == -1
+    # single f0 with df0 = 0: one band, no division (ADVICE round 1)
+    one = W.Grid(f0_start=wl.grid.f0_start, df0=0.0, n_f0=1, sky=wl.grid.sky)
+    ctx.eval(one, "power", 1.6)
+    c = ctx.topk_per_band(0.01, 3, 1)
+    assert c.shape == (1, 3) and (c["idx"] != np.uint64(2 ** 64 - 1)).sum() == 3
+    ctx.close()
+
+
+# ---------------------------------------------------------------- sky-dependent weights (Eq. 4-5)
+@pytest.mark.parametrize("cfg", [2, 1])
+def test_sky_dependent_weights(cfg):
+    """w_a(n) ∝ (a^2 + b^2)(t_a; n) w_a normalised per sky point: full arrays within 1e-5 of the oracle (which
+    evaluates ref. [20]'s a, b directly), counts bit-exact, boxes ranked by z identical to the oracle's sort of z,
+    refined power / z / sigma_G within 1e-12 (the library evaluates a, b through per-SFT and per-sky tables)."""
+    wl = H.apply_injections(_small(cfg))
+    g = wl.grid
+    ant = W.antenna_geometry(wl)
+    o = fo.Oracle(wl, antenna=ant)
+    op, oc, owc, otie, oz, osig = o.eval_range_z()
+    ctx = H.gpu_context(wl)
+    ctx.set_antenna(*ant)
+    gp, gc = H.gpu_full(ctx, wl, stat="both")
+    assert "row-weighted" in ctx.describe()
+    H.assert_full_parity(wl, gp, gc, op, oc, otie)
+    gw, _ = H.gpu_full(ctx, wl, stat="whough", want_count=False)
+    ok = otie == 0
+    assert (np.abs(gw.astype(np.float64) - owc) / owc)[ok].max() <= H.POWER_RTOL
+    # the weights really depend on the sky: the fixed-weight statistic differs
+    o_fixed = fo.Oracle(wl).eval_range()[0]
+    assert np.abs(o_fixed - op).max() > 1e-3 * np.abs(op).mean()
+    n_points = g.n_templates // g.n_f0
+    bpb = int(round(wl.band_width / g.df0))
+    for n_pbox, by_z, k in ((2, True, 1), (3, True, 3), (1, False, 2)):
+        pbox = _pbox(n_points, n_pbox, "blocks")
+        ctx.eval(g, "power", wl.rho_th)
+        cands = ctx.topk_per_box(pbox, n_pbox, wl.band_width, k, rank_by_z=by_z)
+        ref = fo.topk_per_region(oz if by_z else op, g.n_f0, bpb, k, pbox=pbox)
+        H.assert_region_parity(cands, ref, op, {"count": oc},
+                               tol_fields=(("power", op), ("wcount", owc), ("z", oz), ("sigma", osig)))
+    # ranking by z differs from ranking by power somewhere (sigma_G varies over the sky), else the test is vacuous
+    a = fo.topk_per_region(oz, g.n_f0, g.n_f0, 50)[0][0]
+    b = fo.topk_per_region(op, g.n_f0, g.n_f0, 50)[0][0]
+    assert not np.array_equal(a, b)
+    # back to the weights as given
+    ctx.set_antenna(None)
+    gp0, _ = H.gpu_full(ctx, wl, stat="power")
+    assert np.allclose(gp0, o_fixed, rtol=1e-5)
+    ctx.close()
+
+
+def test_sky_dependent_weights_need_per_sft_weights_and_the_tile_kernel():
+    from paper_2411_18370_b200 import binding as B
+    wl4 = _small(4)
+    ctx = H.gpu_context(wl4)
+    with pytest.raises(B.FtError) as e:
+        ctx.set_antenna(*W.antenna_geometry(wl4))
+    assert e.value.code == -7
+    ctx.close()
+    wl = W.config1()
+    ctx = H.gpu_context(wl, kernel=1)
+    ctx.set_antenna(*W.antenna_geometry(wl))
+    with pytest.raises(B.FtError) as e:
+        ctx.eval(wl.grid, "power", 1.6)
+    assert e.value.code == -7
     ctx.close()

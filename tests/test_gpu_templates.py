@@ -76,3 +76,125 @@ def test_empty_list_is_ok():
     ctx = H.gpu_context(wl)
     ctx.eval_templates(torch.empty(0, dtype=torch.float64, device="cuda:0"), 0.0, "power", 1.6, None, None)
     ctx.close()
+
+
+# ---------------------------------------------------------------- arithmetic identities K1 relies on
+def test_division_by_c_and_float_conversion_are_exact():
+    """K1 divides v.n by c with a reciprocal multiply and one fused correction, and converts fp32 to fp64 with
+    integer moves: both must equal the IEEE operations bit for bit (1e8 random quotients; every fp32 pattern)."""
+    ctx = H.gpu_context(W.config1())
+    assert ctx.selftest(0, 100_000_000, seed=3) == 0
+    assert ctx.selftest(0, 10_000_000, seed=4) == 0
+    assert ctx.selftest(1, 1 << 32) == 0
+    ctx.close()
+
+
+# ---------------------------------------------------------------- xi-uniform banks (Eq. A11), drawn on the device
+def _box(wl, binary):
+    g = wl.grid
+    return dict(f0_lo=g.f0_start, f0_hi=g.f0_start + (g.n_f0 - 1) * g.df0, f1_lo=g.f1_start,
+                f1_hi=g.f1_start + (g.n_f1 - 1) * g.df1, ra_lo=0.0, ra_hi=2 * np.pi, sd_lo=-1.0, sd_hi=1.0,
+                ap_lo=float(np.min(g.a_p)) if binary else 0.0, ap_hi=float(np.max(g.a_p)) if binary else 0.0,
+                porb_lo=float(np.min(g.P_orb)), porb_hi=float(np.max(g.P_orb)), t_ref=g.t_ref)
+
+
+@pytest.mark.parametrize("cfg,binary", [(2, False), (3, True)])
+def test_bank_draw_and_eval_bank_match_oracle(cfg, binary):
+    """ft_bank_draw against the oracle's own implementation of the same counter-based xi-uniform draw (parameters to
+    1e-13: pow / sin / cos differ in the last bits between the two libms), and ft_eval_bank (templates drawn in
+    registers) against the oracle evaluating ITS bank: counts bit-exact, power to 1e-6 outside near-ties, and the
+    loudest template of the batch."""
+    import torch
+    wl = {2: lambda: W.config2(n_sft=501, n_sky=7, band_hz=0.35),
+          3: lambda: W.config3(n_sft=403, n_ap=3, n_porb=3, n_tasc=2, n_inj=0)}[cfg]()
+    box = _box(wl, binary)
+    if cfg == 3:   # fixed sky point of the binary config
+        n = wl.grid.sky[0]
+        ra = float(np.arctan2(n[1], n[0]) % (2 * np.pi))
+        box.update(ra_lo=ra, ra_hi=ra, sd_lo=float(n[2]), sd_hi=float(n[2]))
+    n, seed, first = 5000, 17, 123
+    otl = fo.bank_draw(box, seed, first, n)
+    ctx = H.gpu_context(wl)
+    dev = torch.device("cuda:0")
+    t = torch.zeros((n, 8), dtype=torch.float64, device=dev)
+    ctx.bank_draw(box, seed, first, t)
+    torch.cuda.synchronize()
+    gtl = t.cpu().numpy().view(W.TEMPLATE_DTYPE).reshape(-1)
+    for f in W.TEMPLATE_DTYPE.names:
+        assert np.allclose(gtl[f], otl[f], rtol=1e-13, atol=1e-13 * (abs(box["t_ref"]) + 1)), f
+    op, oc, owc, otie = fo.eval_templates(fo.Oracle(wl), otl, box["t_ref"])
+    gp = torch.full((n,), float("nan"), dtype=torch.float32, device=dev)
+    best, btp = ctx.eval_bank(box, seed, first, n, "power", wl.rho_th, out_power=gp)
+    gp = gp.cpu().numpy()
+    ok = otie == 0
+    rel = np.abs(gp.astype(np.float64) - op) / op
+    assert rel[ok].max() <= 1e-6
+    assert int(otie.sum()) <= H.near_tie_bound(wl, n * wl.n_sft)
+    j = int(np.lexsort((np.arange(n), -op))[0])
+    if ok[j]:
+        assert int(best["idx"]) == j
+        assert abs(best["power"] - op[j]) <= 1e-12 * op[j] and best["count"] == oc[j]
+        assert abs(best["wcount"] - owc[j]) <= 1e-12 * owc[j]
+        assert abs(btp["f0"] - otl["f0"][j]) <= 1e-13 * otl["f0"][j]
+    gc = torch.full((n,), -7, dtype=torch.int32, device=dev)
+    bestc, _ = ctx.eval_bank(box, seed, first, n, "hough", wl.rho_th, out_count=gc)
+    gc = gc.cpu().numpy()
+    assert np.array_equal(gc[ok], oc[ok])
+    jc = int(np.lexsort((np.arange(n), -oc))[0])
+    assert int(bestc["idx"]) == jc or not ok[jc]
+    ctx.close()
+
+
+def test_track_of_a_template_equals_the_oracles():
+    wl = W.config3(n_sft=403, n_ap=3, n_porb=3, n_tasc=2, n_inj=0)
+    tl = W.random_bank(wl, 20, seed=5)
+    o = fo.Oracle(wl)
+    ctx = H.gpu_context(wl)
+    for t in tl:
+        k, x, rc = o.track_template(t, wl.grid.t_ref)
+        assert rc == 0
+        kg = ctx.track(t, wl.grid.t_ref)
+        near = np.abs((x - np.floor(x)) - 0.5) < 1e-9
+        assert np.array_equal(kg[~near], k[~near])
+    ctx.close()
+
+
+def test_mismatch_sampler_workload():
+    """a signal injected along a template lambda in Gaussian noise; o N
+    templates drawn uniformly in xi in a box around it; m = (s(lambda) - max s(lambda')) / (s(lambda) - mu_G)
+    (Eq. 24).  The library's loudest template and its statistic equal the oracle's on the oracle's own bank, so
+    the sampled mismatch is the same number; a denser bank gives a smaller mismatch."""
+    import torch
+    wl = W.config2(n_sft=400, n_sky=3, band_hz=0.2)
+    g = wl.grid
+    sig = np.zeros(1, dtype=W.TEMPLATE_DTYPE)
+    n0 = g.sky[1]
+    sig["f0"], sig["f1"] = g.f0_start + 0.1037, -3.3e-10
+    sig["nx"], sig["ny"], sig["nz"] = n0
+    sig["a_p"], sig["P_orb"], sig["t_asc"] = 0.0, 86400.0, 0.0
+    o = fo.Oracle(wl)
+    k, _, rc = o.track_template(sig[0], g.t_ref)
+    assert rc == 0
+    W.inject(wl.P, k, 3.0)                      # inputs: the oracle's track
+    o = fo.Oracle(wl)
+    s_sig = fo.eval_templates(o, sig, g.t_ref)[0][0]
+    mu_G = float(wl.w.astype(np.float64).sum())
+    ra0, sd0 = float(np.arctan2(n0[1], n0[0]) % (2 * np.pi)), float(n0[2])
+    box = dict(f0_lo=float(sig["f0"][0]) - 3 * wl.df, f0_hi=float(sig["f0"][0]) + 3 * wl.df, f1_lo=-4e-10, f1_hi=-2.6e-10,
+               ra_lo=ra0 - 0.02, ra_hi=ra0 + 0.02, sd_lo=max(-1.0, sd0 - 0.02), sd_hi=min(1.0, sd0 + 0.02),
+               ap_lo=0.0, ap_hi=0.0, porb_lo=86400.0, porb_hi=86400.0, t_ref=g.t_ref)
+    ctx = H.gpu_context(wl)
+    ms = []
+    for n in (300, 30000):
+        otl = fo.bank_draw(box, 5, 0, n)
+        op, _, _, otie = fo.eval_templates(o, otl, g.t_ref)
+        j = int(np.lexsort((np.arange(n), -op))[0])
+        m_oracle = float(fo.mismatch(s_sig, op[j], mu_G))
+        best, _ = ctx.eval_bank(box, 5, 0, n, "power", wl.rho_th)
+        m_gpu = (s_sig - best["power"]) / (s_sig - mu_G)
+        if not otie[j]:
+            assert int(best["idx"]) == j and abs(m_gpu - m_oracle) < 1e-12
+        assert 0.0 <= m_gpu < 1.0
+        ms.append(m_gpu)
+    assert ms[1] <= ms[0]
+    ctx.close()

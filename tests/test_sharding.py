@@ -104,3 +104,24 @@ def test_merge_orders_by_value_then_index_and_pads():
     assert m["idx"].tolist() == [[5, 7, 3]]           # ties in value broken by ascending index
     m5 = S.merge_candidates([a, b], 5)
     assert m5["idx"][0, 4] == S.PAD and m5["idx"][0, :4].tolist() == [5, 7, 3, 9]
+
+
+def test_bench_starts_its_own_ranks():
+    """`bench.py --gpus 2` without a launcher re-executes itself under torch.distributed.run (two ranks on
+    127.0.0.1); here with the CPU reference arm so that no GPU is needed: rank 0 prints the one JSON line."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "1",
+                        "--steps", "1", "--warmup", "0", "--cpu-seconds", "0.2"], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    out = json.loads(lines[0])
+    assert out["impl"] == "reference" and out["n_gpus"] == 2 and out["value"] > 0
+    import bench
+    cmd = bench.launcher_command(4, ["--gpus", "4", "--steps", "2"], 29999)
+    assert cmd[1:6] == ["-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=4", "--master-addr"]
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "2"] and "127.0.0.1" in cmd
