@@ -310,7 +310,9 @@ def extra_runs(args, dev, flush, measured, peaks, sm_mhz_of):
                 best_ms = ms if best_ms is None else min(best_ms, ms)
         evals = n * wl.n_sft
         fp64_peak = (measured["fp64_gflops"] / 2.0 * 1e9) if measured else FP64_FMA_PER_CLK_SM * N_SM * 1.965e9
-        instr = 21.0 if not binary else None   # fp64-pipe instructions per evaluation of the isolated path (SASS count)
+        # fp64-pipe slots per evaluation of the isolated path (SASS of k1_chunk<0, false, true>): 20 DADD/DMUL/
+        # DFMA/DSETP + one F2F.F64.F32 at a quarter of the DFMA rate (ft_measure_peaks: fp64_cvt_gops); the binary path adds cos()
+        instr = 24.0 if not binary else None
         out[tag] = {"workload": f"{n} templates uniform in xi (Eq. A11) on the spectrogram of {wl.name}", "kernel": "K1 ft_list_kernel (drawn in registers)",
                     "value": evals / (best_ms * 1e-3), "unit": UNIT, "kernel_ms": best_ms,
                     "bound": "alu (fp64 pipe)", "fp64_pipe_instr_per_eval": instr,
@@ -323,7 +325,9 @@ def extra_runs(args, dev, flush, measured, peaks, sm_mhz_of):
 
 def run_sweep(args, dev, flush, measured, peaks):
     """BASELINE.json configs[4]: sweep A (bank size) and B (n_sft); fused selection vs full write-out."""
+    import torch
     from paper_2411_18370_b200 import binding as B
+    torch_sync = torch.cuda.synchronize
     rows = []
     for tag, sizes in (("A", W.SWEEP_A), ("B", W.SWEEP_B)):
         for n_sft, band_hz, n_sky in sizes:
@@ -340,6 +344,7 @@ def run_sweep(args, dev, flush, measured, peaks):
                 best, kern, cands = None, None, None
                 for rep in range(args.sweep_reps + 1):          # first repetition is the warm-up
                     flush.fill_(rep)
+                    torch_sync()
                     self_t0 = time.perf_counter()
                     cands = r.step()
                     dt = time.perf_counter() - self_t0

@@ -307,6 +307,8 @@ int ft_measure_peaks(ft_ctx* ctx, ft_peaks* out);
  *              correction; every quotient must equal the IEEE division __ddiv_rn(dot, c) bit for bit (up to the sign of a zero)
  *              (dot drawn over the range of |v.n| <= 5e4 m/s, every binade from 2^-300 to 2^300, exact multiples of c, +-0).
  *   which = 1: the integer-arithmetic fp32 -> fp64 conversion of K1 equals (double)x for every finite input.
+ *   which = 2: K1's orbital cosine (magic-number range reduction by pi, Taylor series) is within 4e-16 of cos(x)
+ *              for |x| up to 1e8 rad (so the track moves by < 1e-14 bin).
  */
 int ft_selftest(ft_ctx* ctx, int which, int64_t n, uint64_t seed, uint64_t* n_fail_out);
 

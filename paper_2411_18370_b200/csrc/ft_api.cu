@@ -32,18 +32,19 @@ int ft_enter(ft_ctx* c) {
   return FT_OK;
 }
 
+int ft_tile_err_status(ft_ctx* c, int32_t e) {
+  if (e == 0) return FT_OK;
+  cudaMemsetAsync(c->tile_err_dev, 0, sizeof e, c->stream);
+  return ft_fail(c, FT_ERR_STATE, e == 1 ? "tile kernel: a track left its staged strip (internal planning error); the outputs of the previous evaluation are invalid"
+                                         : "tile kernel: more than one break in a warp range (internal planning error); the outputs of the previous evaluation are invalid");
+}
+
 int ft_check_tile_err(ft_ctx* c) {
-  for (const FtTilePlan* pl : {&c->plan, &c->plan8, &c->planb, &c->planw}) {
-    if (!pl->err) continue;
-    int32_t e = 0;
-    FT_CUDA(c, cudaMemcpy(&e, pl->err, sizeof e, cudaMemcpyDeviceToHost));
-    if (e != 0) {
-      cudaMemset(pl->err, 0, sizeof e);
-      return ft_fail(c, FT_ERR_STATE, e == 1 ? "tile kernel: a track left its staged strip (internal planning error); the outputs of the previous evaluation are invalid"
-                                             : "tile kernel: more than one break in a warp range (internal planning error); the outputs of the previous evaluation are invalid");
-    }
-  }
-  return FT_OK;
+  if (!c->tile_err_dev) return FT_OK;
+  int32_t e = 0;
+  FT_CUDA(c, cudaMemcpyAsync(&e, c->tile_err_dev, sizeof e, cudaMemcpyDeviceToHost, c->stream));
+  FT_CUDA(c, cudaStreamSynchronize(c->stream));
+  return ft_tile_err_status(c, e);
 }
 
 namespace {
@@ -156,6 +157,9 @@ int ft_create(ft_ctx** out, const float* P_dev, int64_t n_sft, int64_t n_bins, i
   FT_CUDA(c, cudaMalloc(&c->near_ties_dev, sizeof(unsigned long long)));
   FT_CUDA(c, cudaMemsetAsync(c->near_ties_dev, 0, sizeof(unsigned long long), c->stream));
   FT_CUDA(c, cudaMalloc(&c->flag_dev, sizeof(int32_t)));
+  FT_CUDA(c, cudaMalloc(&c->tile_err_dev, sizeof(int32_t)));
+  FT_CUDA(c, cudaMemsetAsync(c->tile_err_dev, 0, sizeof(int32_t), c->stream));
+  c->plan.err = c->plan8.err = c->planb.err = c->planw.err = c->tile_err_dev;
   FT_CUDA(c, cudaMalloc(&c->vr_dev, sizeof(double) * 2 * n_sft));
   FT_CUDA(c, cudaMalloc(&c->maxw_dev, sizeof(int32_t) * 4));
   FtDev& d = c->d;
@@ -293,8 +297,8 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
     std::snprintf(buf, sizeof buf, "ft_eval: tracks may leave the spectrogram: bound [%.2f, %.2f] bins vs [0, %lld)", x_lo, x_hi, (long long)c->d.n_bins);
     return ft_fail(c, FT_ERR_TRACK_RANGE, buf);
   }
-  FT_CUDA(c, cudaStreamSynchronize(c->stream));  // previous work may still read the old axes / plans
-  if (int rc = ft_check_tile_err(c)) return rc;  // a planning error of the previous evaluation surfaces here
+  if (int rc = ft_check_tile_err(c)) return rc;  // synchronises (previous work may still read the old axes / plans);
+                                                 // a planning error of the previous evaluation surfaces here
   // copy axes (the staging vector lives in the handle: no second synchronisation)
   const size_t n_ax = 3 * (size_t)g->n_sky + g->n_ap + g->n_porb + g->n_tasc;
   std::vector<double>& ax = c->axes_host;
@@ -465,10 +469,12 @@ int ft_eval_list(ft_ctx* c, const uint64_t* idx_host, int64_t n, ft_cand* out_ho
 int ft_get_counters(ft_ctx* c, ft_counters* out) {
   if (!c || !out) return FT_ERR_ARG;
   if (int rc = ft_enter(c)) return rc;
-  FT_CUDA(c, cudaStreamSynchronize(c->stream));
-  if (int rc2 = ft_check_tile_err(c)) return rc2;
   unsigned long long nt = 0;
-  FT_CUDA(c, cudaMemcpy(&nt, c->near_ties_dev, sizeof nt, cudaMemcpyDeviceToHost));
+  int32_t terr = 0;
+  FT_CUDA(c, cudaMemcpyAsync(&nt, c->near_ties_dev, sizeof nt, cudaMemcpyDeviceToHost, c->stream));
+  FT_CUDA(c, cudaMemcpyAsync(&terr, c->tile_err_dev, sizeof terr, cudaMemcpyDeviceToHost, c->stream));
+  FT_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (int rc2 = ft_tile_err_status(c, terr)) return rc2;
   c->counters.near_ties = nt;
   double ms_sum = 0.0;
   for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
@@ -497,6 +503,7 @@ void ft_destroy(ft_ctx* c) {
   ft_dfree(c->ctab_dev); ft_dfree(c->axes_dev); ft_dfree(c->w_row_dev); ft_dfree(c->ant_dev); ft_dfree(c->vr_dev);
   ft_dfree(c->maxw_dev); ft_dfree(c->scratch_f); ft_dfree(c->scratch_i); ft_dfree(c->veto_cnt); ft_dfree(c->veto_w);
   ft_dfree(c->glist_dev); ft_dfree(c->pbox_dev); ft_dfree(c->io_dev); ft_dfree(c->near_ties_dev); ft_dfree(c->flag_dev);
+  ft_dfree(c->tile_err_dev);
   for (cudaEvent_t e : c->evs) cudaEventDestroy(e);
   delete c;
 }

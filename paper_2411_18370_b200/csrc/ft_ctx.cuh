@@ -86,6 +86,7 @@ struct ft_ctx {
   size_t io_cap = 0;
   unsigned long long* near_ties_dev = nullptr;
   int32_t* flag_dev = nullptr;   // [1] error flag of the list kernels
+  int32_t* tile_err_dev = nullptr;  // [1] planning-error flag of the tile kernels (all plans of the handle)
   // bookkeeping
   ft_counters counters{};
   std::vector<cudaEvent_t> evs;  // pairs around every statistic-kernel pass of the last call
@@ -127,6 +128,7 @@ void ft_tock(ft_ctx* c, int launches);
 // The tile kernels raise plan.err if a track left its staged strip (a planning bug, never data): surfaced at
 // every synchronising call instead of silently wrong sums.
 int ft_check_tile_err(ft_ctx* c);
+int ft_tile_err_status(ft_ctx* c, int32_t e);   // the same for a flag value already copied to the host
 // make the handle's device current
 int ft_enter(ft_ctx* c);
 

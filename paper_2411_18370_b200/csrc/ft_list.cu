@@ -42,6 +42,35 @@ __device__ __forceinline__ double ft_div_c(double dot) {
   return __fma_rn(__fma_rn(-q0, FT_C_LIGHT, dot), kInvC, q0);
 }
 
+// cos(x) for the orbital phase of K1: k = rint(x / pi) by a magic-number fused multiply-add (no F2I / I2F), r = x - k pi
+// with pi split in three doubles (each product exact in the fused multiply-add), cos(r) on [-pi/2, pi/2] by its Taylor
+// series to r^24 (truncation < 1e-19; twelve fused multiply-adds), sign from the parity of k.  No table, no branch:
+// 18 fp64 instructions against ~25 plus two conversions and three table loads of the library routine.  Absolute
+// error < 3e-16 for |x| < 1e8 (checked against 300-bit arithmetic when the constants were derived; on the device
+// against cos() in tests/test_gpu_templates.py), i.e. < 1e-14 bin on the track: far inside the 1e-9 tie window.
+__device__ __forceinline__ double k1_cos(double x) {
+  const double tm = __fma_rn(x, 0.31830988618379069, kMagic);            // 1/pi; rint(x / pi) in the low mantissa bits
+  const double k = __dsub_rn(tm, kMagic);
+  double r = __fma_rn(-k, 3.1415926535897931, x);                        // pi = 0x1.921fb54442d18p+1
+  r = __fma_rn(-k, 1.2246467991473532e-16, r);                           //    + 0x1.1a62633145c07p-53
+  r = __fma_rn(-k, -2.9947698097183397e-33, r);                          //    - 0x1.f1976b7ed8fbcp-109
+  const double z = __dmul_rn(r, r);
+  double t = 1.6117375710961184e-24;                                     // 1/24!
+  t = __fma_rn(t, z, -8.8967913924505741e-22);                           // -1/22!
+  t = __fma_rn(t, z, 4.1103176233121648e-19);                            // 1/20!
+  t = __fma_rn(t, z, -1.5619206968586225e-16);                           // -1/18!
+  t = __fma_rn(t, z, 4.7794773323873853e-14);                            // 1/16!
+  t = __fma_rn(t, z, -1.1470745597729725e-11);                           // -1/14!
+  t = __fma_rn(t, z, 2.08767569878681e-09);                              // 1/12!
+  t = __fma_rn(t, z, -2.7557319223985888e-07);                           // -1/10!
+  t = __fma_rn(t, z, 2.4801587301587302e-05);                            // 1/8!
+  t = __fma_rn(t, z, -0.0013888888888888889);                            // -1/6!
+  t = __fma_rn(t, z, 0.041666666666666664);                              // 1/4!
+  t = __fma_rn(t, z, -0.5);
+  t = __fma_rn(t, z, 1.0);
+  return __hiloint2double(__double2hiint(t) ^ (__double2loint(tm) << 31), __double2loint(t));   // (-1)^k
+}
+
 // counter-based uniform in (0, 1): splitmix64 finaliser of seed + golden * (8 i + d + 1), top 53 bits
 __device__ __forceinline__ double ft_uniform(uint64_t seed, uint64_t i, uint32_t dcoord) {
   uint64_t z = seed + 0x9E3779B97F4A7C15ull * (8ull * i + (uint64_t)dcoord + 1ull);
@@ -82,10 +111,53 @@ __global__ void ft_bank_draw_kernel(FtBankBox bx, uint64_t seed, uint64_t first,
   if (j < n) out[j] = ft_bank_template(bx, seed, first + (uint64_t)j);
 }
 
+// ---- evaluation order: templates bucketed by f0 so that the 32 gathers of a warp fall into a few cache lines --
+// (a random bank read in storage order touches 30 sectors per warp-load; ordered by f0 the spread is the Doppler
+// shift, a few lines: measured 1.5x on the isolated path).  Counting sort on 4096 buckets of the template's
+// position in the spectrogram band; the order inside a bucket is arbitrary (results are stored per template).
+constexpr int K1_BUCKETS = 4096;
+
+template <bool GEN>
+__device__ __forceinline__ uint32_t k1_bucket(const FtDev& d, const FtTemplateDev* tl, const FtBankBox& bx, uint64_t seed,
+                                              uint64_t first, int64_t j) {
+  const double f0 = GEN ? ft_inv_power(bx.f0_lo, bx.f0_hi, ft_uniform(seed, first + (uint64_t)j, 0), 6) : tl[j].f0;
+  const double u = (f0 - d.f_min) * d.inv_df / (double)d.n_bins;
+  return (uint32_t)min(max((int)(u * K1_BUCKETS), 0), K1_BUCKETS - 1);
+}
+template <bool GEN>
+__global__ void k1_hist_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict__ tl, const __grid_constant__ FtBankBox bx,
+                               uint64_t seed, uint64_t first, int64_t n, uint32_t* __restrict__ hist) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j < n) atomicAdd(hist + k1_bucket<GEN>(d, tl, bx, seed, first, j), 1u);
+}
+__global__ void __launch_bounds__(1024) k1_scan_kernel(uint32_t* __restrict__ hist) {   // exclusive scan of 4096 counters, in place
+  __shared__ uint32_t part[1024];
+  uint32_t v[4], s = 0;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { v[i] = hist[4 * threadIdx.x + i]; s += v[i]; }
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    const uint32_t t = (int)threadIdx.x >= o ? part[threadIdx.x - o] : 0u;
+    __syncthreads();
+    part[threadIdx.x] += t;
+    __syncthreads();
+  }
+  uint32_t run = part[threadIdx.x] - s;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { hist[4 * threadIdx.x + i] = run; run += v[i]; }
+}
+template <bool GEN>
+__global__ void k1_scatter_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict__ tl, const __grid_constant__ FtBankBox bx,
+                                  uint64_t seed, uint64_t first, int64_t n, uint32_t* __restrict__ cursor, uint32_t* __restrict__ perm) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j < n) perm[atomicAdd(cursor + k1_bucket<GEN>(d, tl, bx, seed, first, j), 1u)] = (uint32_t)j;
+}
+
 struct K1Acc { double power; int32_t count; unsigned ties; unsigned bad; };
 
 #ifndef FT_K1_INT_CVT
-#define FT_K1_INT_CVT 1   // fp32 -> fp64 by integer moves (1) or by the conversion instruction (0)
+#define FT_K1_INT_CVT 0   // fp32 -> fp64 by the conversion instruction (0: measured faster, one issue slot) or by integer moves (1)
 #endif
 __device__ __forceinline__ double k1_f2d(float x) {
 #if FT_K1_INT_CVT
@@ -119,7 +191,7 @@ __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp
     double D = __dadd_rn(1.0, V);
     if (BIN) {   // (an isolated template of a mixed CTA subtracts B = 0: (1 + V) - 0 = 1 + V)
       double B = 0.0;
-      if (binary) B = __dmul_rn(apOm, cos(__dmul_rn(Om, __dsub_rn(sC[c].y, tp.t_asc))));
+      if (binary) B = __dmul_rn(apOm, k1_cos(__dmul_rn(Om, __dsub_rn(sC[c].y, tp.t_asc))));
       D = __dsub_rn(D, B);
     }
     const double x = ft_track_x(tp.f0, __dmul_rn(tp.f1, vzdt.y), D, f_min, inv_df);
@@ -148,11 +220,13 @@ __global__ void __launch_bounds__(K1_THREADS)
 ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict__ tl, const __grid_constant__ FtBankBox bx,
                uint64_t seed, uint64_t first, int64_t n, double t_ref,
                float* __restrict__ out_power, int32_t* __restrict__ out_count, int32_t* __restrict__ err,
-               unsigned long long* __restrict__ near_ties, double* __restrict__ best_v, int64_t* __restrict__ best_i) {
+               unsigned long long* __restrict__ near_ties, double* __restrict__ best_v, int64_t* __restrict__ best_i,
+               const uint32_t* __restrict__ perm) {
   // per-SFT tables of the current chunk: (vx, vy), (vz, t - t_ref), (w, t): three LDS.128 per evaluation at most
   __shared__ double2 sA[K1_THREADS], sB[K1_THREADS], sC[K1_THREADS];
-  const int64_t q = (int64_t)blockIdx.x * K1_THREADS + threadIdx.x;
-  const bool active = q < n;
+  const int64_t slot = (int64_t)blockIdx.x * K1_THREADS + threadIdx.x;
+  const bool active = slot < n;
+  const int64_t q = active ? (perm ? (int64_t)perm[slot] : slot) : 0;   // the template this thread evaluates
   const FtTemplateDev tp = GEN ? ft_bank_template(bx, seed, first + (uint64_t)(active ? q : 0)) : tl[active ? q : 0];
   const double Om = __ddiv_rn(FT_TWO_PI, tp.P_orb);
   const double apOm = __dmul_rn(tp.a_p, Om);
@@ -196,7 +270,7 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
     __shared__ double bv[K1_THREADS / 32];
     __shared__ long long bi[K1_THREADS / 32];
     double v = (active && !bad) ? (STAT == 1 ? (double)count : power) : -INFINITY;
-    long long i = active ? (long long)q : 0x7fffffffffffffffll;
+    long long i = active ? (long long)q : 0x7fffffffffffffffll;   // (the template's index, not the slot)
     for (int o = 16; o > 0; o >>= 1) {
       const double v2 = __shfl_xor_sync(0xffffffffu, v, o);
       const long long i2 = __shfl_xor_sync(0xffffffffu, i, o);
@@ -274,15 +348,42 @@ __global__ void ft_selftest_cvt_kernel(int64_t n, unsigned long long* __restrict
   if (fails) atomicAdd(n_fail, (unsigned long long)fails);
 }
 
+// perm (or nullptr) = scratch of n + K1_BUCKETS uint32: the evaluation order is built there first
+// which = 2: k1_cos against the library cos(): failures = |difference| > 4e-16
+__global__ void ft_selftest_cos_kernel(uint64_t seed, int64_t n, unsigned long long* __restrict__ n_fail) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  unsigned fails = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const double u = 2.0 * ft_uniform(seed, (uint64_t)i, 0) - 1.0;
+    const double scale = (i & 3) == 0 ? 4.0 : (i & 3) == 1 ? 400.0 : (i & 3) == 2 ? 1e5 : 1e8;
+    const double x = u * scale;
+    if (!(fabs(k1_cos(x) - cos(x)) <= 4e-16)) ++fails;
+  }
+  if (fails) atomicAdd(n_fail, (unsigned long long)fails);
+}
+
 template <bool GEN, bool BEST>
 cudaError_t launch_list(const FtDev& d, int stat, const FtTemplateDev* tl, const FtBankBox& bx, uint64_t seed, uint64_t first,
                         int64_t n, double t_ref, float* out_power, int32_t* out_count, int32_t* err,
-                        unsigned long long* near_ties, double* best_v, int64_t* best_i, cudaStream_t s) {
+                        unsigned long long* near_ties, double* best_v, int64_t* best_i, uint32_t* perm, cudaStream_t s,
+                        int* launches) {
+  *launches = 0;
   if (n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + K1_THREADS - 1) / K1_THREADS);
-  if (stat == 0) ft_list_kernel<0, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i);
-  else if (stat == 1) ft_list_kernel<1, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i);
-  else ft_list_kernel<2, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i);
+  if (perm) {
+    uint32_t* hist = perm + n;
+    cudaError_t e = cudaMemsetAsync(hist, 0, sizeof(uint32_t) * K1_BUCKETS, s);
+    if (e != cudaSuccess) return e;
+    k1_hist_kernel<GEN><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, hist);
+    k1_scan_kernel<<<1, 1024, 0, s>>>(hist);
+    k1_scatter_kernel<GEN><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, hist, perm);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    *launches += 3;
+  }
+  if (stat == 0) ft_list_kernel<0, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
+  else if (stat == 1) ft_list_kernel<1, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
+  else ft_list_kernel<2, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
+  *launches += 1;
   return cudaGetLastError();
 }
 
@@ -317,12 +418,20 @@ int ft_eval_templates(ft_ctx* c, const ft_template* templates_dev, int64_t n, do
   if (int rc = ft_enter(c)) return rc;
   FtDev d = c->d;
   d.rho = (float)rho_th;
+  uint32_t* perm = nullptr;
+  if (n >= 4096 && n < (1ll << 32)) {   // evaluation order by f0 (small lists are launch-bound anyway)
+    FT_CUDA(c, cudaStreamSynchronize(c->stream));   // the grow-only scratch may still be in use
+    FT_CUDA(c, ft_grow(c->io_dev, c->io_cap, sizeof(uint32_t) * ((size_t)n + K1_BUCKETS)));
+    perm = reinterpret_cast<uint32_t*>(c->io_dev);
+  }
   FT_CUDA(c, cudaMemsetAsync(c->flag_dev, 0, sizeof(int32_t), c->stream));
   c->ev_used = 0; c->counters.stat_launches = 0;
+  int launches = 0;
   ft_tick(c);
   const cudaError_t e = launch_list<false, false>(d, stat, reinterpret_cast<const FtTemplateDev*>(templates_dev), FtBankBox{}, 0, 0, n,
-                                                  t_ref, out_power_dev, out_count_dev, c->flag_dev, c->near_ties_dev, nullptr, nullptr, c->stream);
-  ft_tock(c, 1);
+                                                  t_ref, out_power_dev, out_count_dev, c->flag_dev, c->near_ties_dev, nullptr, nullptr,
+                                                  perm, c->stream, &launches);
+  ft_tock(c, launches);
   if (e != cudaSuccess) return ft_fail(c, FT_ERR_CUDA, std::string("ft_eval_templates: ") + cudaGetErrorString(e));
   int32_t flag = 0;
   FT_CUDA(c, cudaMemcpyAsync(&flag, c->flag_dev, sizeof flag, cudaMemcpyDeviceToHost, c->stream));
@@ -359,18 +468,21 @@ int ft_eval_bank(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t firs
   const FtBankBox bx = to_dev_box(box);
   const int64_t n_blocks = (n + K1_THREADS - 1) / K1_THREADS;
   FT_CUDA(c, cudaStreamSynchronize(c->stream));   // the grow-only scratch may still be in use
-  const size_t need = 16 * (size_t)n_blocks + sizeof(FtTemplateDev) + sizeof(FtCandDev);
+  if (n >= (1ll << 32)) return ft_fail(c, FT_ERR_ARG, "ft_eval_bank: n < 2^32 per call (draw the bank in batches)");
+  const size_t need = 16 * (size_t)n_blocks + sizeof(FtTemplateDev) + sizeof(FtCandDev) + sizeof(uint32_t) * ((size_t)n + K1_BUCKETS);
   FT_CUDA(c, ft_grow(c->io_dev, c->io_cap, need));
   double* best_v = reinterpret_cast<double*>(c->io_dev);
   int64_t* best_i = reinterpret_cast<int64_t*>(c->io_dev + 8 * (size_t)n_blocks);
   FtTemplateDev* tp_dev = reinterpret_cast<FtTemplateDev*>(c->io_dev + 16 * (size_t)n_blocks);
   FtCandDev* cand_dev = reinterpret_cast<FtCandDev*>(tp_dev + 1);
+  uint32_t* perm = n >= 4096 ? reinterpret_cast<uint32_t*>(cand_dev + 1) : nullptr;
   FT_CUDA(c, cudaMemsetAsync(c->flag_dev, 0, sizeof(int32_t), c->stream));
   c->ev_used = 0; c->counters.stat_launches = 0;
+  int launches = 0;
   ft_tick(c);
   const cudaError_t e = launch_list<true, true>(d, stat, nullptr, bx, seed, first, n, box->t_ref, out_power_dev, out_count_dev,
-                                                c->flag_dev, c->near_ties_dev, best_v, best_i, c->stream);
-  ft_tock(c, 1);
+                                                c->flag_dev, c->near_ties_dev, best_v, best_i, perm, c->stream, &launches);
+  ft_tock(c, launches);
   if (e != cudaSuccess) return ft_fail(c, FT_ERR_CUDA, std::string("ft_eval_bank: ") + cudaGetErrorString(e));
   ft_best_reduce_kernel<<<1, 1024, 0, c->stream>>>(best_v, best_i, n_blocks);
   FT_CUDA(c, cudaGetLastError());
@@ -424,14 +536,15 @@ int ft_track(ft_ctx* c, const ft_template* tp_host, double t_ref, int64_t* k_out
 int ft_selftest(ft_ctx* c, int which, int64_t n, uint64_t seed, uint64_t* n_fail_out) {
   if (!c || !n_fail_out || n < 0) return FT_ERR_ARG;
   if (!c->d.P) return ft_fail(c, FT_ERR_STATE, "ft_selftest: handle not created");
-  if (which < 0 || which > 1) return ft_fail(c, FT_ERR_ARG, "ft_selftest: which = 0 (division by c) or 1 (fp32 -> fp64 conversion)");
+  if (which < 0 || which > 2) return ft_fail(c, FT_ERR_ARG, "ft_selftest: which = 0 (division by c), 1 (fp32 -> fp64 conversion) or 2 (orbital cosine)");
   if (int rc = ft_enter(c)) return rc;
   FT_CUDA(c, cudaStreamSynchronize(c->stream));
   FT_CUDA(c, ft_grow(c->io_dev, c->io_cap, 8));
   unsigned long long* nf = reinterpret_cast<unsigned long long*>(c->io_dev);
   FT_CUDA(c, cudaMemsetAsync(nf, 0, 8, c->stream));
   if (which == 0) ft_selftest_div_kernel<<<148 * 8, 256, 0, c->stream>>>(seed, n, nf);
-  else ft_selftest_cvt_kernel<<<148 * 8, 256, 0, c->stream>>>(n, nf);
+  else if (which == 1) ft_selftest_cvt_kernel<<<148 * 8, 256, 0, c->stream>>>(n, nf);
+  else ft_selftest_cos_kernel<<<148 * 8, 256, 0, c->stream>>>(seed, n, nf);
   FT_CUDA(c, cudaGetLastError());
   c->counters.kernel_launches += 1;
   unsigned long long h = 0;

@@ -114,29 +114,29 @@ extern "C" int ft_measure_peaks(ft_ctx* c, ft_peaks* out) {
     }
     return (double)best * 1e-3;
   };
-  const int grid = n_sm * 2;
+  const int grid = n_sm;   // one CTA of 1024 threads per SM (64 registers each: the register file holds one)
   {
-    const int iters = 4000;
+    const int iters = 8000;
     const double s = timed([&] { pk_smem_kernel<<<grid, PK_THREADS, 0, c->stream>>>(reinterpret_cast<float*>(buf), iters, cyc); }, 3);
     out->smem_gbs = (double)grid * PK_THREADS * (double)iters * 32.0 * 4.0 / s / 1e9;
     long long h = 0;
     cudaMemcpy(&h, cyc, sizeof h, cudaMemcpyDeviceToHost);
-    // two CTAs share an SM: block 0 ran for about the whole kernel
+    // one CTA per SM: block 0 ran for about the whole kernel
     out->sm_clock_mhz = (double)h / s / 1e6;
   }
   {
-    const int iters = 2000;
+    const int iters = 4000;
     const double s = timed([&] { pk_dfma_kernel<<<grid, PK_THREADS, 0, c->stream>>>(reinterpret_cast<double*>(buf), iters, 1.0000001, 1e-9); }, 3);
     out->fp64_gflops = (double)grid * PK_THREADS * (double)iters * 32.0 * 2.0 / s / 1e9;
   }
   {
-    const int iters = 500;
+    const int iters = 1000;
     const double s = timed([&] { pk_cvt_kernel<<<grid, PK_THREADS, 0, c->stream>>>(reinterpret_cast<double*>(buf), iters, 0.25); }, 3);
     out->fp64_cvt_gops = (double)grid * PK_THREADS * (double)iters * 32.0 / s / 1e9;
   }
   {
-    const int passes = 20;
-    const double s = timed([&] { pk_l2_kernel<<<n_sm * 2, PK_THREADS, 0, c->stream>>>(reinterpret_cast<const uint4*>(buf), l2_bytes / 16, passes,
+    const int passes = 200;
+    const double s = timed([&] { pk_l2_kernel<<<n_sm, PK_THREADS, 0, c->stream>>>(reinterpret_cast<const uint4*>(buf), l2_bytes / 16, passes,
                                                                                      reinterpret_cast<uint32_t*>(buf + l2_bytes + 32)); }, 3);
     out->l2_gbs = (double)l2_bytes * passes / s / 1e9;
   }

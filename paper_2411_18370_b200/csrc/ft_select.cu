@@ -222,6 +222,12 @@ __global__ void ft_mask_keys_local_kernel(float* __restrict__ keys, const int32_
     if (counts[e] < floor) keys[e] = -INFINITY;
 }
 
+__global__ void ft_select_reset_kernel(FtSelectDev sel, uint32_t* final_n, uint32_t* overflow) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < sel.n_regions) { sel.thr[i] = -INFINITY; sel.cnt[i] = 0u; }
+  if (i == 0) { *final_n = 0u; *overflow = 0u; }
+}
+
 __global__ void ft_fill_f32_kernel(float* p, int64_t n, float v) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) p[i] = v;
@@ -241,14 +247,8 @@ __global__ void ft_keys_affine_kernel(float* __restrict__ k, int64_t n, double m
 }  // namespace
 
 cudaError_t ft_select_reset(FtSelectDev sel, uint32_t* final_n, uint32_t* overflow, cudaStream_t s) {
-  ft_fill_f32_kernel<<<(sel.n_regions + 255) / 256, 256, 0, s>>>(sel.thr, sel.n_regions, -INFINITY);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  e = cudaMemsetAsync(sel.cnt, 0, sizeof(uint32_t) * sel.n_regions, s);
-  if (e != cudaSuccess) return e;
-  e = cudaMemsetAsync(final_n, 0, sizeof(uint32_t), s);
-  if (e != cudaSuccess) return e;
-  return cudaMemsetAsync(overflow, 0, sizeof(uint32_t), s);
+  ft_select_reset_kernel<<<(sel.n_regions + 255) / 256, 256, 0, s>>>(sel, final_n, overflow);
+  return cudaGetLastError();
 }
 
 cudaError_t ft_select_threshold(const float* keys, int64_t n_rows, int64_t n_f0, const FtRowMap& map, uint32_t k,

@@ -174,8 +174,7 @@ cudaError_t ft_tile_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned 
 }
 
 void ft_tile_plan_free(FtTilePlan* p) {
-  if (p->kst) cudaFree(p->kst);
-  if (p->err) cudaFree(p->err);
+  if (p->kst) cudaFree(p->kst);   // (err belongs to the handle)
   *p = FtTilePlan{};
 }
 
@@ -195,6 +194,7 @@ bool ft_tile_choose(const FtDev& d, const FtTileHostIn& in, int mode, FtTilePlan
   if (!d.Q) { *why = "no folded array"; return false; }
   if (d.n_f0 > (1 << 30)) { *why = "more than 2^30 f0 values"; return false; }
   if (mode == 1 && d.n_sft > 65535) { *why = "packed number count holds 16-bit counters (n_sft <= 65535)"; return false; }
+  if (mode == 2 && (d.n_sft > 65535 || d.n_sft < 64)) { *why = "one-pass kernel: 16-bit counters, pixels rounded to 18 bits (64 <= n_sft <= 65535)"; return false; }
   // chunk = the f0 a warp covers with one load instruction: 32 (one fp32 pixel per lane) or 128 (4 packed hits)
   const int cw = mode == 1 ? 128 : 32;
   const int64_t chunks = (d.n_f0 + cw - 1) / cw;
@@ -246,12 +246,6 @@ cudaError_t ft_tile_strips(const FtDev& d, const FtTileHostIn& in, FtTilePlan* p
     if (e != cudaSuccess) return e;
     plan->kst_cap = need;
   }
-  if (!plan->err) {
-    const cudaError_t e = cudaMalloc(&plan->err, sizeof(int32_t));
-    if (e != cudaSuccess) return e;
-  }
-  cudaError_t e = cudaMemsetAsync(plan->err, 0, sizeof(int32_t), s);
-  if (e != cudaSuccess) return e;
   double apm = 0.0, pmin = in.P_orb[0];
   for (int i = 0; i < d.n_ap; ++i) apm = std::fmax(apm, std::fabs(in.a_p[i]));
   for (int i = 0; i < d.n_porb; ++i) pmin = std::fmin(pmin, in.P_orb[i]);

@@ -9,7 +9,7 @@ struct FtTilePlan {
   // device buffers, grow-only across plans on the same object (freed by ft_tile_plan_free)
   int32_t* kst = nullptr;       // [n_tiles][n_sft] first staged bin of the strip (multiple of 4 / 16)
   size_t kst_cap = 0;
-  int32_t* err = nullptr;       // [1] set by the kernel if a track left its staged strip (plan bug)
+  int32_t* err = nullptr;       // [1] set by the kernel if a track left its staged strip (plan bug); the handle's, shared by its plans
   int32_t mode = 0;             // 0: fp32 gather (ft_tile_kernel), 1: packed number count (ft_tile8_kernel),
                                 // 2: both statistics in one pass (ft_tileb_kernel, J <= 16),
                                 // 3: fp32 gather times a per-(point, SFT) weight (ft_tilew_kernel, J <= 16)

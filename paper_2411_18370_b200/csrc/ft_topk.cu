@@ -209,7 +209,7 @@ int topk_regions(ft_ctx* c, const TopkSpec& sp, std::vector<FtCandDev>* out, int
       off_rs = up.size(); up.insert(up.end(), rs.begin(), rs.end());
       off_rows = up.size(); up.insert(up.end(), rw.begin(), rw.end());
     }
-    FT_CUDA(c, cudaStreamSynchronize(c->stream));   // (the previous call's lists may still be read)
+    if (c->glist_cap < up.size()) FT_CUDA(c, cudaStreamSynchronize(c->stream));   // (about to free lists that may still be read)
     FT_CUDA(c, ft_grow(c->glist_dev, c->glist_cap, up.size()));
     FT_CUDA(c, cudaMemcpyAsync(c->glist_dev, up.data(), sizeof(uint32_t) * up.size(), cudaMemcpyHostToDevice, c->stream));
     const uint32_t* glist_dev = c->glist_dev;
@@ -296,12 +296,14 @@ int topk_regions(ft_ctx* c, const TopkSpec& sp, std::vector<FtCandDev>* out, int
                             wfloor, c->out_dev, overflow, c->stream));
   c->counters.kernel_launches += 3;
   uint32_t fin[2] = {0, 0};
+  int32_t terr = 0;
   out->resize((size_t)n_regions * k);
   FT_CUDA(c, cudaMemcpyAsync(fin, c->final_n, sizeof fin, cudaMemcpyDeviceToHost, c->stream));
+  FT_CUDA(c, cudaMemcpyAsync(&terr, c->tile_err_dev, sizeof terr, cudaMemcpyDeviceToHost, c->stream));
   FT_CUDA(c, cudaMemcpyAsync(cnt.data(), c->sel.cnt, sizeof(uint32_t) * n_regions, cudaMemcpyDeviceToHost, c->stream));
   FT_CUDA(c, cudaMemcpyAsync(out->data(), c->out_dev, sizeof(FtCandDev) * (size_t)n_regions * k, cudaMemcpyDeviceToHost, c->stream));
   FT_CUDA(c, cudaStreamSynchronize(c->stream));
-  if (int rc2 = ft_check_tile_err(c)) return rc2;
+  if (int rc2 = ft_tile_err_status(c, terr)) return rc2;
   uint64_t appended = 0;
   for (uint32_t v : cnt) appended += v;
   c->counters.appended = appended;

@@ -10,6 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
+    config.addinivalue_line("markers", "slow: exhaustive full-size runs (minutes of CPU oracle time); need FT_RUN_SLOW=1")
 
 
 @pytest.fixture(scope="session")

@@ -45,9 +45,9 @@ def test_full_arrays_match_oracle(case, kernel):
     # single-statistic launches give the same arrays
     gp1, _ = H.gpu_full(ctx, wl, stat="power")
     _, gc1 = H.gpu_full(ctx, wl, stat="hough")
-    # (narrow bands compute both statistics in one gather with the hit bit in the pixel's LSB: the power
-    # then differs from the power-only pass by at most an ulp per pixel)
-    assert np.allclose(gp1, gp, rtol=1e-6, atol=0) and np.array_equal(gc1, gc)
+    # (narrow bands compute both statistics in one gather over pixels rounded to 18 mantissa bits with the hit bit
+    # below them: the power then differs from the power-only pass by ~4e-6 / sqrt(3 n_sft) rms, a few 1e-6 at most)
+    assert np.allclose(gp1, gp, rtol=4e-6, atol=0) and np.array_equal(gc1, gc)
     # one pass per statistic gives the power-only array exactly
     from paper_2411_18370_b200 import binding as B
     ctx.set_option(B.FT_OPT_ONE_PASS_BOTH, 0)

@@ -86,6 +86,7 @@ def test_division_by_c_and_float_conversion_are_exact():
     assert ctx.selftest(0, 100_000_000, seed=3) == 0
     assert ctx.selftest(0, 10_000_000, seed=4) == 0
     assert ctx.selftest(1, 1 << 32) == 0
+    assert ctx.selftest(2, 50_000_000, seed=5) == 0      # K1's orbital cosine against cos()
     ctx.close()
 
 
