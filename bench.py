@@ -40,6 +40,8 @@ UNIT = "evals/s"
 SMEM_BYTES_PER_CLK_SM = 128.0   # nominal: B300_MICROARCH "smem crossbar BW 128 B/cyc/SM" (fallback when not measured)
 FP64_FMA_PER_CLK_SM = 64.0      # nominal B200 vector fp64 (40 TFLOP/s at 148 SMs x 1.965 GHz / 2)
 N_SM = 148
+# fp64-pipe issue slots per evaluation of K1's loop body, counted in the SASS
+K1_FP64_SLOTS = {"isolated": 24.0, "binary": 43.0}
 
 
 def ncu_traffic(config: int, kernel: str):
@@ -197,6 +199,19 @@ class Runner:
         c.eval(self.wl.grid, self.stat, self.wl.rho_th)                  # bind grid (+ fold weights / threshold bit)
         return c.topk_per_band(self.wl.band_width, self.wl.k, self.n_bands)   # evaluate + fused selection; syncs
 
+    def full_arrays_step(self):
+        """The other kind of step: every statistic of the bank written out (A5), no selection."""
+        torch, wl = self.torch, self.wl
+        n = wl.grid.n_templates
+        op = torch.empty(n, dtype=torch.float32, device=self.dev) if self.stat != "hough" else None
+        oc = torch.empty(n, dtype=torch.int32, device=self.dev) if self.stat not in ("power", "whough") else None
+
+        def step(ctx=None):
+            (ctx or self.ctx).eval(wl.grid, self.stat, wl.rho_th, op, oc)
+            torch.cuda.synchronize()
+            return np.zeros(0, dtype=np.uint8)
+        return step
+
     def timed(self, steps, warmup, flush, barrier=lambda: None, step=None):
         """Device-timed steps with an L2 flush between them.  Returns (per-step ms array, statistic-kernel ms per
         step, statistic launches per step)."""
@@ -246,6 +261,41 @@ def roofline_block(evals, k_ms, n_launch, step_ms, peaks, measured, sm_mhz, traf
                        "note": "north_star gather roofline: 4 B per template·SFT evaluation over HBM/L2 bandwidth"}}
 
 
+def bank_run(args, dev, flush, wl, binary, measured):
+    """K1 on a xi-uniform random bank (Eq. A11) over the workload's parameter box, drawn and evaluated on the device
+    by one ft_eval_bank call; best of two timed repetitions after a warm-up."""
+    r = Runner(wl, dev, args)
+    g = wl.grid
+    box = dict(f0_lo=g.f0_start, f0_hi=g.f0_start + (g.n_f0 - 1) * g.df0, f1_lo=g.f1_start, f1_hi=g.f1_start + (g.n_f1 - 1) * g.df1,
+               ra_lo=0.0, ra_hi=2 * np.pi, sd_lo=-1.0, sd_hi=1.0,
+               ap_lo=float(np.min(g.a_p)) if binary else 0.0, ap_hi=float(np.max(g.a_p)) if binary else 0.0,
+               porb_lo=float(np.min(g.P_orb)), porb_hi=float(np.max(g.P_orb)), t_ref=g.t_ref)
+    if binary:
+        n0 = g.sky[0]
+        ra = float(np.arctan2(n0[1], n0[0]) % (2 * np.pi))
+        box.update(ra_lo=ra, ra_hi=ra, sd_lo=float(n0[2]), sd_hi=float(n0[2]))
+    n = args.bank
+    best_ms = None
+    for rep in range(3):
+        flush.fill_(rep)
+        r.ctx.eval_bank(box, 7, 0, n, "power", wl.rho_th)          # synchronises
+        ms = r.ctx.counters()["last_kernel_ms"]
+        if rep > 0:
+            best_ms = ms if best_ms is None else min(best_ms, ms)
+    evals = n * wl.n_sft
+    fp64_peak = (measured["fp64_gflops"] / 2.0 * 1e9) if measured else FP64_FMA_PER_CLK_SM * N_SM * 1.965e9
+    # fp64-pipe slots per evaluation (SASS of k1_chunk, DESIGN.md "K1")
+    instr = K1_FP64_SLOTS["binary" if binary else "isolated"]
+    res = {"workload": f"{n} templates uniform in xi (Eq. A11) on the spectrogram of {wl.name}", "kernel": "K1 ft_list_kernel (drawn in registers)",
+           "value": evals / (best_ms * 1e-3), "unit": UNIT, "kernel_ms": best_ms,
+           "bound": "alu (fp64 pipe)", "fp64_pipe_slots_per_eval": instr,
+           "roofline_frac": evals * instr / (best_ms * 1e-3) / fp64_peak,
+           "peak": fp64_peak, "peak_unit": "fp64 instr/s",
+           "peak_source": "ft_measure_peaks DFMA rate (of measured)" if measured else "nominal 64 DFMA/clk/SM (of nominal)"}
+    r.close()
+    return res
+
+
 def extra_runs(args, dev, flush, measured, peaks, sm_mhz_of):
     """The other target configuration and the other kernels, two timed steps each (device-timed, L2 flushed)."""
     import torch
@@ -254,16 +304,7 @@ def extra_runs(args, dev, flush, measured, peaks, sm_mhz_of):
 
     def one(tag, wl, config, stat=None, step_kind="topk", traffic_kernel="ft_tile_kernel"):
         r = Runner(wl, dev, args, stat=stat)
-        n = wl.grid.n_templates
-        if step_kind == "full":      # full statistic arrays (write-out), no selection
-            op = torch.empty(n, dtype=torch.float32, device=dev) if r.stat != "hough" else None
-            oc = torch.empty(n, dtype=torch.int32, device=dev) if r.stat != "power" else None
-
-            def step():
-                r.ctx.eval(wl.grid, r.stat, wl.rho_th, op, oc)
-                torch.cuda.synchronize()
-        else:
-            step = r.step
+        step = r.full_arrays_step() if step_kind == "full" else r.step
         sampler = ClockSampler(dev.index or 0); sampler.start()
         ms, k_ms, n_launch = r.timed(2, 2, flush, step=step)
         clocks = sampler.stop()
@@ -289,37 +330,8 @@ def extra_runs(args, dev, flush, measured, peaks, sm_mhz_of):
     wl2, _ = make_workload(args, config=2)
     one("cfg2_count_full_array_k2h", wl2, 2, stat="hough", step_kind="full", traffic_kernel="ft_tile8_kernel")
     # K1: a xi-uniform random bank, drawn and evaluated on the device
-    for tag, wl, binary in (("k1_bank_cfg2_isolated", wl2, False), ("k1_bank_cfg3_binary", wl3, True)):
-        r = Runner(wl, dev, args)
-        g = wl.grid
-        box = dict(f0_lo=g.f0_start, f0_hi=g.f0_start + (g.n_f0 - 1) * g.df0, f1_lo=g.f1_start, f1_hi=g.f1_start + (g.n_f1 - 1) * g.df1,
-                   ra_lo=0.0, ra_hi=2 * np.pi, sd_lo=-1.0, sd_hi=1.0,
-                   ap_lo=float(np.min(g.a_p)) if binary else 0.0, ap_hi=float(np.max(g.a_p)) if binary else 0.0,
-                   porb_lo=float(np.min(g.P_orb)), porb_hi=float(np.max(g.P_orb)), t_ref=g.t_ref)
-        if binary:
-            n0 = g.sky[0]
-            ra = float(np.arctan2(n0[1], n0[0]) % (2 * np.pi))
-            box.update(ra_lo=ra, ra_hi=ra, sd_lo=float(n0[2]), sd_hi=float(n0[2]))
-        n = args.bank
-        best_ms = None
-        for rep in range(3):
-            flush.fill_(rep)
-            r.ctx.eval_bank(box, 7, 0, n, "power", wl.rho_th)          # synchronises
-            ms = r.ctx.counters()["last_kernel_ms"]
-            if rep > 0:
-                best_ms = ms if best_ms is None else min(best_ms, ms)
-        evals = n * wl.n_sft
-        fp64_peak = (measured["fp64_gflops"] / 2.0 * 1e9) if measured else FP64_FMA_PER_CLK_SM * N_SM * 1.965e9
-        # fp64-pipe slots per evaluation of the isolated path (SASS of k1_chunk<0, false, true>): 20 DADD/DMUL/
-        # DFMA/DSETP + one F2F.F64.F32 at a quarter of the DFMA rate (ft_measure_peaks: fp64_cvt_gops); the binary path adds cos()
-        instr = 24.0 if not binary else None
-        out[tag] = {"workload": f"{n} templates uniform in xi (Eq. A11) on the spectrogram of {wl.name}", "kernel": "K1 ft_list_kernel (drawn in registers)",
-                    "value": evals / (best_ms * 1e-3), "unit": UNIT, "kernel_ms": best_ms,
-                    "bound": "alu (fp64 pipe)", "fp64_pipe_instr_per_eval": instr,
-                    "roofline_frac": (evals * instr / (best_ms * 1e-3) / fp64_peak) if instr else None,
-                    "peak": fp64_peak, "peak_unit": "fp64 instr/s",
-                    "peak_source": "ft_measure_peaks DFMA rate (of measured)" if measured else "nominal 64 DFMA/clk/SM (of nominal)"}
-        r.close()
+    out["k1_bank_cfg2_isolated"] = bank_run(args, dev, flush, wl2, False, measured)
+    out["k1_bank_cfg3_binary"] = bank_run(args, dev, flush, wl3, True, measured)
     return out
 
 
@@ -406,11 +418,23 @@ def run_gpu(args):
 
     wl, idx_off = make_workload(args, rank, world)
     g = wl.grid
-    r = Runner(wl, dev, args)
+    if args.only_bank:   # K1 alone (the command of profiles/r02_k1_*.md)
+        r0 = Runner(wl, dev, args)
+        measured = r0.ctx.measure_peaks() if not args.no_peaks else None
+        r0.close()
+        res = bank_run(args, dev, flush, wl, args.only_bank == "binary", measured)
+        print(json.dumps({"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": 1, "steps": 2, "warmup": 1,
+                          "ms_per_step": res["kernel_ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                          "dtype": "f64", "data": "synthetic", "config": {"workload": res["workload"]}, "k1": res}))
+        return
+    r = Runner(wl, dev, args, stat=args.stat or None)
     measured = r.ctx.measure_peaks() if not args.no_peaks else None
+    base_step = r.full_arrays_step() if args.full_arrays else r.step
 
     def step(c=None):
-        cands = r.step(c)
+        cands = base_step(c)
+        if args.full_arrays:
+            return cands
         if world > 1:  # KBs of records: all-gather + merge under the same total order
             cands = S.merge_candidates(S.all_gather_candidates(S.to_global(cands, idx_off), dev if on_dev else None), wl.k,
                                        by_count=(wl.stat == "hough"))
@@ -458,12 +482,18 @@ def run_gpu(args):
 
     if rank == 0:
         sm_mhz = clocks.get("sm_mhz") or 1965.0
-        traffic = args.traffic if args.traffic is not None else ncu_traffic(args.config, "ft_tile_kernel")
+        traffic_kernel = "ft_tile_kernel"
+        if args.full_arrays and r.stat == "both" and args.config == 3:
+            traffic_kernel = "ft_tileb_kernel"
+        if args.full_arrays and r.stat == "hough" and args.config == 2:
+            traffic_kernel = "ft_tile8_kernel"
+        traffic = args.traffic if args.traffic is not None else ncu_traffic(args.config, traffic_kernel)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": warm, "ms_per_step": total_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic", "config": workload_config(wl, args, world, args.config),
+            "data": "synthetic", "config": dict(workload_config(wl, args, world, args.config), statistic=r.stat,
+                           step="ft_eval, full arrays written out" if args.full_arrays else "ft_eval (bind) + ft_topk_per_band (fused selection)"),
             "templates_per_sec": value / wl.n_sft,
             "gpu_launches": int(c1["kernel_launches"] - c0["kernel_launches"]),
             "clocks": clocks,
@@ -475,7 +505,7 @@ def run_gpu(args):
             "counters": {k: c1[k] for k in ("near_ties", "appended", "refined", "refine_fallbacks")},
             "kernel_geometry": r.ctx.describe(),
         }
-        if world == 1 and not args.no_extra and args.config == 2 and not args.n_sky and not args.n_sft:
+        if world == 1 and not args.no_extra and args.config == 2 and not args.n_sky and not args.n_sft and not args.stat and not args.full_arrays:
             out["extra"] = extra_runs(args, dev, flush, measured, peaks, None)
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"], _ = oracle_sample(wl, seconds=args.cpu_seconds)
@@ -514,6 +544,10 @@ def main(argv=None):
     ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per launch (default: profiles/r02_dram_traffic.csv)")
     ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
                     help="gloo: exercise the N>1 path with every rank on one GPU (testing only)")
+    ap.add_argument("--stat", default="", choices=["", "power", "hough", "both", "whough"], help="statistic (default: the configuration's)")
+    ap.add_argument("--full-arrays", action="store_true", help="step = ft_eval with full statistic arrays written out, no selection")
+    ap.add_argument("--only-bank", default="", choices=["", "isolated", "binary"],
+                    help="run K1 alone: a xi-uniform random bank on the configuration's spectrogram")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="headline configuration only")
     ap.add_argument("--no-peaks", action="store_true", help="skip ft_measure_peaks (roofline against nominal peaks)")
