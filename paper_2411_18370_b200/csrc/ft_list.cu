@@ -48,26 +48,35 @@ __device__ __forceinline__ double ft_div_c(double dot) {
 // 18 fp64 instructions against ~25 plus two conversions and three table loads of the library routine.  Absolute
 // error < 3e-16 for |x| < 1e8 (checked against 300-bit arithmetic when the constants were derived; on the device
 // against cos() in tests/test_gpu_templates.py), i.e. < 1e-14 bin on the track: far inside the 1e-9 tie window.
+// (the constants live in the constant bank: a DFMA takes c[bank][offset] as an operand, whereas a 64-bit literal costs two
+// UMOV issue slots per use -- 26 of the ~110 instructions of a binary evaluation before this)
+__constant__ double kCosC[17] = {
+    0.31830988618379069,        // 1/pi
+    3.1415926535897931,         // pi = 0x1.921fb54442d18p+1
+    1.2246467991473532e-16,     //    + 0x1.1a62633145c07p-53
+    -2.9947698097183397e-33,    //    - 0x1.f1976b7ed8fbcp-109
+    1.6117375710961184e-24,     // 1/24!
+    -8.8967913924505741e-22,    // -1/22!
+    4.1103176233121648e-19,     // 1/20!
+    -1.5619206968586225e-16,    // -1/18!
+    4.7794773323873853e-14,     // 1/16!
+    -1.1470745597729725e-11,    // -1/14!
+    2.08767569878681e-09,       // 1/12!
+    -2.7557319223985888e-07,    // -1/10!
+    2.4801587301587302e-05,     // 1/8!
+    -0.0013888888888888889,     // -1/6!
+    0.041666666666666664,       // 1/4!
+    -0.5, 1.0};
 __device__ __forceinline__ double k1_cos(double x) {
-  const double tm = __fma_rn(x, 0.31830988618379069, kMagic);            // 1/pi; rint(x / pi) in the low mantissa bits
+  const double tm = __fma_rn(x, kCosC[0], kMagic);                       // rint(x / pi) in the low mantissa bits
   const double k = __dsub_rn(tm, kMagic);
-  double r = __fma_rn(-k, 3.1415926535897931, x);                        // pi = 0x1.921fb54442d18p+1
-  r = __fma_rn(-k, 1.2246467991473532e-16, r);                           //    + 0x1.1a62633145c07p-53
-  r = __fma_rn(-k, -2.9947698097183397e-33, r);                          //    - 0x1.f1976b7ed8fbcp-109
+  double r = __fma_rn(-k, kCosC[1], x);
+  r = __fma_rn(-k, kCosC[2], r);
+  r = __fma_rn(-k, kCosC[3], r);
   const double z = __dmul_rn(r, r);
-  double t = 1.6117375710961184e-24;                                     // 1/24!
-  t = __fma_rn(t, z, -8.8967913924505741e-22);                           // -1/22!
-  t = __fma_rn(t, z, 4.1103176233121648e-19);                            // 1/20!
-  t = __fma_rn(t, z, -1.5619206968586225e-16);                           // -1/18!
-  t = __fma_rn(t, z, 4.7794773323873853e-14);                            // 1/16!
-  t = __fma_rn(t, z, -1.1470745597729725e-11);                           // -1/14!
-  t = __fma_rn(t, z, 2.08767569878681e-09);                              // 1/12!
-  t = __fma_rn(t, z, -2.7557319223985888e-07);                           // -1/10!
-  t = __fma_rn(t, z, 2.4801587301587302e-05);                            // 1/8!
-  t = __fma_rn(t, z, -0.0013888888888888889);                            // -1/6!
-  t = __fma_rn(t, z, 0.041666666666666664);                              // 1/4!
-  t = __fma_rn(t, z, -0.5);
-  t = __fma_rn(t, z, 1.0);
+  double t = kCosC[4];
+#pragma unroll
+  for (int i = 5; i < 17; ++i) t = __fma_rn(t, z, kCosC[i]);
   return __hiloint2double(__double2hiint(t) ^ (__double2loint(tm) << 31), __double2loint(t));   // (-1)^k
 }
 
@@ -167,11 +176,11 @@ __device__ __forceinline__ double k1_f2d(float x) {
 #endif
 }
 
-// The SFT loop over one staged chunk of m SFTs.  BIN: some template of the CTA is a binary (the orbital cosine
-// is in the loop body); CTAs of isolated templates run the body without it.  PERSFT: per-SFT weights (staged as
+// The SFT loop over one staged chunk of m SFTs.  BIN: 0 no template of the CTA is a binary (no orbital cosine in the
+// loop body), 2 every template is (cosine without a branch), 1 mixed (cosine under a per-thread branch).  PERSFT: per-SFT weights (staged as
 // doubles) or per-bin weights (gathered like the pixel).  The loop has no branch: an out-of-range bin is clamped
 // for the load and remembered in acc.bad (the template's outputs are then discarded).
-template <int STAT, bool BIN, bool PERSFT>
+template <int STAT, int BIN, bool PERSFT>
 __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp, double Om, double apOm, bool binary,
                                          const double2* sA, const double2* sB, const double2* sC, int m, int64_t a0,
                                          uint32_t n_bins, K1Acc& acc) {
@@ -191,7 +200,7 @@ __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp
     double D = __dadd_rn(1.0, V);
     if (BIN) {   // (an isolated template of a mixed CTA subtracts B = 0: (1 + V) - 0 = 1 + V)
       double B = 0.0;
-      if (binary) B = __dmul_rn(apOm, k1_cos(__dmul_rn(Om, __dsub_rn(sC[c].y, tp.t_asc))));
+      if (BIN == 2 || binary) B = __dmul_rn(apOm, k1_cos(__dmul_rn(Om, __dsub_rn(sC[c].y, tp.t_asc))));
       D = __dsub_rn(D, B);
     }
     const double x = ft_track_x(tp.f0, __dmul_rn(tp.f1, vzdt.y), D, f_min, inv_df);
@@ -232,6 +241,7 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
   const double apOm = __dmul_rn(tp.a_p, Om);
   const bool binary = tp.a_p != 0.0;
   const bool any_binary = __syncthreads_or(binary && active) != 0;
+  const bool all_binary = __syncthreads_and(binary || !active) != 0;
   const uint32_t n_bins = (uint32_t)min(d.n_bins, (int64_t)0x7fffffff);
   const bool per_sft = d.wkind == 1;
   K1Acc acc{0.0, 0, 0u, 0u};
@@ -247,12 +257,15 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
     __syncthreads();
     const int m = (int)min((int64_t)K1_THREADS, d.n_sft - a0);
     if (active) {
-      if (any_binary) {
-        if (per_sft) k1_chunk<STAT, true, true>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
-        else k1_chunk<STAT, true, false>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+      if (all_binary) {
+        if (per_sft) k1_chunk<STAT, 2, true>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 2, false>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+      } else if (any_binary) {
+        if (per_sft) k1_chunk<STAT, 1, true>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 1, false>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
       } else {
-        if (per_sft) k1_chunk<STAT, false, true>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
-        else k1_chunk<STAT, false, false>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+        if (per_sft) k1_chunk<STAT, 0, true>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 0, false>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
       }
     }
   }

@@ -191,7 +191,7 @@ __device__ __forceinline__ uint32_t ft_tile_entry(const FtDev& d, const FtPoint&
 // fp32 pixels: J conflict-free LDS.32 + J/2 packed adds per row
 struct GatherF32 {
   static constexpr int CW = 32, PER = 1;
-  static constexpr bool ROWW = false, VETO = false, HASCNT = false;
+  static constexpr bool ROWW = false, VETO = false, HASCNT = false, PAIRS = false;
   template <int J> struct State { float acc[J]; };
   static __device__ __forceinline__ size_t extra_smem(int, int) { return 0; }
   template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t, uint32_t) {
@@ -268,7 +268,7 @@ struct GatherF32W : GatherF32 {
 // per block of 32 SFTs.  The pixel is rounded to 18 mantissa bits (<= 3.8e-6 of |q| per pixel, random sign:
 // ~3e-8 of the statistic at n_sft = 8000; the plan keeps this kernel to 64 <= n_sft <= 65535).
 struct GatherBoth : GatherF32 {
-  static constexpr bool VETO = true, HASCNT = true;
+  static constexpr bool VETO = true, HASCNT = true, PAIRS = true;
   static constexpr uint32_t kLowMask = 63u;
   template <int J> struct State { float acc[J]; uint32_t raw[J]; uint32_t c16[(J + 1) / 2]; };
   template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t, uint32_t) {
@@ -288,17 +288,48 @@ struct GatherBoth : GatherF32 {
 #pragma unroll
     for (int j = 0; j + 1 < J; j += 2) ft_add2(st.acc[j], st.acc[j + 1], v[j], v[j + 1]);
     if (J & 1) st.acc[J - 1] += v[J - 1];
-    // the hit bit rides in the low bits: one integer add of the raw word.  Alternate chunks add on the FMA pipe
-    // (IMAD by a register holding 1) and on the ALU pipe (IADD3), so neither pipe limits the issue rate.
-#ifndef FT_K2B_IMAD
-#define FT_K2B_IMAD 1
-#endif
-    uint32_t one = 1u;
-    asm volatile("" : "+r"(one));
+    // the hit bit rides in the low bits: one integer add of the raw word
 #pragma unroll
-    for (int j = 0; j < J; ++j) {
-      if (FT_K2B_IMAD == 2 || (FT_K2B_IMAD == 1 && (j & 1))) asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(st.raw[j]) : "r"(__float_as_uint(v[j])), "r"(one));
-      else st.raw[j] += __float_as_uint(v[j]);
+    for (int j = 0; j < J; ++j) st.raw[j] += __float_as_uint(v[j]);
+  }
+  // Two rows at once (both without a break in the warp's range): the raw words of the two rows and the running
+  // sum are ONE three-input integer add (IADD3), so a pixel costs 1 LDS + 1/2 FADD2 + 1/2 IADD3.  Loads are issued
+  // in two half batches to bound the registers in flight.
+  template <int J> static __device__ __forceinline__ void rows_fast_pair(State<J>& st, uint32_t e0, uint32_t e1, uint32_t base0,
+                                                                         uint32_t base1, bool last_ok) {
+    const uint32_t ad0 = base0 + 4u * e0, ad1 = base1 + 4u * e1;
+    constexpr int H = (((J + 1) / 2) + 1) & ~1;   // even, so the packed adds never straddle a batch
+#pragma unroll
+    for (int h0 = 0; h0 < J; h0 += H) {
+      float v0[H], v1[H];
+#pragma unroll
+      for (int i = 0; i < H; ++i) {
+        const int j = h0 + i;
+        if (j < J) {
+          if (j < J - 1 || last_ok) { v0[i] = lds_f32(ad0 + 128u * j); v1[i] = lds_f32(ad1 + 128u * j); }
+          else { v0[i] = 0.f; v1[i] = 0.f; }
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < H; i += 2) {
+        const int j = h0 + i;
+        if (j + 1 < J) {
+          ft_add2(st.acc[j], st.acc[j + 1], v0[i], v0[i + 1]);
+          ft_add2(st.acc[j], st.acc[j + 1], v1[i], v1[i + 1]);
+        } else if (j < J) {
+          st.acc[j] += v0[i];
+          st.acc[j] += v1[i];
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < H; ++i) {
+        const int j = h0 + i;
+        if (j < J) {
+          uint32_t r = st.raw[j];
+          asm("{\n.reg .u32 t;\nadd.u32 t, %1, %2;\nadd.u32 %0, %0, t;\n}" : "+r"(r) : "r"(__float_as_uint(v0[i])), "r"(__float_as_uint(v1[i])));
+          st.raw[j] = r;
+        }
+      }
     }
   }
   template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t,
@@ -334,7 +365,7 @@ struct GatherBoth : GatherF32 {
 // SFTs the counters are folded into 16-bit levels in shared memory (n_sft <= 65535 is a plan condition).
 struct GatherHit8 {
   static constexpr int CW = 128, PER = 4;
-  static constexpr bool ROWW = false, VETO = false, HASCNT = true;
+  static constexpr bool ROWW = false, VETO = false, HASCNT = true, PAIRS = false;
   static constexpr int kFlushBlocks = 7;  // 7 blocks of 32 SFTs = 224 <= 255 increments per 8-bit counter
   template <int J> struct State { uint32_t c8[J]; uint32_t c16, n_ct; };
   template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t extra0, uint32_t n_ct) {
@@ -534,14 +565,27 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
         asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
                      : "=r"(u4[0]), "=r"(u4[1]), "=r"(u4[2]), "=r"(u4[3]) : "r"(wtab + 4u * (uint32_t)q));
       mbar_wait(full0 + 8 * s, ph);
+      if (q + kRPS <= n_rows && (e4[0] | e4[1] | e4[2] | e4[3]) < 8192u) {
+        // a full stage and no break in this warp's range in any of its rows (the common case): straight-line body
+        if constexpr (G::PAIRS) {
+          G::template rows_fast_pair<J>(st, e4[0], e4[1], stage_addr, stage_addr + row_bytes, last_ok);
+          G::template rows_fast_pair<J>(st, e4[2], e4[3], stage_addr + 2u * row_bytes, stage_addr + 3u * row_bytes, last_ok);
+        } else {
 #pragma unroll
-      for (int r = 0; r < kRPS; ++r) {
-        if (q + r < n_rows) {
-          const uint32_t e = e4[r];
-          const uint32_t base = stage_addr + (uint32_t)r * row_bytes;
-          const float u = G::ROWW ? __uint_as_float(u4[r]) : 1.f;
-          if (e < 8192u) G::template row_fast<J>(st, e, base, copy_pitch, last_ok, u);   // no break in this warp's range
-          else G::template row_break<J>(st, e, base, copy_pitch, lane, u);
+          for (int r = 0; r < kRPS; ++r)
+            G::template row_fast<J>(st, e4[r], stage_addr + (uint32_t)r * row_bytes, copy_pitch, last_ok,
+                                    G::ROWW ? __uint_as_float(u4[r]) : 1.f);
+        }
+      } else {
+#pragma unroll
+        for (int r = 0; r < kRPS; ++r) {
+          if (q + r < n_rows) {
+            const uint32_t e = e4[r];
+            const uint32_t base = stage_addr + (uint32_t)r * row_bytes;
+            const float u = G::ROWW ? __uint_as_float(u4[r]) : 1.f;
+            if (e < 8192u) G::template row_fast<J>(st, e, base, copy_pitch, last_ok, u);   // no break in this warp's range
+            else G::template row_break<J>(st, e, base, copy_pitch, lane, u);
+          }
         }
       }
       __syncwarp();
