@@ -224,8 +224,9 @@ bool ft_tile_choose(const FtDev& d, const FtTileHostIn& in, int mode, FtTilePlan
   pl.tile_w = (int32_t)(((chunks + bT - 1) / bT) * cw);
   pl.n_tiles = (int32_t)((d.n_f0 + pl.tile_w - 1) / pl.tile_w);
   // default: 24-27 consumer warps per CTA (measured best on B200 at 72 registers: R = 12 at wpp = 2,
-  // R = 6 at wpp = 4, R = 27 at wpp = 1); the 80-register kernels keep 23
-  int R = in.points_per_cta > 0 ? in.points_per_cta : (mode != 0 ? 23 / pl.wpp : (pl.wpp == 1 ? 27 : 24 / pl.wpp));
+  // R = 6 at wpp = 4, R = 27 at wpp = 1; the one-pass kernel the same, its thread limit permitting); the 80-register
+  // kernels keep 23
+  int R = in.points_per_cta > 0 ? in.points_per_cta : ((mode == 1 || mode == 3) ? 23 / pl.wpp : (pl.wpp == 1 ? 27 : 24 / pl.wpp));
   const int max_threads = mode == 1 ? ft_tile8_max_threads(pl.J) : mode == 2 ? ft_tileb_max_threads(pl.J)
                         : mode == 3 ? ft_tilew_max_threads(pl.J) : ft_tile_max_threads(pl.J);
   R = std::min<int>(R, (max_threads / 32 - 1) / pl.wpp);  // + 1 producer warp

@@ -48,8 +48,8 @@ __host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 
 __host__ __device__ constexpr int ft_tile8_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tile8_max_threads(int J) { return J <= 8 ? 1024 : 768; }
 // both statistics in one pass: J accumulators + J counters + J loads in flight
-__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : 80; }
-__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : 768; }
+__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : J <= 15 ? 72 : 80; }
+__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : J <= 15 ? 896 : 768; }
 // row-weighted gather: J accumulators + J loads in flight + the fp64 weight sums
 __host__ __device__ constexpr int ft_tilew_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tilew_max_threads(int J) { return J <= 8 ? 1024 : 768; }
@@ -296,7 +296,7 @@ struct GatherBoth : GatherF32 {
   // sum are ONE three-input integer add (IADD3), so a pixel costs 1 LDS + 1/2 FADD2 + 1/2 IADD3.  Loads are issued
   // in two half batches to bound the registers in flight.
   template <int J> static __device__ __forceinline__ void rows_fast_pair(State<J>& st, uint32_t e0, uint32_t e1, uint32_t base0,
-                                                                         uint32_t base1, bool last_ok) {
+                                                                         uint32_t base1, uint32_t, bool last_ok) {
     const uint32_t ad0 = base0 + 4u * e0, ad1 = base1 + 4u * e1;
     constexpr int H = (((J + 1) / 2) + 1) & ~1;   // even, so the packed adds never straddle a batch
 #pragma unroll
@@ -365,7 +365,7 @@ struct GatherBoth : GatherF32 {
 // SFTs the counters are folded into 16-bit levels in shared memory (n_sft <= 65535 is a plan condition).
 struct GatherHit8 {
   static constexpr int CW = 128, PER = 4;
-  static constexpr bool ROWW = false, VETO = false, HASCNT = true, PAIRS = false;
+  static constexpr bool ROWW = false, VETO = false, HASCNT = true, PAIRS = true;
   static constexpr int kFlushBlocks = 7;  // 7 blocks of 32 SFTs = 224 <= 255 increments per 8-bit counter
   template <int J> struct State { uint32_t c8[J]; uint32_t c16, n_ct; };
   template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t extra0, uint32_t n_ct) {
@@ -399,6 +399,22 @@ struct GatherHit8 {
 #pragma unroll
     for (int j = 0; j < J; ++j)
       if (j < J - 1 || last_ok) st.c8[j] += v[j];
+  }
+  // two rows at once: the packed hits of both rows and the running counters are one three-input add (IADD3)
+  template <int J> static __device__ __forceinline__ void rows_fast_pair(State<J>& st, uint32_t e0, uint32_t e1, uint32_t base0,
+                                                                         uint32_t base1, uint32_t copy_pitch, bool last_ok) {
+    const uint32_t ad0 = base0 + (e0 & 3u) * copy_pitch + (e0 & ~3u), ad1 = base1 + (e1 & 3u) * copy_pitch + (e1 & ~3u);
+    uint32_t v0[J], v1[J];
+#pragma unroll
+    for (int j = 0; j < J; ++j)
+      if (j < J - 1 || last_ok) { v0[j] = lds_u32(ad0 + 128u * j); v1[j] = lds_u32(ad1 + 128u * j); }
+#pragma unroll
+    for (int j = 0; j < J; ++j)
+      if (j < J - 1 || last_ok) {
+        uint32_t r = st.c8[j];
+        asm("{\n.reg .u32 t;\nadd.u32 t, %1, %2;\nadd.u32 %0, %0, t;\n}" : "+r"(r) : "r"(v0[j]), "r"(v1[j]));
+        st.c8[j] = r;
+      }
   }
   template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t copy_pitch,
                                                                     int lane, float) {
@@ -568,8 +584,8 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
       if (q + kRPS <= n_rows && (e4[0] | e4[1] | e4[2] | e4[3]) < 8192u) {
         // a full stage and no break in this warp's range in any of its rows (the common case): straight-line body
         if constexpr (G::PAIRS) {
-          G::template rows_fast_pair<J>(st, e4[0], e4[1], stage_addr, stage_addr + row_bytes, last_ok);
-          G::template rows_fast_pair<J>(st, e4[2], e4[3], stage_addr + 2u * row_bytes, stage_addr + 3u * row_bytes, last_ok);
+          G::template rows_fast_pair<J>(st, e4[0], e4[1], stage_addr, stage_addr + row_bytes, copy_pitch, last_ok);
+          G::template rows_fast_pair<J>(st, e4[2], e4[3], stage_addr + 2u * row_bytes, stage_addr + 3u * row_bytes, copy_pitch, last_ok);
         } else {
 #pragma unroll
           for (int r = 0; r < kRPS; ++r)
