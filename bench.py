@@ -302,9 +302,11 @@ def extra_runs(args, dev, flush, measured, peaks, sm_mhz_of):
     from paper_2411_18370_b200 import binding as B
     out = {}
 
-    def one(tag, wl, config, stat=None, step_kind="topk", traffic_kernel="ft_tile_kernel"):
+    def one(tag, wl, config, stat=None, step_kind="topk", traffic_kernel="ft_tile_kernel", prepare=None, step_of=None):
         r = Runner(wl, dev, args, stat=stat)
-        step = r.full_arrays_step() if step_kind == "full" else r.step
+        if prepare:
+            prepare(r)
+        step = step_of(r) if step_of else r.full_arrays_step() if step_kind == "full" else r.step
         sampler = ClockSampler(dev.index or 0); sampler.start()
         ms, k_ms, n_launch = r.timed(2, 2, flush, step=step)
         clocks = sampler.stop()
@@ -329,6 +331,24 @@ def extra_runs(args, dev, flush, measured, peaks, sm_mhz_of):
     del wl4
     wl2, _ = make_workload(args, config=2)
     one("cfg2_count_full_array_k2h", wl2, 2, stat="hough", step_kind="full", traffic_kernel="ft_tile8_kernel")
+    # the weighted number count as the statistic; sky-dependent weights (Eq. 4-5) with the paper's
+    # post-processing (loudest template per box of sky points x sub-band, ranked by z, Eq. 36); power top-k under the
+    # weighted-count veto
+    one("cfg2_weighted_count_topk", wl2, 2, stat="whough", step_kind="topk (ranked by the weighted number count)")
+    n_pts = wl2.grid.n_templates // wl2.grid.n_f0
+    pbox = (np.arange(n_pts, dtype=np.int64) * 16 // n_pts).astype(np.int32)
+
+    def box_step(r):
+        def step():
+            r.ctx.eval(wl2.grid, "power", wl2.rho_th)
+            return r.ctx.topk_per_box(pbox, 16, wl2.band_width, 1, rank_by_z=True)
+        return step
+    one("cfg2_antenna_weights_loudest_per_box_by_z", wl2, 2, stat="power", step_kind="ft_eval + ft_topk_per_box (16 boxes of sky points x 20 sub-bands, k = 1, by z)",
+        traffic_kernel="ft_tilew_kernel", prepare=lambda r: r.ctx.set_antenna(*W.antenna_geometry(wl2)), step_of=box_step)
+    p_hit = float(np.exp(-wl2.rho_th)); w2 = np.asarray(wl2.w, dtype=np.float64)
+    wfloor = p_hit * w2.sum() + 3.0 * np.sqrt(p_hit * (1.0 - p_hit) * (w2 ** 2).sum())
+    one("cfg2_power_topk_weighted_count_veto", wl2, 2, stat="both", step_kind="topk under the weighted number-count floor mu + 3 sigma",
+        prepare=lambda r: r.ctx.set_option_f64(B.FT_OPT_WCOUNT_FLOOR, wfloor))
     # K1: a xi-uniform random bank, drawn and evaluated on the device
     out["k1_bank_cfg2_isolated"] = bank_run(args, dev, flush, wl2, False, measured)
     out["k1_bank_cfg3_binary"] = bank_run(args, dev, flush, wl3, True, measured)
@@ -429,6 +449,8 @@ def run_gpu(args):
         return
     r = Runner(wl, dev, args, stat=args.stat or None)
     measured = r.ctx.measure_peaks() if not args.no_peaks else None
+    if args.antenna:   # sky-dependent weights (Eq. 4-5): the row-weighted tile kernel
+        r.ctx.set_antenna(*W.antenna_geometry(wl))
     base_step = r.full_arrays_step() if args.full_arrays else r.step
 
     def step(c=None):
@@ -487,6 +509,8 @@ def run_gpu(args):
             traffic_kernel = "ft_tileb_kernel"
         if args.full_arrays and r.stat == "hough" and args.config == 2:
             traffic_kernel = "ft_tile8_kernel"
+        if args.antenna:
+            traffic_kernel = "ft_tilew_kernel"
         traffic = args.traffic if args.traffic is not None else ncu_traffic(args.config, traffic_kernel)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -505,7 +529,7 @@ def run_gpu(args):
             "counters": {k: c1[k] for k in ("near_ties", "appended", "refined", "refine_fallbacks")},
             "kernel_geometry": r.ctx.describe(),
         }
-        if world == 1 and not args.no_extra and args.config == 2 and not args.n_sky and not args.n_sft and not args.stat and not args.full_arrays:
+        if world == 1 and not args.no_extra and args.config == 2 and not args.n_sky and not args.n_sft and not args.stat and not args.full_arrays and not args.antenna:
             out["extra"] = extra_runs(args, dev, flush, measured, peaks, None)
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"], _ = oracle_sample(wl, seconds=args.cpu_seconds)
@@ -548,6 +572,7 @@ def main(argv=None):
     ap.add_argument("--full-arrays", action="store_true", help="step = ft_eval with full statistic arrays written out, no selection")
     ap.add_argument("--only-bank", default="", choices=["", "isolated", "binary"],
                     help="run K1 alone: a xi-uniform random bank on the configuration's spectrogram")
+    ap.add_argument("--antenna", action="store_true", help="sky-dependent weights w_a(n) (ft_set_antenna with the workload's detector geometry)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="headline configuration only")
     ap.add_argument("--no-peaks", action="store_true", help="skip ft_measure_peaks (roofline against nominal peaks)")

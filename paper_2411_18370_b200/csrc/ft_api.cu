@@ -66,6 +66,7 @@ int tile_pass(ft_ctx* c, const FtTilePlan& plan, const FtPass& p, const float* A
   run.zmode = zmode; run.out_key = zmode ? p.out_key : 0;
   run.z_mu = c->d.mu_G; run.z_inv_sigma = c->d.sigma_G > 0.0 ? 1.0 / c->d.sigma_G : 1.0;
   run.near_ties = c->near_ties_dev;
+  run.sky_norm = c->skyn_dev; run.norm_cb = (A == c->WH_dev) ? 3 : 2;
   int launches = 0;
   ft_tick(c);
   const cudaError_t e = ft_launch_tile(c->d, plan, run, p.pt_begin, p.pt_end, c->stream, &launches, p.glist, p.n_glist, p.gskip);
@@ -416,6 +417,12 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
     c->counters.kernel_launches += 1;
     c->WH_rho = d.rho; c->WH_valid = true;
   }
+  if (c->tilew_ok) {
+    // sky-dependent weights: normalisation, add-back and sigma_G of every sky point of the grid (one small pass)
+    FT_CUDA(c, ft_grow(c->skyn_dev, c->skyn_cap, 4 * (size_t)d.n_sky));
+    FT_CUDA(c, ft_launch_skyw_norm(d, c->cQ_dev, (want_wh && c->WH_valid) ? c->cWH_dev : nullptr, c->skyn_dev, c->stream));
+    c->counters.kernel_launches += 1;
+  }
   {
     char buf[400];
     auto geom = [&](const FtTilePlan& pl) {
@@ -501,7 +508,7 @@ void ft_destroy(ft_ctx* c) {
   ft_dfree(c->H8_dev); ft_dfree(c->QB_dev); ft_dfree(c->WH_dev); ft_dfree(c->cWH_dev); ft_dfree(c->cQ_dev);
   ft_dfree(c->t_mid_dev); ft_dfree(c->vel_dev); ft_dfree(c->w_dev); ft_dfree(c->Q_dev); ft_dfree(c->H_dev);
   ft_dfree(c->ctab_dev); ft_dfree(c->axes_dev); ft_dfree(c->w_row_dev); ft_dfree(c->ant_dev); ft_dfree(c->vr_dev);
-  ft_dfree(c->maxw_dev); ft_dfree(c->scratch_f); ft_dfree(c->scratch_i); ft_dfree(c->veto_cnt); ft_dfree(c->veto_w);
+  ft_dfree(c->skyn_dev); ft_dfree(c->maxw_dev); ft_dfree(c->scratch_f); ft_dfree(c->scratch_i); ft_dfree(c->veto_cnt); ft_dfree(c->veto_w);
   ft_dfree(c->glist_dev); ft_dfree(c->pbox_dev); ft_dfree(c->io_dev); ft_dfree(c->near_ties_dev); ft_dfree(c->flag_dev);
   ft_dfree(c->tile_err_dev);
   for (cudaEvent_t e : c->evs) cudaEventDestroy(e);

@@ -32,6 +32,8 @@ struct ft_ctx {
   float WH_rho = 0.f; bool WH_valid = false;
   double* w_row_dev = nullptr;  // [n_sft] row means of per-bin weights
   double* ant_dev = nullptr;    // [n_sft][9] antenna coefficients (ft_set_antenna)
+  double* skyn_dev = nullptr;   // [n_sky][4] normalisation sums of the sky-dependent weights of the bound grid (grow-only)
+  size_t skyn_cap = 0;
   double* axes_dev = nullptr;   // sky | a_p | P_orb | tasc (grow-only buffer)
   size_t axes_cap = 0;
   std::vector<double> axes_host;

@@ -208,7 +208,7 @@ bool ft_tile_choose(const FtDev& d, const FtTileHostIn& in, int mode, FtTilePlan
     if (nt > 1 && in.force_tiles <= 0 && (chunks + nt - 2) / (nt - 1) == cpt) continue;  // same tile size as nt-1
     for (int wpp = 1; wpp <= 4; ++wpp) {
       const int64_t Jn = (cpt + wpp - 1) / wpp;
-      if (Jn > (mode == 0 ? 32 : 16)) continue;
+      if (Jn > ((mode == 0 || mode == 3) ? 32 : 16)) continue;
       int J = 0;
       for (int c : kJList) if (c >= Jn) { J = c; break; }
       if (J == 0 || J > maxJ_eps) continue;
@@ -226,7 +226,7 @@ bool ft_tile_choose(const FtDev& d, const FtTileHostIn& in, int mode, FtTilePlan
   // default: 24-27 consumer warps per CTA (measured best on B200 at 72 registers: R = 12 at wpp = 2,
   // R = 6 at wpp = 4, R = 27 at wpp = 1; the one-pass kernel the same, its thread limit permitting); the 80-register
   // kernels keep 23
-  int R = in.points_per_cta > 0 ? in.points_per_cta : ((mode == 1 || mode == 3) ? 23 / pl.wpp : (pl.wpp == 1 ? 27 : 24 / pl.wpp));
+  int R = in.points_per_cta > 0 ? in.points_per_cta : (mode == 1 ? 23 / pl.wpp : (pl.wpp == 1 ? 27 : 24 / pl.wpp));
   const int max_threads = mode == 1 ? ft_tile8_max_threads(pl.J) : mode == 2 ? ft_tileb_max_threads(pl.J)
                         : mode == 3 ? ft_tilew_max_threads(pl.J) : ft_tile_max_threads(pl.J);
   R = std::min<int>(R, (max_threads / 32 - 1) / pl.wpp);  // + 1 producer warp
@@ -323,6 +323,7 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const FtTileR
   a.pbox = run.pbox; a.n_bands = run.n_bands;
   a.zmode = run.zmode; a.out_key = run.out_key; a.z_mu = run.z_mu; a.z_inv_sigma = run.z_inv_sigma;
   a.out_sigma = run.out_sigma;
+  a.sky_norm = run.sky_norm; a.norm_cb = run.norm_cb;
   a.near_ties = run.near_ties;
   a.glist = glist; a.gskip = gskip;
   const unsigned block = (unsigned)((plan.R * plan.wpp + 1) * 32);

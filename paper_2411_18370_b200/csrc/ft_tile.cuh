@@ -12,7 +12,7 @@ struct FtTilePlan {
   int32_t* err = nullptr;       // [1] set by the kernel if a track left its staged strip (plan bug); the handle's, shared by its plans
   int32_t mode = 0;             // 0: fp32 gather (ft_tile_kernel), 1: packed number count (ft_tile8_kernel),
                                 // 2: both statistics in one pass (ft_tileb_kernel, J <= 16),
-                                // 3: fp32 gather times a per-(point, SFT) weight (ft_tilew_kernel, J <= 16)
+                                // 3: fp32 gather times a per-(point, SFT) weight (ft_tilew_kernel)
   int32_t cw = 32;              // f0 per chunk (per warp load instruction): 32 or 128
   int32_t align = 4;            // strip start / length granularity, bins
   int32_t n_tiles = 0;          // f0 tiles
@@ -63,6 +63,8 @@ struct FtTileRun {
   int32_t zmode = 0, out_key = 0;
   double z_mu = 0.0, z_inv_sigma = 1.0;
   float* out_sigma = nullptr;
+  const double* sky_norm = nullptr;   // row-weighted gather: [n_sky][4] normalisation sums (ft_launch_skyw_norm)
+  int32_t norm_cb = 2;                // which add-back column of sky_norm: 2 (power array Q) or 3 (weighted hits WH)
   unsigned long long* near_ties = nullptr;
 };
 // glist != nullptr: evaluate only the CTA groups glist[0 .. n_glist) (the threshold sample; a group = R consecutive
@@ -81,4 +83,7 @@ cudaError_t ft_launch_fold_centered(const float* P, const float* w_sft, const fl
                                     cudaStream_t s);
 // QB = Q with the least significant bit replaced by the hit (P > rho): gather array of ft_tileb_kernel
 cudaError_t ft_launch_qb(const float* Q, const float* P, float rho, float* QB, int64_t n, cudaStream_t s);
+// Sky-dependent weights: per sky point  sum_a u_a r_a,  sum_a (u_a r_a)^2,  sum_a u_a cQ_a,  sum_a u_a cWH_a  with
+// u_a = fl32(a^2 + b^2) as the row-weighted gather applies it (cWH may be nullptr).  out [n_sky][4].
+cudaError_t ft_launch_skyw_norm(const FtDev& d, const float* cQ, const float* cWH, double* out, cudaStream_t s);
 void ft_tile_plan_free(FtTilePlan* plan);

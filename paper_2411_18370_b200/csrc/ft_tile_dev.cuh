@@ -33,6 +33,9 @@ struct FtTileArgs {
   int32_t out_key;      // out_f receives the selection key (z in zmode) instead of the statistic
   double z_mu, z_inv_sigma;
   float* out_sigma;     // row-weighted gather: sigma_G of every outer point, [n_points] (or nullptr)
+  const double* sky_norm;  // row-weighted gather: per sky point  sum_a u_a r_a,  sum_a (u_a r_a)^2,  sum_a u_a cQ_a,  sum_a u_a cWH_a
+                           // [n_sky][4] (ft_skyw_norm_kernel, bind time);  norm_cb = 2 or 3: the add-back column of this pass
+  int32_t norm_cb;
   unsigned long long* near_ties;
   const uint32_t* glist;  // != nullptr: the launch runs the CTA groups glist[0 .. grid / n_tiles) (the threshold
                           // sample), outputs packed by launch-local row (group_local * R + r) * n_f0 + i_f0
@@ -48,11 +51,12 @@ __host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 
 __host__ __device__ constexpr int ft_tile8_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tile8_max_threads(int J) { return J <= 8 ? 1024 : 768; }
 // both statistics in one pass: J accumulators + J counters + J loads in flight
-__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : J <= 15 ? 72 : 80; }
-__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : J <= 15 ? 896 : 768; }
-// row-weighted gather: J accumulators + J loads in flight + the fp64 weight sums
-__host__ __device__ constexpr int ft_tilew_max_regs(int J) { return J <= 8 ? 64 : 80; }
-__host__ __device__ constexpr int ft_tilew_max_threads(int J) { return J <= 8 ? 1024 : 768; }
+__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : 80; }
+__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : 768; }
+// row-weighted gather: as the plain gather (the sky-point tables live in shared memory, the normalisation sums come
+// from a bind-time pass)
+__host__ __device__ constexpr int ft_tilew_max_regs(int J) { return ft_tile_max_regs(J); }
+__host__ __device__ constexpr int ft_tilew_max_threads(int J) { return ft_tile_max_threads(J); }
 
 cudaError_t ft_tile_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
 cudaError_t ft_tilew_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
@@ -79,7 +83,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "{\n"
       ".reg .pred p;\n"
       "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 0x989680;\n"   // suspend-time hint: sleep in hardware, not in a spin loop
       "@p bra DONE_%=;\n"
       "bra WAIT_%=;\n"
       "DONE_%=:\n"
@@ -453,10 +457,10 @@ struct GatherHit8 {
 };
 
 // Shared-memory layout (bytes): ring [NS][kRPS][row_bytes] | full[NS] empty[NS] mbarriers | FtPoint[n_cw] |
-// entry table [n_cw][32] u32 | (ROWW: weight table [n_cw][32] f32) | policy extra.
+// entry table [n_cw][32] u32 | (ROWW: weight table [n_cw][32] f32 | FtSkyPoint[n_cw]) | policy extra.
 template <class G>
 __host__ __device__ inline size_t ft_tile_state_bytes(int J, int n_cw) {
-  return (sizeof(FtPoint) + 128 + (G::ROWW ? 128 : 0)) * (size_t)n_cw + 16 +
+  return (sizeof(FtPoint) + 128 + (G::ROWW ? 128 + sizeof(FtSkyPoint) : 0)) * (size_t)n_cw + 16 +
          (G::PER == 4 ? (size_t)8 * J * 32 * n_cw : 0);
 }
 
@@ -533,7 +537,7 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
   const uint32_t etab0 = smem_u32(reinterpret_cast<FtPoint*>(bars + 2 * NS) + n_cw);
   const uint32_t etab = etab0 + 128u * (uint32_t)warp;
   const uint32_t wtab = etab0 + 128u * (uint32_t)n_cw + 128u * (uint32_t)warp;
-  const uint32_t extra0 = etab0 + (G::ROWW ? 256u : 128u) * (uint32_t)n_cw;
+  const uint32_t extra0 = etab0 + (G::ROWW ? 256u + (uint32_t)sizeof(FtSkyPoint) : 128u) * (uint32_t)n_cw;
   const int tile_i0 = tile * a.tile_w;
   const int wlo = sub * J * G::CW;                                     // warp's first output, tile-relative
   const int tile_n = min(a.tile_w, (int)d.n_f0 - tile_i0);             // valid f0 in this tile
@@ -543,13 +547,18 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
   typename G::template State<J> st;
   G::template init<J>(st, extra0, 32u * (uint32_t)n_cw);
   unsigned ties = 0;
-  // row-weighted gather: this lane's share of  sum_a u_a r_a,  sum_a (u_a r_a)^2,  sum_a u_a c_a  (fp64)
-  double w_sum = 0.0, w_sq = 0.0, w_cb = 0.0;
-  FtSkyPoint skyp;
-  if (G::ROWW) skyp = ft_sky_point(sp->nx, sp->ny, sp->nz);
+  // row-weighted gather: the sky-dependent part of a(t; n), b(t; n) of this warp's point, in shared memory
+  FtSkyPoint* skyp = reinterpret_cast<FtSkyPoint*>(reinterpret_cast<unsigned char*>(reinterpret_cast<FtPoint*>(bars + 2 * NS) + n_cw) +
+                                                   256 * (size_t)n_cw) + warp;
+  if (G::ROWW) {
+    if (lane == 0) *skyp = ft_sky_point(sp->nx, sp->ny, sp->nz);
+    __syncwarp();
+  }
   const uint32_t lane_bytes = ring0 + 4u * (uint32_t)lane;
   uint32_t stage_addr = lane_bytes;
-  int s = 0;
+  // barriers of the current stage: full at fb, empty at fb + 8 NS; advanced by addition, reset when the ring wraps
+  uint32_t fb = full0;
+  const uint32_t fb_end = full0 + 8u * (uint32_t)NS, stage_bytes = (uint32_t)kRPS * row_bytes;
   uint32_t ph = 0;
 
   for (int a0 = 0; a0 < n_sft; a0 += 32) {
@@ -560,28 +569,23 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
     sts_u32(etab + 4u * (uint32_t)lane, entry);
     if (G::ROWW) {
       float uf = 0.f;
-      if (a0 + lane < n_sft) {
-        const double u = ft_antenna_u(d.ant + 9 * (size_t)(a0 + lane), skyp);   // a^2 + b^2 (Eq. 4)
-        uf = (float)u;
-        const double ur = __dmul_rn((double)uf, (double)d.w[a0 + lane]);
-        w_sum = __dadd_rn(w_sum, ur);
-        w_sq = __dadd_rn(w_sq, __dmul_rn(ur, ur));
-        w_cb = __dadd_rn(w_cb, __dmul_rn((double)uf, (double)a.c_row[a0 + lane]));
-      }
+      if (a0 + lane < n_sft) uf = (float)ft_antenna_u(d.ant + 9 * (size_t)(a0 + lane), *skyp);   // a^2 + b^2 (Eq. 4)
       sts_u32(wtab + 4u * (uint32_t)lane, __float_as_uint(uf));
     }
     __syncwarp();
-    // -- A4: gather + reduce over the block's SFTs -----------------------------------------------
+    // -- A4: gather + reduce over the block's SFTs, one ring stage (kRPS rows) at a time ------------
     const int n_rows = min(32, n_sft - a0);
-    for (int q = 0; q < n_rows; q += kRPS) {
+    // `rows` = kRPS for the full stages of the block (the loop below walks the entry table by pointer, so a stage
+    // costs no index arithmetic); the ragged last stage of the last block comes after it
+    auto stage = [&](uint32_t ep, int rows) {
       uint32_t e4[kRPS], u4[kRPS];
       asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                   : "=r"(e4[0]), "=r"(e4[1]), "=r"(e4[2]), "=r"(e4[3]) : "r"(etab + 4u * (uint32_t)q));
+                   : "=r"(e4[0]), "=r"(e4[1]), "=r"(e4[2]), "=r"(e4[3]) : "r"(ep));
       if (G::ROWW)
         asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                     : "=r"(u4[0]), "=r"(u4[1]), "=r"(u4[2]), "=r"(u4[3]) : "r"(wtab + 4u * (uint32_t)q));
-      mbar_wait(full0 + 8 * s, ph);
-      if (q + kRPS <= n_rows && (e4[0] | e4[1] | e4[2] | e4[3]) < 8192u) {
+                     : "=r"(u4[0]), "=r"(u4[1]), "=r"(u4[2]), "=r"(u4[3]) : "r"(ep + 128u * (uint32_t)n_cw));
+      mbar_wait(fb, ph);
+      if (rows == kRPS && (e4[0] | e4[1] | e4[2] | e4[3]) < 8192u) {
         // a full stage and no break in this warp's range in any of its rows (the common case): straight-line body
         if constexpr (G::PAIRS) {
           G::template rows_fast_pair<J>(st, e4[0], e4[1], stage_addr, stage_addr + row_bytes, copy_pitch, last_ok);
@@ -595,7 +599,7 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
       } else {
 #pragma unroll
         for (int r = 0; r < kRPS; ++r) {
-          if (q + r < n_rows) {
+          if (r < rows) {
             const uint32_t e = e4[r];
             const uint32_t base = stage_addr + (uint32_t)r * row_bytes;
             const float u = G::ROWW ? __uint_as_float(u4[r]) : 1.f;
@@ -605,9 +609,13 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
         }
       }
       __syncwarp();
-      if (lane == 0) mbar_arrive(empty0 + 8 * s);
-      if (++s == NS) { s = 0; ph ^= 1u; stage_addr = lane_bytes; } else { stage_addr += kRPS * row_bytes; }
-    }
+      if (lane == 0) mbar_arrive(fb + 8u * (uint32_t)NS);
+      fb += 8u; stage_addr += stage_bytes;
+      if (fb == fb_end) { fb = full0; ph ^= 1u; stage_addr = lane_bytes; }
+    };
+    const uint32_t ep_end = etab + 4u * (uint32_t)(n_rows & ~(kRPS - 1));
+    for (uint32_t ep = etab; ep != ep_end; ep += 4u * kRPS) stage(ep, kRPS);
+    if (n_rows & (kRPS - 1)) stage(ep_end, n_rows & (kRPS - 1));
     G::template block_end<J>(st, a0 / 32 + 1);
   }
 
@@ -619,11 +627,8 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
   double add_back = a.add_back, scale = 1.0, z_mu = a.z_mu, z_is = a.z_inv_sigma;
   if (G::ROWW) {
     // Eq. (5): the weights of this point are u_a r_a / sum_b u_b r_b; sigma_G^2 = sum w^2 (Eq. 14 on the P = s/2 scale)
-    for (int o = 16; o > 0; o >>= 1) {
-      w_sum += __shfl_xor_sync(0xffffffffu, w_sum, o);
-      w_sq += __shfl_xor_sync(0xffffffffu, w_sq, o);
-      w_cb += __shfl_xor_sync(0xffffffffu, w_cb, o);
-    }
+    const uint64_t i_sky = pt / ((uint64_t)d.n_ap * (uint64_t)d.n_porb * (uint64_t)d.n_tasc * (uint64_t)d.n_f1);
+    const double w_sum = a.sky_norm[4 * i_sky], w_sq = a.sky_norm[4 * i_sky + 1], w_cb = a.sky_norm[4 * i_sky + a.norm_cb];
     add_back = w_cb;
     scale = 1.0 / w_sum;
     const double sigma = sqrt(w_sq) * scale;
