@@ -267,11 +267,15 @@ typedef enum {
                                veto of :496-502; for uniform weights the paper's weighted-count floor times n_sft) */
   FT_OPT_ONE_PASS_BOTH = 7, /* 1 (default): narrow bands compute both statistics in one gather (hit bit in the LSB of
                                the folded pixel); 0: one pass per statistic */
-  FT_OPT_WCOUNT_FLOOR = 8   /* ft_set_option_f64: 0 off (default); x > 0: with FT_STAT_BOTH bound, the selection keeps the
+  FT_OPT_WCOUNT_FLOOR = 8,  /* ft_set_option_f64: 0 off (default); x > 0: with FT_STAT_BOTH bound, the selection keeps the
                                loudest normalized power among templates whose WEIGHTED number count sum_a w_a [P > rho_th]
                                is >= x -- the veto as the paper states it (:496-502; "three standard deviations above
                                the average number count in Gaussian noise": x = p sum w + 3 sqrt(p (1 - p) sum w^2),
                                p = exp(-rho_th)).  Costs one weighted-count pass over the bank. */
+  FT_OPT_VETO_FIRST = 9     /* 1 (default): with a floor set, the number-count pass runs first with the floor as its fused
+                               filter; if its survivors fit the candidate buffers (a floor of mu + 3 sigma leaves ~1e-3 of a
+                               noise bank) only they are evaluated for power and the bank-wide power pass is skipped.
+                               0: always both bank-wide passes.  Same candidates either way. */
 } ft_option;
 int ft_set_option(ft_ctx* ctx, int option, int64_t value);
 int ft_set_option_f64(ft_ctx* ctx, int option, double value);

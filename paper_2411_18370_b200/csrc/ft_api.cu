@@ -214,6 +214,7 @@ int ft_set_option(ft_ctx* c, int option, int64_t value) {
     case FT_OPT_SELECT_CAP: if (value < 0 || value > (1 << 20)) return ft_fail(c, FT_ERR_ARG, "FT_OPT_SELECT_CAP: 0 .. 2^20"); c->opt_cap = value; break;
     case FT_OPT_COUNT_FLOOR: if (value < 0 || value > (1 << 24)) return ft_fail(c, FT_ERR_ARG, "FT_OPT_COUNT_FLOOR: 0 .. 2^24"); c->opt_floor = value; break;
     case FT_OPT_ONE_PASS_BOTH: c->opt_onepass = value ? 1 : 0; break;
+    case FT_OPT_VETO_FIRST: c->opt_veto_first = value ? 1 : 0; break;
     case FT_OPT_F0_TILES: if (value < 0) return ft_fail(c, FT_ERR_ARG, "FT_OPT_F0_TILES >= 0"); c->opt_tiles = value; break;
     case FT_OPT_POINTS_PER_CTA: if (value < 0) return ft_fail(c, FT_ERR_ARG, "FT_OPT_POINTS_PER_CTA >= 0"); c->opt_ppc = value; break;
     default: return ft_fail(c, FT_ERR_ARG, "unknown option");
@@ -509,7 +510,7 @@ void ft_destroy(ft_ctx* c) {
   ft_dfree(c->t_mid_dev); ft_dfree(c->vel_dev); ft_dfree(c->w_dev); ft_dfree(c->Q_dev); ft_dfree(c->H_dev);
   ft_dfree(c->ctab_dev); ft_dfree(c->axes_dev); ft_dfree(c->w_row_dev); ft_dfree(c->ant_dev); ft_dfree(c->vr_dev);
   ft_dfree(c->skyn_dev); ft_dfree(c->maxw_dev); ft_dfree(c->scratch_f); ft_dfree(c->scratch_i); ft_dfree(c->veto_cnt); ft_dfree(c->veto_w);
-  ft_dfree(c->glist_dev); ft_dfree(c->pbox_dev); ft_dfree(c->io_dev); ft_dfree(c->near_ties_dev); ft_dfree(c->flag_dev);
+  ft_dfree(c->surv_dev); ft_dfree(c->glist_dev); ft_dfree(c->pbox_dev); ft_dfree(c->io_dev); ft_dfree(c->near_ties_dev); ft_dfree(c->flag_dev);
   ft_dfree(c->tile_err_dev);
   for (cudaEvent_t e : c->evs) cudaEventDestroy(e);
   delete c;

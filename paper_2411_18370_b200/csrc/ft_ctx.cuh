@@ -62,7 +62,8 @@ struct ft_ctx {
   uint8_t* H8_dev = nullptr;    // four byte-shifted hit maps
   float H8_rho = 0.f; bool H8_valid = false;
   // options
-  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0, opt_cap = 0, opt_floor = 0, opt_onepass = 1;
+  int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0, opt_cap = 0, opt_floor = 0, opt_onepass = 1,
+          opt_veto_first = 1;
   double opt_wfloor = 0.0;
   // selection buffers
   FtSelectDev sel{};
@@ -79,6 +80,8 @@ struct ft_ctx {
   int32_t* veto_cnt = nullptr;  // number count of every template (FT_OPT_COUNT_FLOOR), grow-only
   float* veto_w = nullptr;      // weighted number count of every template (FT_OPT_WCOUNT_FLOOR), grow-only
   size_t veto_cap = 0, vetow_cap = 0;
+  unsigned char* surv_dev = nullptr;  // veto-first selection: refined records | idx list | region offsets (grow-only)
+  size_t surv_cap = 0;
   uint32_t* glist_dev = nullptr; // sample group list | skip bitmask | pbox row lists (grow-only)
   size_t glist_cap = 0;
   int32_t* pbox_dev = nullptr;

@@ -144,6 +144,50 @@ ft_refine_kernel(const __grid_constant__ FtDev d, const uint64_t* __restrict__ i
   }
 }
 
+// Long candidate lists (the survivors of a number-count veto, ft_topk.cu): ONE THREAD per candidate walks the SFTs
+// in ascending order, so the sums have the oracle's rounding sequence without the 32-fold redundancy of the
+// warp-per-candidate form (which is the faster one for the few hundred candidates of a plain top-k).
+__global__ void __launch_bounds__(128)
+ft_refine_thread_kernel(const __grid_constant__ FtDev d, const uint64_t* __restrict__ idx_list, int64_t n,
+                        FtCandDev* __restrict__ out, unsigned long long* __restrict__ near_ties) {
+  const int64_t cand = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cand >= n) return;
+  const uint64_t idx = idx_list[cand];
+  const uint64_t pt = idx / (uint64_t)d.n_f0;
+  const FtPoint p = ft_decode_point(d, pt);
+  const double f0 = ft_f0(d, (int64_t)(idx % (uint64_t)d.n_f0));
+  double power = 0.0, wcount = 0.0, wsum = 0.0, wsq = 0.0;
+  int32_t count = 0;
+  unsigned ties = 0;
+  FtSkyPoint sk;
+  if (d.skyw) sk = ft_sky_point(p.nx, p.ny, p.nz);
+  for (int64_t a = 0; a < d.n_sft; ++a) {
+    const double t = d.t_mid[a];
+    const double D = ft_doppler(d, p, a, t);
+    const double x = ft_track_x(f0, __dmul_rn(p.f1, __dsub_rn(t, d.t_ref)), D, d.f_min, d.inv_df);
+    ties += ft_near_tie(x) ? 1u : 0u;
+    const int64_t k = __double2ll_rn(x);
+    if (k < 0 || k >= d.n_bins || !(x == x)) continue;
+    const int64_t off = a * d.ld + k;
+    const float pix = __ldg(d.P + off);
+    double wa = (double)((d.wkind == 1) ? __ldg(d.w + a) : __ldg(d.w + off));
+    if (d.skyw) {
+      wa = __dmul_rn(ft_antenna_u(d.ant + 9 * a, sk), wa);
+      wsum = __dadd_rn(wsum, wa);
+      wsq = __dadd_rn(wsq, __dmul_rn(wa, wa));
+    }
+    power = __dadd_rn(power, __dmul_rn(wa, (double)pix));
+    if (pix > d.rho) { wcount = __dadd_rn(wcount, wa); ++count; }
+  }
+  double mu = d.mu_G, sigma = d.sigma_G;
+  if (d.skyw) { power = power / wsum; wcount = wcount / wsum; mu = 1.0; sigma = sqrt(wsq) / wsum; }
+  FtCandDev c;
+  c.power = power; c.wcount = wcount; c.idx = idx; c.count = count; c.band = -1;   // (bad cannot happen: the grid was validated at bind)
+  c.sigma = sigma; c.z = (power - mu) / sigma;
+  out[cand] = c;
+  if (ties && near_ties) atomicAdd(near_ties, (unsigned long long)ties);
+}
+
 // The same for ONE explicit template (a record of 8 doubles), optionally with its bins: ft_track, ft_eval_bank.
 __global__ void __launch_bounds__(32)
 ft_refine_template_kernel(const __grid_constant__ FtDev d, const double* __restrict__ tp, double t_ref,
@@ -208,6 +252,10 @@ cudaError_t ft_launch_generic(const FtDev& d, int stat, uint64_t pt_begin, uint6
 cudaError_t ft_launch_refine(const FtDev& d, const uint64_t* idx_dev, const uint32_t* n_dev, int64_t n_max,
                              FtCandDev* out, unsigned long long* near_ties, cudaStream_t s) {
   if (n_max <= 0) return cudaSuccess;
+  if (!n_dev && n_max >= 8192) {   // a long list of known length: one thread per candidate
+    ft_refine_thread_kernel<<<(unsigned)((n_max + 127) / 128), 128, 0, s>>>(d, idx_dev, n_max, out, near_ties);
+    return cudaGetLastError();
+  }
   const int64_t warps_per_block = 4;
   const unsigned grid = (unsigned)((n_max + warps_per_block - 1) / warps_per_block);
   ft_refine_kernel<<<grid, 128, 0, s>>>(d, idx_dev, n_dev, n_max, out, near_ties);

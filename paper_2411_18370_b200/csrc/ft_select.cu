@@ -215,6 +215,46 @@ ft_rank_kernel(const FtCandDev* __restrict__ cand, const int32_t* __restrict__ c
   }
 }
 
+// Veto-first selection (ft_topk.cu): every appended entry of every region, compacted region by region into one list
+// (off[b] = first slot of region b; the host computed it from the append counters).
+__global__ void __launch_bounds__(256)
+ft_take_all_kernel(FtSelectDev sel, const uint32_t* __restrict__ off, uint64_t* __restrict__ list_idx) {
+  const int b = blockIdx.x;
+  const uint32_t n = min(sel.cnt[b], sel.cap), o = off[b];
+  const uint64_t* idxs = sel.idx + (size_t)b * sel.cap;
+  for (uint32_t e = blockIdx.y * blockDim.x + threadIdx.x; e < n; e += gridDim.y * blockDim.x) list_idx[o + e] = idxs[e];
+}
+
+// Per region: among the refined candidates cand[off[b] .. off[b+1]) that pass the exact floors, the k-th largest
+// ranking value as an fp32 key (the cast is monotone, so everything >= it is a superset of the top k); those are
+// copied to out_cand / out_region (the input of ft_rank_kernel).
+__global__ void __launch_bounds__(SEL_THREADS)
+ft_trim_refined_kernel(const FtCandDev* __restrict__ cand, const uint32_t* __restrict__ off, int rank_by, uint32_t k,
+                       int32_t count_floor, double wcount_floor, FtCandDev* __restrict__ out_cand,
+                       int32_t* __restrict__ out_region, uint32_t* __restrict__ out_n, uint32_t out_cap) {
+  __shared__ uint32_t hist[256];
+  __shared__ uint32_t bcast[2];
+  const int b = blockIdx.x;
+  const FtCandDev* seg = cand + off[b];
+  const int64_t n = (int64_t)(off[b + 1] - off[b]);
+  auto get = [&](int64_t e) {
+    const FtCandDev& c = seg[e];
+    if (c.count < count_floor || !(c.wcount >= wcount_floor)) return -INFINITY;
+    const double v = rank_by == FT_RANK_COUNT ? (double)c.count : rank_by == FT_RANK_WCOUNT ? c.wcount
+                   : rank_by == FT_RANK_Z ? c.z : c.power;
+    return (float)v;
+  };
+  const uint32_t kk = block_kth_largest(n, k, get, hist, bcast);
+  const float t = (kk == 0u) ? -INFINITY : ft_unkey(kk);   // fewer than k pass: keep every one that does
+  for (int64_t e = threadIdx.x; e < n; e += blockDim.x) {
+    const float v = get(e);
+    if (v > -INFINITY && v >= t) {
+      const uint32_t slot = atomicAdd(out_n, 1u);
+      if (slot < out_cap) { out_cand[slot] = seg[e]; out_region[slot] = b; }
+    }
+  }
+}
+
 // keys[e] = -inf where the element's own number count (same layout) is below the floor
 __global__ void ft_mask_keys_local_kernel(float* __restrict__ keys, const int32_t* __restrict__ counts, int64_t n, int32_t floor) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -281,6 +321,19 @@ cudaError_t ft_select_rank(const FtCandDev* cand, const int32_t* cand_region, co
                            uint32_t cap, int rank_by, uint32_t k, int32_t n_regions, int32_t count_floor,
                            double wcount_floor, FtCandDev* out, uint32_t* overflow, cudaStream_t s) {
   ft_rank_kernel<<<n_regions, SEL_THREADS, 0, s>>>(cand, cand_region, n_dev, cap, rank_by, k, count_floor, wcount_floor, out, overflow);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_select_take_all(FtSelectDev sel, const uint32_t* off, uint64_t* list_idx, cudaStream_t s) {
+  ft_take_all_kernel<<<dim3((unsigned)sel.n_regions, 8), 256, 0, s>>>(sel, off, list_idx);
+  return cudaGetLastError();
+}
+
+cudaError_t ft_select_trim_refined(const FtCandDev* cand, const uint32_t* off, int32_t n_regions, int rank_by, uint32_t k,
+                                   int32_t count_floor, double wcount_floor, FtCandDev* out_cand, int32_t* out_region,
+                                   uint32_t* out_n, uint32_t out_cap, cudaStream_t s) {
+  ft_trim_refined_kernel<<<n_regions, SEL_THREADS, 0, s>>>(cand, off, rank_by, k, count_floor, wcount_floor, out_cand, out_region,
+                                                            out_n, out_cap);
   return cudaGetLastError();
 }
 

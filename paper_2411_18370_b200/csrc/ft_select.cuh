@@ -69,6 +69,12 @@ cudaError_t ft_select_trim(FtSelectDev sel, uint32_t k, FtMargin margin, uint64_
 cudaError_t ft_select_rank(const FtCandDev* cand, const int32_t* cand_region, const uint32_t* n_dev,
                            uint32_t cap, int rank_by, uint32_t k, int32_t n_regions, int32_t count_floor,
                            double wcount_floor, FtCandDev* out, uint32_t* overflow, cudaStream_t s);
+// veto-first selection: all appended entries compacted by region (off [n_regions + 1], device); then, on the refined
+// values, the candidates of each region that pass the floors and reach its k-th largest ranking value
+cudaError_t ft_select_take_all(FtSelectDev sel, const uint32_t* off, uint64_t* list_idx, cudaStream_t s);
+cudaError_t ft_select_trim_refined(const FtCandDev* cand, const uint32_t* off, int32_t n_regions, int rank_by, uint32_t k,
+                                   int32_t count_floor, double wcount_floor, FtCandDev* out_cand, int32_t* out_region,
+                                   uint32_t* out_n, uint32_t out_cap, cudaStream_t s);
 cudaError_t ft_count_to_key(const int32_t* c, float* k, int64_t n, cudaStream_t s);
 cudaError_t ft_select_tighten(FtSelectDev sel, uint32_t k, FtMargin margin, cudaStream_t s);
 cudaError_t ft_fill_f32(float* p, int64_t n, float v, cudaStream_t s);

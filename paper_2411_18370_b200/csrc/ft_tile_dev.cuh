@@ -45,14 +45,23 @@ struct FtTileArgs {
 // Threads per CTA the kernels are compiled for: (consumer warps + 1 producer warp) * 32.  The accumulators
 // (J) and the loads in flight (J) set the register need, hence the bound.
 // (the register file is 4 x 16 384: 80 registers allow 6 warps per SM sub-partition, 72 allow 7, 64 allow 8)
-__host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : 72; }
-__host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 1024 : 896; }
+#ifndef FT_TILE_BATCH
+#define FT_TILE_BATCH 0
+#endif
+#ifndef FT_TILE_REGS
+#define FT_TILE_REGS 72
+#endif
+__host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : FT_TILE_REGS; }
+__host__ __device__ constexpr int ft_tile_max_threads(int J) { return (J <= 12 || FT_TILE_REGS <= 64) ? 1024 : 896; }
 // packed number-count kernel: J registers of 8-bit counters + J loads in flight (16-bit levels in shared memory)
 __host__ __device__ constexpr int ft_tile8_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tile8_max_threads(int J) { return J <= 8 ? 1024 : 768; }
 // both statistics in one pass: J accumulators + J counters + J loads in flight
-__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : 80; }
-__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : 768; }
+#ifndef FT_TILEB_REGS
+#define FT_TILEB_REGS 80
+#endif
+__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : FT_TILEB_REGS; }
+__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : (FT_TILEB_REGS <= 72 ? 896 : 768); }
 // row-weighted gather: as the plain gather (the sky-point tables live in shared memory, the normalisation sums come
 // from a bind-time pass)
 __host__ __device__ constexpr int ft_tilew_max_regs(int J) { return ft_tile_max_regs(J); }
@@ -78,12 +87,22 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// Wait for a phase of an mbarrier.  With the suspend-time hint the warp sleeps in hardware until the phase completes
+// (SASS: one TRYWAIT, then a blocking PHASECHK) instead of spinning on TRYWAIT + BRA in the issue slots the other
+// warps need.
+#ifndef FT_WAIT_HINT
+#define FT_WAIT_HINT 1
+#endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
       "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 0x989680;\n"   // suspend-time hint: sleep in hardware, not in a spin loop
+#if FT_WAIT_HINT
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 0x989680;\n"
+#else
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+#endif
       "@p bra DONE_%=;\n"
       "bra WAIT_%=;\n"
       "DONE_%=:\n"
@@ -212,17 +231,27 @@ struct GatherF32 {
     const int64_t src = (int64_t)row * d.ld + k0;
     return 4u * (uint32_t)min((int64_t)a.copy_floats, d.n_sft * d.ld - src);
   }
+  // Loads in flight per row: all J of them, or (FT_TILE_BATCH > 0, J > 16) batches of FT_TILE_BATCH so that wide
+  // tiles fit 64 registers and one more consumer warp per scheduler
   template <int J> static __device__ __forceinline__ void row_fast(State<J>& st, uint32_t e, uint32_t base, uint32_t,
                                                                    bool last_ok, float) {
     const uint32_t ad = base + 4u * e;
-    float v[J];
+    constexpr int B = (FT_TILE_BATCH > 0 && J > 16) ? FT_TILE_BATCH : ((J + 1) & ~1);   // even
 #pragma unroll
-    for (int j = 0; j < J; ++j)
-      if (j < J - 1 || last_ok) v[j] = lds_f32(ad + 128u * j);
-    if (!last_ok) v[J - 1] = 0.f;
+    for (int h0 = 0; h0 < J; h0 += B) {
+      float v[B];
 #pragma unroll
-    for (int j = 0; j + 1 < J; j += 2) ft_add2(st.acc[j], st.acc[j + 1], v[j], v[j + 1]);
-    if (J & 1) st.acc[J - 1] += v[J - 1];
+      for (int i = 0; i < B; ++i) {
+        const int j = h0 + i;
+        if (j < J) v[i] = (j < J - 1 || last_ok) ? lds_f32(ad + 128u * j) : 0.f;
+      }
+#pragma unroll
+      for (int i = 0; i < B; i += 2) {
+        const int j = h0 + i;
+        if (j + 1 < J) ft_add2(st.acc[j], st.acc[j + 1], v[i], v[i + 1]);
+        else if (j < J) st.acc[j] += v[i];
+      }
+    }
   }
   template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t,
                                                                     int lane, float) {
@@ -271,8 +300,14 @@ struct GatherF32W : GatherF32 {
 // sum count the hits of up to 63 rows (carries only travel upwards), so they are folded into 16-bit counters once
 // per block of 32 SFTs.  The pixel is rounded to 18 mantissa bits (<= 3.8e-6 of |q| per pixel, random sign:
 // ~3e-8 of the statistic at n_sft = 8000; the plan keeps this kernel to 64 <= n_sft <= 65535).
+#ifndef FT_PAIRS_B
+#define FT_PAIRS_B 1
+#endif
+#ifndef FT_K2B_SKIP
+#define FT_K2B_SKIP 0   // timing experiments only (wrong results): 1 no fp32 adds, 2 no integer adds
+#endif
 struct GatherBoth : GatherF32 {
-  static constexpr bool VETO = true, HASCNT = true, PAIRS = true;
+  static constexpr bool VETO = true, HASCNT = true, PAIRS = FT_PAIRS_B != 0;
   static constexpr uint32_t kLowMask = 63u;
   template <int J> struct State { float acc[J]; uint32_t raw[J]; uint32_t c16[(J + 1) / 2]; };
   template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t, uint32_t) {
@@ -317,6 +352,10 @@ struct GatherBoth : GatherF32 {
 #pragma unroll
       for (int i = 0; i < H; i += 2) {
         const int j = h0 + i;
+#if FT_K2B_SKIP == 1
+        if (j < J) st.acc[j] = v0[i];
+        continue;
+#endif
         if (j + 1 < J) {
           ft_add2(st.acc[j], st.acc[j + 1], v0[i], v0[i + 1]);
           ft_add2(st.acc[j], st.acc[j + 1], v1[i], v1[i + 1]);
@@ -328,6 +367,10 @@ struct GatherBoth : GatherF32 {
 #pragma unroll
       for (int i = 0; i < H; ++i) {
         const int j = h0 + i;
+#if FT_K2B_SKIP == 2
+        if (j < J) st.raw[j] = __float_as_uint(v1[i]);
+        continue;
+#endif
         if (j < J) {
           uint32_t r = st.raw[j];
           asm("{\n.reg .u32 t;\nadd.u32 t, %1, %2;\nadd.u32 %0, %0, t;\n}" : "+r"(r) : "r"(__float_as_uint(v0[i])), "r"(__float_as_uint(v1[i])));

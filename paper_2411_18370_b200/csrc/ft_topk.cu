@@ -137,30 +137,80 @@ int topk_regions(ft_ctx* c, const TopkSpec& sp, std::vector<FtCandDev>* out, int
   const bool onepass_veto = floor > 0 && fused && c->tileb_ok;
   if (onepass_veto) c->sel.veto_floor = floor;
   const uint64_t n_templates = d.n_points * (uint64_t)d.n_f0;
+  const int rank_by_v = by_count ? FT_RANK_COUNT : by_wcount ? FT_RANK_WCOUNT : zmode ? FT_RANK_Z : FT_RANK_POWER;
+  bool by_survivors = false;   // veto-first: the selection was made from the survivors of the number-count pass
   if ((floor > 0 && !onepass_veto) || wfloor > 0.0) {
     if (n_templates > ((uint64_t)1 << 34)) return ft_fail(c, FT_ERR_ALLOC, "top-k: a number-count floor needs 4 B per template (bank too large)");
+    // Veto first (FT_OPT_VETO_FIRST, default on, fused selection): the LAST number-count pass also runs the fused filter
+    // with the floor as the threshold of every region.  A floor of mu + 3 sigma leaves ~1e-3 of a noise bank: if the
+    // survivors fit the append buffers, only they are evaluated for power (fp64, the refinement kernel) and the
+    // bank-wide power pass is not needed.  Otherwise the pass has still written the veto array and the selection goes
+    // on as before (power pass with the array looked up by the fused filter).
+    const bool try_first = fused && c->opt_veto_first;
     FtPass p;
     p.pt_begin = 0; p.pt_end = d.n_points;
+    p.bpb = (int32_t)bpb; p.n_bands = n_bands; p.pbox = pbox_dev;
     if (floor > 0 && !onepass_veto) {
       FT_CUDA(c, ft_grow(c->veto_cnt, c->veto_cap, (size_t)n_templates));
       p.stat = FT_STAT_HOUGH; p.out_i = c->veto_cnt; p.out_f = nullptr;
+      p.filter = try_first && !(wfloor > 0.0);
+      if (p.filter) { FT_CUDA(c, ft_fill_f32(c->sel.thr, n_regions, (float)floor, c->stream)); c->counters.kernel_launches += 1; }
       if ((rc = ft_run_stat(c, p)) != FT_OK) return rc;
       c->sel.veto_cnt = c->veto_cnt; c->sel.veto_floor = floor;
     }
     if (wfloor > 0.0) {
       FT_CUDA(c, ft_grow(c->veto_w, c->vetow_cap, (size_t)n_templates));
       p.stat = FT_STAT_WHOUGH; p.out_f = c->veto_w; p.out_i = nullptr;
-      if ((rc = ft_run_stat(c, p)) != FT_OK) return rc;
       // the fp32 weighted count decides only outside a 4e-5 band around the floor; inside, the fp64 refinement does
+      const float wlo = (float)(wfloor * (1.0 - 4e-5)), whi = (float)(wfloor * (1.0 + 4e-5));
+      p.filter = try_first;
+      if (p.filter) { FT_CUDA(c, ft_fill_f32(c->sel.thr, n_regions, wlo, c->stream)); c->counters.kernel_launches += 1; }
+      if ((rc = ft_run_stat(c, p)) != FT_OK) return rc;   // (an integer floor set above is applied by the filter: that pass is complete)
       c->sel.veto_w = c->veto_w;
-      c->sel.veto_wlo = (float)(wfloor * (1.0 - 4e-5)); c->sel.veto_whi = (float)(wfloor * (1.0 + 4e-5));
+      c->sel.veto_wlo = wlo; c->sel.veto_whi = whi;
+    }
+    if (try_first) {
+      std::vector<uint32_t> cnt0(n_regions);
+      FT_CUDA(c, cudaMemcpyAsync(cnt0.data(), c->sel.cnt, sizeof(uint32_t) * n_regions, cudaMemcpyDeviceToHost, c->stream));
+      FT_CUDA(c, cudaStreamSynchronize(c->stream));
+      std::vector<uint32_t> off((size_t)n_regions + 1, 0u);
+      uint64_t total = 0;
+      bool fits = true;
+      for (int32_t b = 0; b < n_regions; ++b) { fits = fits && cnt0[b] <= c->sel.cap; total += cnt0[b]; off[(size_t)b + 1] = (uint32_t)std::min<uint64_t>(total, 0xffffffffu); }
+      if (fits && total < ((uint64_t)1 << 26)) {
+        by_survivors = true;
+        c->counters.appended = total;
+        // survivors: list | refined records | region offsets (grow-only)
+        const size_t need = sizeof(uint64_t) * (size_t)total + sizeof(FtCandDev) * (size_t)total + sizeof(uint32_t) * off.size() + 64;
+        FT_CUDA(c, ft_grow(c->surv_dev, c->surv_cap, need));
+        FtCandDev* s_cand = reinterpret_cast<FtCandDev*>(c->surv_dev);
+        uint64_t* s_idx = reinterpret_cast<uint64_t*>(s_cand + total);
+        uint32_t* s_off = reinterpret_cast<uint32_t*>(s_idx + total);
+        FT_CUDA(c, cudaMemcpyAsync(s_off, off.data(), sizeof(uint32_t) * off.size(), cudaMemcpyHostToDevice, c->stream));
+        if (total > 0) {
+          FT_CUDA(c, ft_select_take_all(c->sel, s_off, s_idx, c->stream));
+          FT_CUDA(c, ft_launch_refine(d, s_idx, nullptr, (int64_t)total, s_cand, c->near_ties_dev, c->stream));
+        }
+        FT_CUDA(c, ft_select_trim_refined(s_cand, s_off, n_regions, rank_by_v, (uint32_t)k, floor, wfloor, c->cand, c->final_region,
+                                          c->final_n, c->final_cap, c->stream));
+        FT_CUDA(c, ft_select_rank(c->cand, c->final_region, c->final_n, c->final_cap, rank_by_v, (uint32_t)k, n_regions, floor,
+                                  wfloor, c->out_dev, overflow, c->stream));
+        c->counters.kernel_launches += 4;
+        FT_CUDA(c, cudaStreamSynchronize(c->stream));   // (off is a local: the upload must have completed)
+      } else {
+        // too many survivors for the buffers: thresholds and counters back to the start, the veto arrays stay
+        FT_CUDA(c, ft_select_reset(c->sel, c->final_n, overflow, c->stream));
+        c->counters.kernel_launches += 1;
+      }
     }
   }
   const int pass_stat = onepass_veto ? (int)FT_STAT_BOTH : sel_stat;
   std::vector<uint32_t> cnt(n_regions);
   FtRowMap map{};
   map.pbox = pbox_dev; map.n_bands = n_bands; map.bpb = (int32_t)bpb; map.n_pbox = n_pbox; map.pt_end = d.n_points;
-  if (fused) {
+  if (by_survivors) {
+    // (selection complete: only the copies to the host remain)
+  } else if (fused) {
     // ---- Phase A: thresholds from a sample of CTA groups --------------------------------------------------
     const FtTilePlan& spl = pass_stat == FT_STAT_BOTH ? c->planb : (by_count && c->tile8_ok) ? c->plan8
                           : d.skyw ? c->planw : c->plan;   // the plan the statistic pass runs
@@ -290,11 +340,13 @@ int topk_regions(ft_ctx* c, const TopkSpec& sp, std::vector<FtCandDev>* out, int
       c->counters.kernel_launches += 2;
     }
   }
-  FT_CUDA(c, ft_select_trim(c->sel, (uint32_t)k, margin, c->final_idx, c->final_region, c->final_n, c->final_cap, overflow, c->stream));
-  FT_CUDA(c, ft_launch_refine(d, c->final_idx, c->final_n, c->final_cap, c->cand, c->near_ties_dev, c->stream));
-  FT_CUDA(c, ft_select_rank(c->cand, c->final_region, c->final_n, c->final_cap, rank_by, (uint32_t)k, n_regions, floor,
-                            wfloor, c->out_dev, overflow, c->stream));
-  c->counters.kernel_launches += 3;
+  if (!by_survivors) {
+    FT_CUDA(c, ft_select_trim(c->sel, (uint32_t)k, margin, c->final_idx, c->final_region, c->final_n, c->final_cap, overflow, c->stream));
+    FT_CUDA(c, ft_launch_refine(d, c->final_idx, c->final_n, c->final_cap, c->cand, c->near_ties_dev, c->stream));
+    FT_CUDA(c, ft_select_rank(c->cand, c->final_region, c->final_n, c->final_cap, rank_by, (uint32_t)k, n_regions, floor,
+                              wfloor, c->out_dev, overflow, c->stream));
+    c->counters.kernel_launches += 3;
+  }
   uint32_t fin[2] = {0, 0};
   int32_t terr = 0;
   out->resize((size_t)n_regions * k);
@@ -304,10 +356,12 @@ int topk_regions(ft_ctx* c, const TopkSpec& sp, std::vector<FtCandDev>* out, int
   FT_CUDA(c, cudaMemcpyAsync(out->data(), c->out_dev, sizeof(FtCandDev) * (size_t)n_regions * k, cudaMemcpyDeviceToHost, c->stream));
   FT_CUDA(c, cudaStreamSynchronize(c->stream));
   if (int rc2 = ft_tile_err_status(c, terr)) return rc2;
-  uint64_t appended = 0;
-  for (uint32_t v : cnt) appended += v;
-  c->counters.appended = appended;
-  c->counters.refined = fin[0];
+  if (!by_survivors) {
+    uint64_t appended = 0;
+    for (uint32_t v : cnt) appended += v;
+    c->counters.appended = appended;
+  }
+  c->counters.refined = by_survivors ? c->counters.appended : fin[0];
   if (fin[1] != 0 || fin[0] > c->final_cap) {
     char buf[200];
     std::snprintf(buf, sizeof buf, "top-k: candidate buffers overflowed (%u attempts in one region / %u refined): too many exact ties at the k-th value", fin[1], fin[0]);

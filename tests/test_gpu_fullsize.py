@@ -253,6 +253,84 @@ def test_config3_full_size_number_count_veto():
     ctx.close()
 
 
+@pytest.mark.parametrize("weighted", [True, False])
+def test_veto_first_long_survivor_list_against_the_oracle(weighted):
+    """Wide band (1 Hz at 200 Hz, config 2's spectrogram, 300 sky points = 2.7e6 templates) with a floor of mean +
+    1 sigma: ~16 % of the bank survives the number-count pass (4e5 templates, evaluated for power one thread per
+    candidate).  Oracle-exhaustive: the plain per-band sort of the masked full power array; refined values
+    bit-identical; and the same candidates from the two bank-wide passes (FT_OPT_VETO_FIRST = 0)."""
+    from paper_2411_18370_b200 import binding as B
+    wl = W.config2(n_sky=300)
+    g = wl.grid
+    o = fo.Oracle(wl)
+    op, oc, owc, _ = o.eval_range()
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    p_hit = float(np.exp(-wl.rho_th))
+    w = wl.w.astype(np.float64)
+    if weighted:
+        floor = p_hit * w.sum() + 1.0 * np.sqrt(p_hit * (1 - p_hit) * (w ** 2).sum())
+        keep = owc >= floor
+    else:
+        floor = int(np.ceil(wl.n_sft * p_hit + 1.0 * np.sqrt(wl.n_sft * p_hit * (1 - p_hit))))
+        keep = oc >= floor
+    assert 0.05 < keep.mean() < 0.3 and keep.sum() > 100_000
+    ref = fo.topk_per_region(op, g.n_f0, bpb, wl.k, keep=keep)
+    ctx = H.gpu_context(wl)
+    if weighted:
+        ctx.set_option_f64(B.FT_OPT_WCOUNT_FLOOR, floor)
+    else:
+        ctx.set_option(B.FT_OPT_COUNT_FLOOR, floor)
+    got = {}
+    for first in (1, 0):
+        ctx.set_option(B.FT_OPT_VETO_FIRST, first)
+        ctx.eval(g, "both", wl.rho_th)
+        cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+        c = ctx.counters()
+        assert (c["stat_launches"] == 1) == (first == 1), c
+        if first:
+            assert c["refined"] > 100_000      # the survivors, not a top-k superset
+        H.assert_region_parity(cands, ref, op, {"power": op, "count": oc, "wcount": owc})
+        got[first] = cands
+    assert np.array_equal(got[0]["idx"], got[1]["idx"]) and np.array_equal(got[0]["power"], got[1]["power"])
+    ctx.close()
+
+
+def test_config2_full_size_weighted_count_veto_first():
+    """Config 2 at full size under the paper's floor (weighted count three sigma above its Gaussian-noise mean,
+    PAPER.md:502), in the launch configuration bench.py's `extra` times: the number-count pass alone, then its
+    survivors (~2e5).  Every candidate re-evaluated by the oracle (bit-identical power / weighted count, floor
+    respected, ordered), and the same candidates as the two bank-wide passes."""
+    from paper_2411_18370_b200 import binding as B
+    wl = _full(2)
+    g = wl.grid
+    o = fo.Oracle(wl)
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    p_hit = float(np.exp(-wl.rho_th))
+    w = wl.w.astype(np.float64)
+    floor = p_hit * w.sum() + 3.0 * np.sqrt(p_hit * (1 - p_hit) * (w ** 2).sum())
+    ctx = H.gpu_context(wl)
+    ctx.set_option_f64(B.FT_OPT_WCOUNT_FLOOR, floor)
+    got = {}
+    for first in (1, 0):
+        ctx.set_option(B.FT_OPT_VETO_FIRST, first)
+        ctx.eval(g, "both", wl.rho_th)
+        got[first] = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+        assert (ctx.counters()["stat_launches"] == 1) == (first == 1)
+    assert np.array_equal(got[0]["idx"], got[1]["idx"]) and np.array_equal(got[0]["power"], got[1]["power"])
+    cands = got[1]
+    live = cands["idx"] != PAD
+    assert live.sum() > 0
+    flat = cands[live]
+    cp, cc, cw, _ = o.eval_list(flat["idx"])
+    assert np.array_equal(flat["power"], cp) and np.array_equal(flat["count"], cc) and np.array_equal(flat["wcount"], cw)
+    assert np.all(cw >= floor)
+    for b in range(n_bands):
+        c = cands[b][cands[b]["idx"] != PAD]
+        key = list(zip(-c["power"], c["idx"]))
+        assert key == sorted(key) and np.all((c["idx"] % np.uint64(g.n_f0)) // np.uint64(bpb) == b)
+    ctx.close()
+
+
 def test_tight_orbit_limits_chunks_per_warp():
     """a_p Omega = 3.6e-3 (10 lt-s at P_orb = 0.2 d): the shift drifts by a bin every ~270 f0, so the plan
     must keep a warp's range short (32 J |D - 1| < 0.45) for the single-break model to hold; parity with

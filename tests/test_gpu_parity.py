@@ -131,8 +131,14 @@ def test_errors_and_edge_cases():
     ctx.close()
 
 
-@pytest.mark.parametrize("cfg,kernel,fused", [(3, 0, 1), (3, 0, 0), (1, 0, 1), (2, 1, 0), (4, 0, 1)])
-def test_number_count_veto(cfg, kernel, fused):
+@pytest.mark.parametrize("cfg,kernel,fused,one_pass,veto_first,cap",
+                         [(3, 0, 1, 1, 1, 0), (3, 0, 0, 1, 1, 0), (1, 0, 1, 1, 1, 0), (2, 1, 0, 1, 1, 0), (4, 0, 1, 1, 1, 0),
+                          # the bank-wide count pass (one pass per statistic): veto first (the survivors of the count
+                          # pass alone are evaluated for power), both bank-wide passes, and veto first with buffers too
+                          # small for the survivors (falls back to both passes)
+                          (2, 0, 1, 0, 1, 0), (2, 0, 1, 0, 0, 0), (4, 0, 1, 0, 1, 0), (3, 0, 1, 0, 1, 0), (1, 0, 1, 0, 1, 0),
+                          (2, 0, 1, 0, 1, 24)])
+def test_number_count_veto(cfg, kernel, fused, one_pass, veto_first, cap):
     """per region, the loudest normalized power among templates scoring at least a
     pre-established number count.  Oracle: mask the full arrays, then the plain per-band sort."""
     from paper_2411_18370_b200 import binding as B
@@ -146,8 +152,15 @@ def test_number_count_veto(cfg, kernel, fused):
     ref = fo.topk_per_band(masked, wl.grid.n_f0, bpb, wl.k)
     ctx = H.gpu_context(wl, kernel=kernel, fused=fused)
     ctx.set_option(B.FT_OPT_COUNT_FLOOR, floor)
+    ctx.set_option(B.FT_OPT_ONE_PASS_BOTH, one_pass)
+    ctx.set_option(B.FT_OPT_VETO_FIRST, veto_first)
+    ctx.set_option(B.FT_OPT_SELECT_CAP, cap)
     ctx.eval(wl.grid, "both", wl.rho_th)
     cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    n_launch = ctx.counters()["stat_launches"]
+    if fused and not one_pass and kernel == 0:
+        # veto first: one bank-wide launch (the count pass); otherwise count pass + sample + fused power pass (+ repeats)
+        assert (n_launch == 1) == (veto_first == 1 and cap == 0), n_launch
     vetoed_some = False
     for b, (ridx, rval) in enumerate(ref):
         keep = np.isfinite(rval)
@@ -205,8 +218,9 @@ def test_weighted_count_statistic(cfg, kernel):
     ctx.close()
 
 
-@pytest.mark.parametrize("cfg,kernel,fused", [(2, 0, 1), (2, 0, 0), (2, 1, 0), (4, 0, 1), (3, 0, 1), (1, 0, 1)])
-def test_weighted_count_veto(cfg, kernel, fused):
+@pytest.mark.parametrize("cfg,kernel,fused,veto_first", [(2, 0, 1, 1), (2, 0, 0, 1), (2, 1, 0, 1), (4, 0, 1, 1), (3, 0, 1, 1), (1, 0, 1, 1),
+                                                         (2, 0, 1, 0), (4, 0, 1, 0)])
+def test_weighted_count_veto(cfg, kernel, fused, veto_first):
     """The veto as the paper states it: loudest normalized power among templates whose WEIGHTED number count is at
     least a floor (mean + sigma of the weighted count in Gaussian noise here, so that a good fraction is vetoed).
     The floor is then set EXACTLY on a template's own fp64 weighted count: the fp32 array cannot decide that
@@ -221,6 +235,7 @@ def test_weighted_count_veto(cfg, kernel, fused):
     wbar = w.mean(axis=1) if w.ndim == 2 else w
     floor0 = p_hit * wbar.sum() + 1.0 * np.sqrt(p_hit * (1 - p_hit) * (wbar ** 2).sum())
     ctx = H.gpu_context(wl, kernel=kernel, fused=fused)
+    ctx.set_option(B.FT_OPT_VETO_FIRST, veto_first)
     plain_ref = fo.topk_per_region(op, wl.grid.n_f0, bpb, wl.k)
     top_unvetoed = int(plain_ref[0][0][0])                      # the loudest template of band 0
     for floor in (floor0, float(owc[top_unvetoed]), float(np.nextafter(owc[top_unvetoed], 1.0))):
