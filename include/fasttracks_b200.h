@@ -272,10 +272,13 @@ typedef enum {
                                is >= x -- the veto as the paper states it (:496-502; "three standard deviations above
                                the average number count in Gaussian noise": x = p sum w + 3 sqrt(p (1 - p) sum w^2),
                                p = exp(-rho_th)).  Costs one weighted-count pass over the bank. */
-  FT_OPT_VETO_FIRST = 9     /* 1 (default): with a floor set, the number-count pass runs first with the floor as its fused
+  FT_OPT_VETO_FIRST = 9,    /* 1 (default): with a floor set, the number-count pass runs first with the floor as its fused
                                filter; if its survivors fit the candidate buffers (a floor of mu + 3 sigma leaves ~1e-3 of a
                                noise bank) only they are evaluated for power and the bank-wide power pass is skipped.
                                0: always both bank-wide passes.  Same candidates either way. */
+  FT_OPT_TAIL_PACKING = 10  /* 1 (default): a narrow band whose f0 count is 32 m + t with 1 <= t <= 16 runs two outer points
+                               per warp, their t-wide tails sharing one load (fewer shared-memory wavefronts); 0: one
+                               point per warp.  Same results bit for bit. */
 } ft_option;
 int ft_set_option(ft_ctx* ctx, int option, int64_t value);
 int ft_set_option_f64(ft_ctx* ctx, int option, double value);

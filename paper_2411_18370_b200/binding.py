@@ -12,7 +12,7 @@ from . import build as _build
 
 FT_STAT = {"power": 0, "hough": 1, "both": 2, "whough": 3}
 FT_OPT_KERNEL, FT_OPT_FUSED_TOPK, FT_OPT_POINTS_PER_CTA, FT_OPT_PACKED_COUNT, FT_OPT_F0_TILES = 0, 1, 2, 3, 4
-FT_OPT_SELECT_CAP, FT_OPT_COUNT_FLOOR, FT_OPT_ONE_PASS_BOTH, FT_OPT_WCOUNT_FLOOR, FT_OPT_VETO_FIRST = 5, 6, 7, 8, 9
+FT_OPT_SELECT_CAP, FT_OPT_COUNT_FLOOR, FT_OPT_ONE_PASS_BOTH, FT_OPT_WCOUNT_FLOOR, FT_OPT_VETO_FIRST, FT_OPT_TAIL_PACKING = 5, 6, 7, 8, 9, 10
 SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_topk_per_box", "ft_set_antenna", "ft_eval_list",
            "ft_eval_templates", "ft_bank_draw", "ft_eval_bank", "ft_track", "ft_set_option", "ft_set_option_f64",
            "ft_get_counters", "ft_measure_peaks", "ft_selftest", "ft_last_error", "ft_describe", "ft_destroy"]

@@ -215,6 +215,7 @@ int ft_set_option(ft_ctx* c, int option, int64_t value) {
     case FT_OPT_COUNT_FLOOR: if (value < 0 || value > (1 << 24)) return ft_fail(c, FT_ERR_ARG, "FT_OPT_COUNT_FLOOR: 0 .. 2^24"); c->opt_floor = value; break;
     case FT_OPT_ONE_PASS_BOTH: c->opt_onepass = value ? 1 : 0; break;
     case FT_OPT_VETO_FIRST: c->opt_veto_first = value ? 1 : 0; break;
+    case FT_OPT_TAIL_PACKING: c->opt_tail = value ? 1 : 0; break;
     case FT_OPT_F0_TILES: if (value < 0) return ft_fail(c, FT_ERR_ARG, "FT_OPT_F0_TILES >= 0"); c->opt_tiles = value; break;
     case FT_OPT_POINTS_PER_CTA: if (value < 0) return ft_fail(c, FT_ERR_ARG, "FT_OPT_POINTS_PER_CTA >= 0"); c->opt_ppc = value; break;
     default: return ft_fail(c, FT_ERR_ARG, "unknown option");
@@ -344,7 +345,7 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   const bool want_wh = stat == FT_STAT_WHOUGH || (stat == FT_STAT_BOTH && c->opt_wfloor > 0.0);
   c->tile_ok = c->tile8_ok = c->tileb_ok = c->tilew_ok = false;
   if (c->opt_kernel != 1) {
-    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc, (int)c->opt_tiles};
+    FtTileHostIn hin{c->t_mid.data(), c->vel.data(), g->sky, g->a_p, g->P_orb, c->df, eps, (int)c->opt_ppc, (int)c->opt_tiles, (int)c->opt_tail};
     std::string why8, whyb, whyw;
     bool t0 = ft_tile_choose(d, hin, 0, &c->plan, &c->why);
     bool t8 = t0 && stat != FT_STAT_POWER && c->opt_packed && ft_tile_choose(d, hin, 1, &c->plan8, &why8);
@@ -353,7 +354,7 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
     t8 = t8 && c->plan8.J >= 6;
     // both statistics in one pass only where the fp32 plan itself is narrow (J <= 16): wide bands run power on
     // K2 and the count packed
-    bool tb = t0 && stat == FT_STAT_BOTH && c->opt_onepass && !skyw && c->plan.J <= 16 &&
+    bool tb = t0 && stat == FT_STAT_BOTH && c->opt_onepass && !skyw && (c->plan.J <= 16 || c->plan.ppw == 2) &&
               ft_tile_choose(d, hin, 2, &c->planb, &whyb) && c->planb.n_tiles == c->plan.n_tiles;
     bool tw = t0 && skyw && ft_tile_choose(d, hin, 3, &c->planw, &whyw);
     if (t0) {
@@ -427,9 +428,9 @@ int ft_eval(ft_ctx* c, const ft_grid* g, int stat, double rho_th, float* out_pow
   {
     char buf[400];
     auto geom = [&](const FtTilePlan& pl) {
-      std::snprintf(buf, sizeof buf, "J=%d wpp=%d R=%d n_tiles=%d tile_w=%d threads=%d pitch=%d copy=%d stages=%dx%d smem=%zu",
-                    pl.J, pl.wpp, pl.R, pl.n_tiles, pl.tile_w, (pl.R * pl.wpp + 1) * 32, pl.pitch, pl.copy_floats,
-                    pl.n_stages, pl.rows_per_stage, pl.smem_bytes);
+      std::snprintf(buf, sizeof buf, "J=%d wpp=%d%s R=%d n_tiles=%d tile_w=%d threads=%d pitch=%d copy=%d stages=%dx%d smem=%zu",
+                    pl.J, pl.wpp, pl.ppw == 2 ? " (two points per warp)" : "", pl.R, pl.n_tiles, pl.tile_w,
+                    (pl.R * pl.wpp / pl.ppw + 1) * 32, pl.pitch, pl.copy_floats, pl.n_stages, pl.rows_per_stage, pl.smem_bytes);
       return std::string(buf);
     };
     if (c->tile_ok && c->opt_kernel != 1) c->desc = "K2 tile kernel: " + geom(c->plan);

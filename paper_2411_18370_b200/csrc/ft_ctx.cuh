@@ -63,7 +63,7 @@ struct ft_ctx {
   float H8_rho = 0.f; bool H8_valid = false;
   // options
   int64_t opt_kernel = 0, opt_fused = 1, opt_ppc = 0, opt_packed = 1, opt_tiles = 0, opt_cap = 0, opt_floor = 0, opt_onepass = 1,
-          opt_veto_first = 1;
+          opt_veto_first = 1, opt_tail = 1;
   double opt_wfloor = 0.0;
   // selection buffers
   FtSelectDev sel{};

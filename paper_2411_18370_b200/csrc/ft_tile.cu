@@ -232,6 +232,20 @@ bool ft_tile_choose(const FtDev& d, const FtTileHostIn& in, int mode, FtTilePlan
   R = std::min<int>(R, (max_threads / 32 - 1) / pl.wpp);  // + 1 producer warp
   R = (int)std::min<uint64_t>((uint64_t)R, d.n_points);
   pl.R = std::max(R, 1);
+  // Narrow band with a ragged tail (n_f0 = 32 JA + t, 1 <= t <= 16, one tile, one warp per point): two points per
+  // warp, their tails sharing one chunk (ft_tile2.cu): 2 JA + 1 loads per two (point, SFT) rows instead of 2 JA + 2
+  if (mode == 0 && in.tail_packing && pl.n_tiles == 1 && pl.wpp == 1 && d.n_points >= 2) {
+    const int JA = (int)(d.n_f0 / 32), t = (int)(d.n_f0 % 32);
+    if (JA >= 1 && JA <= 15 && t >= 1 && t <= 16 && JA + 1 <= maxJ_eps) {
+      pl.ppw = 2;
+      pl.J = 2 * JA + 1;
+      const int warps_max = ft_tile_max_threads(pl.J) / 32 - 1;
+      int warps = in.points_per_cta > 0 ? std::max(1, in.points_per_cta / 2) : std::min(27, warps_max);
+      warps = std::min(warps, warps_max);
+      warps = (int)std::min<uint64_t>((uint64_t)warps, (d.n_points + 1) / 2);
+      pl.R = 2 * warps;
+    }
+  }
   *plan = pl;
   return true;
 }
@@ -271,14 +285,15 @@ bool ft_tile_finish(const FtDev& d, FtTilePlan* plan, int32_t max_w, std::string
   }
   pl.pitch = (pl.copy_floats + cw * pl.J - min_warp_n + 8 + align - 1) / align * align;
   pl.pitch = std::max(pl.pitch, (cw * pl.J + 8 + align - 1) / align * align);  // warps without valid outputs read [0, cw J)
+  if (pl.ppw == 2) pl.pitch = (pl.copy_floats + 32 + 8 + align - 1) / align * align;   // idle tail lanes read up to 31 bins past a strip
   if (pl.copy_floats > kMaxPitch + 1) { *why = "strip too wide for the packed track entry"; return false; }
-  const int threads = (pl.R * pl.wpp + 1) * 32;
+  const int threads = (pl.R * pl.wpp / pl.ppw + 1) * 32;
   const int regs_est = (mode == 2 ? 3 : 2) * pl.J + 30;
   int ctas = std::min(4, std::min(2048 / threads, 65536 / (threads * regs_est)));
   ctas = std::max(ctas, 1);
   const size_t row_bytes = (size_t)pl.pitch * 4;
   // per-warp state: point parameters, entry table (+ weight table); packed mode: the 16-bit counter levels
-  const int n_cw = pl.R * pl.wpp;
+  const int n_cw = pl.R * pl.wpp;   // (two points per warp: R / 2 warps with two point records and two entry tables each)
   const size_t state_bytes = mode == 1 ? ft_tile_state_bytes<GatherHit8>(pl.J, n_cw)
                            : mode == 3 ? ft_tile_state_bytes<GatherF32W>(pl.J, n_cw)
                                        : ft_tile_state_bytes<GatherF32>(pl.J, n_cw);
@@ -326,12 +341,13 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const FtTileR
   a.sky_norm = run.sky_norm; a.norm_cb = run.norm_cb;
   a.near_ties = run.near_ties;
   a.glist = glist; a.gskip = gskip;
-  const unsigned block = (unsigned)((plan.R * plan.wpp + 1) * 32);
+  const unsigned block = (unsigned)((plan.R * plan.wpp / plan.ppw + 1) * 32);
   const uint64_t max_groups = 0x7fffffffull / (uint64_t)plan.n_tiles;
   auto launch = [&](unsigned grid) {
     return plan.mode == 1 ? ft_tile8_launch(plan.J, d, a, grid, block, plan.smem_bytes, s)
          : plan.mode == 2 ? ft_tileb_launch(plan.J, d, a, grid, block, plan.smem_bytes, s)
          : plan.mode == 3 ? ft_tilew_launch(plan.J, d, a, grid, block, plan.smem_bytes, s)
+         : plan.ppw == 2  ? ft_tile2_launch(plan.J / 2, d, a, grid, block, plan.smem_bytes, s)
                           : ft_tile_launch(plan.J, d, a, grid, block, plan.smem_bytes, s);
   };
   if (glist || gskip) {  // the threshold sample, or the rest of the bank: one launch over [pt_begin = 0, pt_end)

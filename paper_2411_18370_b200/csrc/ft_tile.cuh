@@ -20,6 +20,7 @@ struct FtTilePlan {
   int32_t J = 0;                // cw-wide f0 chunks per consumer warp (template parameter)
   int32_t wpp = 0;              // consumer warps per outer point
   int32_t R = 0;                // outer points per CTA
+  int32_t ppw = 1;              // outer points per consumer warp: 2 = narrow band with a ragged tail (ft_tile2.cu; then J = 2 (n_f0 / 32) + 1)
   int32_t pitch = 0;            // bins per staged row in shared memory (mode 1: per byte-shifted copy)
   int32_t copy_floats = 0;      // bins copied per row (multiple of align; <= pitch)
   int32_t rows_per_stage = 0;   // divides 32
@@ -35,6 +36,7 @@ struct FtTileHostIn {
   double df; double eps_bound;
   int points_per_cta;
   int force_tiles;  // > 0: use exactly this many f0 tiles (FT_OPT_F0_TILES)
+  int tail_packing; // 1: narrow bands may run two points per warp (FT_OPT_TAIL_PACKING)
 };
 
 // A plan is built in three steps so that one bind costs ONE stream synchronisation for all gather modes:

@@ -45,29 +45,22 @@ struct FtTileArgs {
 // Threads per CTA the kernels are compiled for: (consumer warps + 1 producer warp) * 32.  The accumulators
 // (J) and the loads in flight (J) set the register need, hence the bound.
 // (the register file is 4 x 16 384: 80 registers allow 6 warps per SM sub-partition, 72 allow 7, 64 allow 8)
-#ifndef FT_TILE_BATCH
-#define FT_TILE_BATCH 0
-#endif
-#ifndef FT_TILE_REGS
-#define FT_TILE_REGS 72
-#endif
-__host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : FT_TILE_REGS; }
-__host__ __device__ constexpr int ft_tile_max_threads(int J) { return (J <= 12 || FT_TILE_REGS <= 64) ? 1024 : 896; }
+// (measured: 64 registers and 14-15 points per CTA for the wide tiles is slower, 89.7-91.0 ms against 87.9 on config 2)
+__host__ __device__ constexpr int ft_tile_max_regs(int J) { return J <= 12 ? 64 : 72; }
+__host__ __device__ constexpr int ft_tile_max_threads(int J) { return J <= 12 ? 1024 : 896; }
 // packed number-count kernel: J registers of 8-bit counters + J loads in flight (16-bit levels in shared memory)
 __host__ __device__ constexpr int ft_tile8_max_regs(int J) { return J <= 8 ? 64 : 80; }
 __host__ __device__ constexpr int ft_tile8_max_threads(int J) { return J <= 8 ? 1024 : 768; }
 // both statistics in one pass: J accumulators + J counters + J loads in flight
-#ifndef FT_TILEB_REGS
-#define FT_TILEB_REGS 80
-#endif
-__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : FT_TILEB_REGS; }
-__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : (FT_TILEB_REGS <= 72 ? 896 : 768); }
+__host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 : 80; }
+__host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : 768; }
 // row-weighted gather: as the plain gather (the sky-point tables live in shared memory, the normalisation sums come
 // from a bind-time pass)
 __host__ __device__ constexpr int ft_tilew_max_regs(int J) { return ft_tile_max_regs(J); }
 __host__ __device__ constexpr int ft_tilew_max_threads(int J) { return ft_tile_max_threads(J); }
 
 cudaError_t ft_tile_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
+cudaError_t ft_tile2_launch(int JA, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
 cudaError_t ft_tilew_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
 cudaError_t ft_tileb_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
 cudaError_t ft_tile8_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
@@ -231,27 +224,17 @@ struct GatherF32 {
     const int64_t src = (int64_t)row * d.ld + k0;
     return 4u * (uint32_t)min((int64_t)a.copy_floats, d.n_sft * d.ld - src);
   }
-  // Loads in flight per row: all J of them, or (FT_TILE_BATCH > 0, J > 16) batches of FT_TILE_BATCH so that wide
-  // tiles fit 64 registers and one more consumer warp per scheduler
   template <int J> static __device__ __forceinline__ void row_fast(State<J>& st, uint32_t e, uint32_t base, uint32_t,
                                                                    bool last_ok, float) {
     const uint32_t ad = base + 4u * e;
-    constexpr int B = (FT_TILE_BATCH > 0 && J > 16) ? FT_TILE_BATCH : ((J + 1) & ~1);   // even
+    float v[J];
 #pragma unroll
-    for (int h0 = 0; h0 < J; h0 += B) {
-      float v[B];
+    for (int j = 0; j < J; ++j)
+      if (j < J - 1 || last_ok) v[j] = lds_f32(ad + 128u * j);
+    if (!last_ok) v[J - 1] = 0.f;
 #pragma unroll
-      for (int i = 0; i < B; ++i) {
-        const int j = h0 + i;
-        if (j < J) v[i] = (j < J - 1 || last_ok) ? lds_f32(ad + 128u * j) : 0.f;
-      }
-#pragma unroll
-      for (int i = 0; i < B; i += 2) {
-        const int j = h0 + i;
-        if (j + 1 < J) ft_add2(st.acc[j], st.acc[j + 1], v[i], v[i + 1]);
-        else if (j < J) st.acc[j] += v[i];
-      }
-    }
+    for (int j = 0; j + 1 < J; j += 2) ft_add2(st.acc[j], st.acc[j + 1], v[j], v[j + 1]);
+    if (J & 1) st.acc[J - 1] += v[J - 1];
   }
   template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t,
                                                                     int lane, float) {
@@ -300,14 +283,9 @@ struct GatherF32W : GatherF32 {
 // sum count the hits of up to 63 rows (carries only travel upwards), so they are folded into 16-bit counters once
 // per block of 32 SFTs.  The pixel is rounded to 18 mantissa bits (<= 3.8e-6 of |q| per pixel, random sign:
 // ~3e-8 of the statistic at n_sft = 8000; the plan keeps this kernel to 64 <= n_sft <= 65535).
-#ifndef FT_PAIRS_B
-#define FT_PAIRS_B 1
-#endif
-#ifndef FT_K2B_SKIP
-#define FT_K2B_SKIP 0   // timing experiments only (wrong results): 1 no fp32 adds, 2 no integer adds
-#endif
+
 struct GatherBoth : GatherF32 {
-  static constexpr bool VETO = true, HASCNT = true, PAIRS = FT_PAIRS_B != 0;
+  static constexpr bool VETO = true, HASCNT = true, PAIRS = true;
   static constexpr uint32_t kLowMask = 63u;
   template <int J> struct State { float acc[J]; uint32_t raw[J]; uint32_t c16[(J + 1) / 2]; };
   template <int J> static __device__ __forceinline__ void init(State<J>& st, uint32_t, uint32_t) {
@@ -352,10 +330,6 @@ struct GatherBoth : GatherF32 {
 #pragma unroll
       for (int i = 0; i < H; i += 2) {
         const int j = h0 + i;
-#if FT_K2B_SKIP == 1
-        if (j < J) st.acc[j] = v0[i];
-        continue;
-#endif
         if (j + 1 < J) {
           ft_add2(st.acc[j], st.acc[j + 1], v0[i], v0[i + 1]);
           ft_add2(st.acc[j], st.acc[j + 1], v1[i], v1[i + 1]);
@@ -367,10 +341,6 @@ struct GatherBoth : GatherF32 {
 #pragma unroll
       for (int i = 0; i < H; ++i) {
         const int j = h0 + i;
-#if FT_K2B_SKIP == 2
-        if (j < J) st.raw[j] = __float_as_uint(v1[i]);
-        continue;
-#endif
         if (j < J) {
           uint32_t r = st.raw[j];
           asm("{\n.reg .u32 t;\nadd.u32 t, %1, %2;\nadd.u32 %0, %0, t;\n}" : "+r"(r) : "r"(__float_as_uint(v0[i])), "r"(__float_as_uint(v1[i])));
@@ -499,6 +469,39 @@ struct GatherHit8 {
   }
 };
 
+// ---- producer warp: streams the strips (A3).  The whole warp fetches the 32 strip starts of a block of SFTs with
+// one coalesced load; lane 0 issues one bulk copy per row into the ring stage, after the consumers released it.
+template <class G>
+__device__ __forceinline__ void ft_tile_produce(const FtDev& d, const FtTileArgs& a, const int32_t* kst, int n_sft, int NS,
+                                                uint32_t ring0, uint32_t full0, uint32_t empty0, uint32_t row_bytes, int lane) {
+  int s = 0;
+  uint32_t lap = 0;  // how many times the ring has wrapped
+  for (int a0 = 0; a0 < n_sft; a0 += 32) {
+    const int kk = (a0 + lane < n_sft) ? kst[a0 + lane] : 0;
+    const int n_rows = min(32, n_sft - a0);
+    for (int q = 0; q < n_rows; q += kRPS) {
+      if (lap > 0) mbar_wait(empty0 + 8 * s, (lap - 1u) & 1u);  // consumers released the previous use
+      const int rows = min(kRPS, n_rows - q);
+      int kr[kRPS];
+#pragma unroll
+      for (int r = 0; r < kRPS; ++r) kr[r] = __shfl_sync(0xffffffffu, kk, (q + r) & 31);
+      if (lane == 0) {
+        uint32_t bytes = 0;
+#pragma unroll
+        for (int r = 0; r < kRPS; ++r)
+          if (r < rows) bytes += G::row_tx_bytes(d, a, a0 + q + r, kr[r]);
+        mbar_expect_tx(full0 + 8 * s, bytes);
+        const uint32_t dst = ring0 + (uint32_t)(s * kRPS) * row_bytes;
+#pragma unroll
+        for (int r = 0; r < kRPS; ++r)
+          if (r < rows) G::produce_row(d, a, dst + (uint32_t)r * row_bytes, a0 + q + r, kr[r], full0 + 8 * s);
+      }
+      __syncwarp();
+      if (++s == NS) { s = 0; ++lap; }
+    }
+  }
+}
+
 // Shared-memory layout (bytes): ring [NS][kRPS][row_bytes] | full[NS] empty[NS] mbarriers | FtPoint[n_cw] |
 // entry table [n_cw][32] u32 | (ROWW: weight table [n_cw][32] f32 | FtSkyPoint[n_cw]) | policy extra.
 template <class G>
@@ -534,34 +537,7 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
   const int32_t* kst = a.kst + (size_t)tile * n_sft;
 
   if (warp == n_cw) {
-    // ---- producer: streams the strips (A3).  The whole warp fetches the 32 strip starts of a block
-    // with one coalesced load; lane 0 issues the bulk copies.
-    int s = 0;
-    uint32_t lap = 0;  // how many times the ring has wrapped
-    for (int a0 = 0; a0 < n_sft; a0 += 32) {
-      const int kk = (a0 + lane < n_sft) ? kst[a0 + lane] : 0;
-      const int n_rows = min(32, n_sft - a0);
-      for (int q = 0; q < n_rows; q += kRPS) {
-        if (lap > 0) mbar_wait(empty0 + 8 * s, (lap - 1u) & 1u);  // consumers released the previous use
-        const int rows = min(kRPS, n_rows - q);
-        int kr[kRPS];
-#pragma unroll
-        for (int r = 0; r < kRPS; ++r) kr[r] = __shfl_sync(0xffffffffu, kk, (q + r) & 31);
-        if (lane == 0) {
-          uint32_t bytes = 0;
-#pragma unroll
-          for (int r = 0; r < kRPS; ++r)
-            if (r < rows) bytes += G::row_tx_bytes(d, a, a0 + q + r, kr[r]);
-          mbar_expect_tx(full0 + 8 * s, bytes);
-          const uint32_t dst = ring0 + (uint32_t)(s * kRPS) * row_bytes;
-#pragma unroll
-          for (int r = 0; r < kRPS; ++r)
-            if (r < rows) G::produce_row(d, a, dst + (uint32_t)r * row_bytes, a0 + q + r, kr[r], full0 + 8 * s);
-        }
-        __syncwarp();
-        if (++s == NS) { s = 0; ++lap; }
-      }
-    }
+    ft_tile_produce<G>(d, a, kst, n_sft, NS, ring0, full0, empty0, row_bytes, lane);
     return;
   }
   if (warp > n_cw) return;

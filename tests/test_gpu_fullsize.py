@@ -137,6 +137,44 @@ def test_tile_geometry_edge_cases(band_hz, n_sft, n_sky, ppc):
     ctx.close()
 
 
+TAILS = [
+    # (n_f0, n_sft, n_sky, points per CTA, two points per warp expected)
+    (450, 130, 5, 0, True),     # config 3's band: 14 x 32 + 2; 25 outer points: the last warp holds one point only
+    (33, 77, 3, 0, True),       # 32 + 1
+    (48, 64, 1, 0, True),       # 32 + 16: both tails fill the shared chunk; 5 points
+    (49, 64, 2, 0, False),      # tail of 17: one point per warp
+    (496, 40, 4, 2, True),      # 15 x 32 + 16, the widest; one warp (two points) per CTA
+    (130, 203, 7, 5, True),     # 4 x 32 + 2; ppc = 5 -> two warps per CTA, ragged last group
+    (64, 50, 2, 0, False),      # no tail at all
+]
+
+
+@pytest.mark.parametrize("n_f0,n_sft,n_sky,ppc,packed", TAILS)
+def test_narrow_band_tail_packing(n_f0, n_sft, n_sky, ppc, packed):
+    """Narrow bands of 32 m + t f0 (t <= 16) run two outer points per warp with the tails sharing one chunk
+    (ft_tile2.cu): element-by-element parity with the oracle (power, count, candidates), and the same bits as the
+    one-point-per-warp kernel (the accumulation order of a template does not change)."""
+    from paper_2411_18370_b200 import binding as B
+    wl = W.config2(n_sft=n_sft, n_sky=n_sky, band_hz=n_f0 / 1800.0, band_width=0.01 if n_f0 > 36 else n_f0 / 1800.0, k=3)
+    assert wl.grid.n_f0 == n_f0
+    o = fo.Oracle(wl)
+    op, oc, _, otie = o.eval_range()
+    ctx = H.gpu_context(wl, kernel=2, ppc=ppc)
+    gp, _ = H.gpu_full(ctx, wl, stat="power", want_count=False)
+    assert ("two points per warp" in ctx.describe()) == packed, ctx.describe()
+    _, gc = H.gpu_full(ctx, wl, stat="hough")
+    H.assert_full_parity(wl, gp, gc, op, oc, otie)
+    bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
+    ctx.eval(wl.grid, "power", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    H.assert_topk_parity(wl, cands, op, op, oc, wl.k, bpb)
+    ctx.set_option(B.FT_OPT_TAIL_PACKING, 0)
+    gp1, _ = H.gpu_full(ctx, wl, stat="power", want_count=False)
+    assert "two points per warp" not in ctx.describe()
+    assert np.array_equal(gp1, gp)
+    ctx.close()
+
+
 def test_generic_kernel_when_f0_step_differs_from_bin_width():
     """df0 = df/2 (a finer f0 grid than Eq. A1): not tileable, runs K0; forcing K2 is an error."""
     from paper_2411_18370_b200 import binding as B
