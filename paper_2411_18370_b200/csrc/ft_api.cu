@@ -67,6 +67,7 @@ int tile_pass(ft_ctx* c, const FtTilePlan& plan, const FtPass& p, const float* A
   run.z_mu = c->d.mu_G; run.z_inv_sigma = c->d.sigma_G > 0.0 ? 1.0 / c->d.sigma_G : 1.0;
   run.near_ties = c->near_ties_dev;
   run.sky_norm = c->skyn_dev; run.norm_cb = (A == c->WH_dev) ? 3 : 2;
+  run.skip_host = p.skip_host; run.n_skip_host = p.n_skip_host;
   int launches = 0;
   ft_tick(c);
   const cudaError_t e = ft_launch_tile(c->d, plan, run, p.pt_begin, p.pt_end, c->stream, &launches, p.glist, p.n_glist, p.gskip);

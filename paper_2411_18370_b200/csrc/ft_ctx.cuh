@@ -150,5 +150,6 @@ struct FtPass {
   int zmode = 0, out_key = 0;
   const uint32_t* glist = nullptr; uint32_t n_glist = 0;
   const uint32_t* gskip = nullptr;
+  const uint32_t* skip_host = nullptr; uint32_t n_skip_host = 0;   // the groups gskip marks, sorted (host), for the split tail
 };
 int ft_run_stat(ft_ctx* c, const FtPass& p);

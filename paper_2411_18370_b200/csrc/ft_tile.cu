@@ -240,7 +240,7 @@ bool ft_tile_choose(const FtDev& d, const FtTileHostIn& in, int mode, FtTilePlan
       pl.ppw = 2;
       pl.J = 2 * JA + 1;
       const int warps_max = ft_tile_max_threads(pl.J) / 32 - 1;
-      int warps = in.points_per_cta > 0 ? std::max(1, in.points_per_cta / 2) : std::min(27, warps_max);
+      int warps = in.points_per_cta > 0 ? std::max(1, in.points_per_cta / 2) : std::min(24, warps_max);   // (R = 48: many divisors for the split tail)
       warps = std::min(warps, warps_max);
       warps = (int)std::min<uint64_t>((uint64_t)warps, (d.n_points + 1) / 2);
       pl.R = 2 * warps;
@@ -322,6 +322,38 @@ uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points, uint32
   return std::min(n_sg * R, n_points);
 }
 
+// Split tail: a launch of n_groups CTA groups (n_skip of them exit at once) runs (n_groups - n_skip) / 148 waves; the
+// last, partial wave would leave SMs idle for up to a whole CTA time.  Its groups are split in S parts of R / S points
+// each (S the largest divisor of R with rem * S <= 148), run by CTAs with that many fewer consumer warps.  Single-tile
+// plans with one CTA per SM only.  Sets a->main_groups / main_ctas / tail_split and returns the grid size.
+static uint64_t ft_split_tail(const FtTilePlan& plan, uint64_t n_groups, const uint32_t* skip_sorted, uint32_t n_skip,
+                              FtTileArgs* a) {
+  a->tail_split = 1; a->main_groups = 0; a->main_ctas = 0;
+  const uint64_t grid1 = n_groups * (uint64_t)plan.n_tiles;
+  constexpr uint64_t kSMs = 148;
+  if (plan.mode == 1 || plan.n_tiles != 1 || plan.ctas_per_sm != 1 || n_skip > n_groups) return grid1;   // (mode 1: see ft_tile_body)
+  const uint64_t eff = n_groups - n_skip;
+  const uint64_t W = eff / kSMs, rem = eff % kSMs;
+  if (W == 0 || rem == 0) return grid1;
+  auto nonskipped = [&](uint64_t G) {   // groups of [0, G) that run
+    const uint32_t* e = std::lower_bound(skip_sorted, skip_sorted + n_skip, (uint32_t)std::min<uint64_t>(G, 0xffffffffu));
+    return G - (uint64_t)(e - skip_sorted);
+  };
+  uint64_t lo = 0, hi = n_groups;      // smallest G with nonskipped(G) == W * 148
+  while (lo < hi) {
+    const uint64_t mid = (lo + hi) / 2;
+    if (nonskipped(mid) >= W * kSMs) hi = mid; else lo = mid + 1;
+  }
+  const uint64_t G_main = lo;
+  const int unit = plan.ppw == 2 ? 2 : 1;
+  int S = 1;
+  for (int s = 2; s <= plan.R; ++s)
+    if (plan.R % s == 0 && (plan.R / s) % unit == 0 && rem * (uint64_t)s <= kSMs) S = s;
+  if (S == 1 || G_main > 0x7fffffffull) return grid1;
+  a->main_groups = (uint32_t)G_main; a->main_ctas = (uint32_t)G_main; a->tail_split = (uint32_t)S;
+  return G_main + (n_groups - G_main) * (uint64_t)S;
+}
+
 cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const FtTileRun& run, uint64_t pt_begin,
                            uint64_t pt_end, cudaStream_t s, int* launches, const uint32_t* glist, uint32_t n_glist,
                            const uint32_t* gskip) {
@@ -356,7 +388,10 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const FtTileR
     if (pt_begin != 0 || n_launch > max_groups) return cudaErrorInvalidValue;
     if (n_launch == 0) return cudaSuccess;
     a.pt_begin = 0; a.pt_end = pt_end;
-    const cudaError_t e = launch((unsigned)(n_launch * plan.n_tiles));
+    uint64_t grid = n_launch * (uint64_t)plan.n_tiles;
+    if (gskip && (run.skip_host || run.n_skip_host == 0)) grid = ft_split_tail(plan, all_groups, run.skip_host, run.n_skip_host, &a);
+    if (grid > 0x7fffffffull) return cudaErrorInvalidValue;
+    const cudaError_t e = launch((unsigned)grid);
     if (e == cudaSuccess) *launches = 1;
     return e;
   }
@@ -366,7 +401,10 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const FtTileR
     if (groups > max_groups) groups = max_groups;
     a.pt_begin = pt;
     a.pt_end = std::min<uint64_t>(pt_end, pt + groups * plan.R);
-    const cudaError_t e = launch((unsigned)(groups * plan.n_tiles));
+    uint64_t grid = groups * (uint64_t)plan.n_tiles;
+    if (pt + groups * plan.R >= pt_end) grid = ft_split_tail(plan, groups, nullptr, 0, &a);   // the last chunk of the range
+    if (grid > 0x7fffffffull) { a.tail_split = 1; grid = groups * (uint64_t)plan.n_tiles; }
+    const cudaError_t e = launch((unsigned)grid);
     if (e != cudaSuccess) return e;
     *launches += 1;
     pt = a.pt_end;

@@ -68,6 +68,8 @@ struct FtTileRun {
   const double* sky_norm = nullptr;   // row-weighted gather: [n_sky][4] normalisation sums (ft_launch_skyw_norm)
   int32_t norm_cb = 2;                // which add-back column of sky_norm: 2 (power array Q) or 3 (weighted hits WH)
   unsigned long long* near_ties = nullptr;
+  const uint32_t* skip_host = nullptr;   // with gskip: the skipped groups, sorted ascending (host copy), for the split tail
+  uint32_t n_skip_host = 0;
 };
 // glist != nullptr: evaluate only the CTA groups glist[0 .. n_glist) (the threshold sample; a group = R consecutive
 // outer points) and pack the outputs by launch-local row (group_local * R + r) * n_f0 + i_f0.  gskip != nullptr (a

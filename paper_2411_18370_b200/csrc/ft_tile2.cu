@@ -18,8 +18,9 @@ __device__ __forceinline__ void ft_tile2_body(const FtDev& d, const FtTileArgs& 
   constexpr int J = 2 * JA + 1;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_cw = a.R / 2;                                   // consumer warps (a.R = points per CTA, even)
-  const uint64_t group_l = blockIdx.x;                        // (one f0 tile)
+  const FtCtaWork cw = ft_cta_work<true>(a);                        // (one f0 tile; the split tail of a launch: part of a group)
+  const int n_cw = cw.R_cta / 2;                              // consumer warps (points per CTA are even)
+  const uint64_t group_l = cw.group_l;
   const uint64_t group = a.glist ? (uint64_t)__ldg(a.glist + group_l) : group_l;
   if (a.gskip && ((__ldg(a.gskip + (group >> 5)) >> (group & 31)) & 1u)) return;
   const int n_sft = (int)d.n_sft;
@@ -46,7 +47,8 @@ __device__ __forceinline__ void ft_tile2_body(const FtDev& d, const FtTileArgs& 
   // ---- consumers: points A = first + 2 warp, B = A + 1 ---------------------------------------------
   const int n_f0 = (int)d.n_f0;
   const int t = n_f0 - 32 * JA;                               // f0 per point in the shared tail chunk, 1 .. 16
-  uint64_t ptA = a.pt_begin + group * (uint64_t)a.R + 2u * (uint64_t)warp, ptB = ptA + 1;
+  const int r_pt = cw.part * cw.R_cta + 2 * warp;             // A's place in its group
+  uint64_t ptA = a.pt_begin + group * (uint64_t)a.R + (uint64_t)r_pt, ptB = ptA + 1;
   const bool actA = ptA < a.pt_end, actB = ptB < a.pt_end;
   if (!actA) ptA = a.pt_end - 1;   // keep the barrier protocol; results are discarded
   if (!actB) ptB = a.pt_end - 1;
@@ -156,7 +158,7 @@ __device__ __forceinline__ void ft_tile2_body(const FtDev& d, const FtTileArgs& 
     if (valid) {
       const uint64_t pt = isB ? ptB : ptA;
       const uint64_t idx = pt * (uint64_t)n_f0 + (uint64_t)i;
-      const uint64_t o = a.glist ? (group_l * (uint64_t)a.R + 2u * (uint64_t)warp + (isB ? 1u : 0u)) * (uint64_t)n_f0 + (uint64_t)i
+      const uint64_t o = a.glist ? (group_l * (uint64_t)a.R + (uint64_t)r_pt + (isB ? 1u : 0u)) * (uint64_t)n_f0 + (uint64_t)i
                                  : idx - a.out_base;
       const double vd = (double)acc[j] + a.add_back;
       const float v = (float)vd;

@@ -40,7 +40,30 @@ struct FtTileArgs {
   const uint32_t* glist;  // != nullptr: the launch runs the CTA groups glist[0 .. grid / n_tiles) (the threshold
                           // sample), outputs packed by launch-local row (group_local * R + r) * n_f0 + i_f0
   const uint32_t* gskip;  // != nullptr: bit g set = group g was in the sample; its CTAs exit at once (the rest of the bank)
+  // Split tail (ft_launch_tile): CTAs [0, main_ctas) each run one whole group of R points; the groups from main_groups
+  // on -- the last, partial wave of the launch -- are split in tail_split parts of R / tail_split points each, run by
+  // CTAs with that many fewer consumer warps (the other warps of the block exit at once), so that every SM has work
+  // until the end.  tail_split = 1: no split.
+  uint32_t main_ctas, main_groups, tail_split;
 };
+
+// Which (f0 tile, launch-local group, part of the group) a CTA runs, and how many of the group's points
+struct FtCtaWork { int tile; uint64_t group_l; int part, R_cta; };
+template <bool SPLIT>
+__device__ __forceinline__ FtCtaWork ft_cta_work(const FtTileArgs& a) {
+  FtCtaWork w;
+  const unsigned bid = blockIdx.x;
+  if (!SPLIT || a.tail_split <= 1u || bid < a.main_ctas) {
+    w.tile = (int)(bid % (unsigned)a.n_tiles); w.group_l = bid / (unsigned)a.n_tiles; w.part = 0; w.R_cta = a.R;
+  } else {
+    const unsigned tb = bid - a.main_ctas, rest = tb / (unsigned)a.n_tiles;
+    w.tile = (int)(tb % (unsigned)a.n_tiles);
+    w.part = (int)(rest % a.tail_split);
+    w.group_l = (uint64_t)a.main_groups + rest / a.tail_split;
+    w.R_cta = a.R / (int)a.tail_split;
+  }
+  return w;
+}
 
 // Threads per CTA the kernels are compiled for: (consumer warps + 1 producer warp) * 32.  The accumulators
 // (J) and the loads in flight (J) set the register need, hence the bound.
@@ -56,8 +79,11 @@ __host__ __device__ constexpr int ft_tileb_max_regs(int J) { return J <= 8 ? 64 
 __host__ __device__ constexpr int ft_tileb_max_threads(int J) { return J <= 8 ? 1024 : 768; }
 // row-weighted gather: as the plain gather (the sky-point tables live in shared memory, the normalisation sums come
 // from a bind-time pass)
-__host__ __device__ constexpr int ft_tilew_max_regs(int J) { return ft_tile_max_regs(J); }
-__host__ __device__ constexpr int ft_tilew_max_threads(int J) { return ft_tile_max_threads(J); }
+#ifndef FT_TILEW_REGS
+#define FT_TILEW_REGS 72
+#endif
+__host__ __device__ constexpr int ft_tilew_max_regs(int J) { return J <= 12 ? 64 : FT_TILEW_REGS; }
+__host__ __device__ constexpr int ft_tilew_max_threads(int J) { return J <= 12 ? 1024 : FT_TILEW_REGS <= 72 ? 896 : 768; }
 
 cudaError_t ft_tile_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
 cudaError_t ft_tile2_launch(int JA, const FtDev& d, const FtTileArgs& a, unsigned grid, unsigned block, size_t smem, cudaStream_t s);
@@ -421,17 +447,26 @@ struct GatherHit8 {
   template <int J> static __device__ __forceinline__ void rows_fast_pair(State<J>& st, uint32_t e0, uint32_t e1, uint32_t base0,
                                                                          uint32_t base1, uint32_t copy_pitch, bool last_ok) {
     const uint32_t ad0 = base0 + (e0 & 3u) * copy_pitch + (e0 & ~3u), ad1 = base1 + (e1 & 3u) * copy_pitch + (e1 & ~3u);
-    uint32_t v0[J], v1[J];
+    // loads in two half batches (2 x 8 in flight)
+    constexpr int H = (J + 1) / 2;
 #pragma unroll
-    for (int j = 0; j < J; ++j)
-      if (j < J - 1 || last_ok) { v0[j] = lds_u32(ad0 + 128u * j); v1[j] = lds_u32(ad1 + 128u * j); }
+    for (int h0 = 0; h0 < J; h0 += H) {
+      uint32_t v0[H], v1[H];
 #pragma unroll
-    for (int j = 0; j < J; ++j)
-      if (j < J - 1 || last_ok) {
-        uint32_t r = st.c8[j];
-        asm("{\n.reg .u32 t;\nadd.u32 t, %1, %2;\nadd.u32 %0, %0, t;\n}" : "+r"(r) : "r"(v0[j]), "r"(v1[j]));
-        st.c8[j] = r;
+      for (int i = 0; i < H; ++i) {
+        const int j = h0 + i;
+        if (j < J && (j < J - 1 || last_ok)) { v0[i] = lds_u32(ad0 + 128u * j); v1[i] = lds_u32(ad1 + 128u * j); }
       }
+#pragma unroll
+      for (int i = 0; i < H; ++i) {
+        const int j = h0 + i;
+        if (j < J && (j < J - 1 || last_ok)) {
+          uint32_t r = st.c8[j];
+          asm("{\n.reg .u32 t;\nadd.u32 t, %1, %2;\nadd.u32 %0, %0, t;\n}" : "+r"(r) : "r"(v0[i]), "r"(v1[i]));
+          st.c8[j] = r;
+        }
+      }
+    }
   }
   template <int J> static __device__ __forceinline__ void row_break(State<J>& st, uint32_t e, uint32_t base, uint32_t copy_pitch,
                                                                     int lane, float) {
@@ -514,9 +549,12 @@ template <int J, class G>
 __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_cw = a.R * a.wpp;
-  const int tile = (int)(blockIdx.x % (unsigned)a.n_tiles);
-  const uint64_t group_l = blockIdx.x / (unsigned)a.n_tiles;  // launch-local group
+  // (the packed number-count kernel sits at its register limit -- a few more live values and ptxas schedules its
+  // row loop two loads at a time, 34.9 -> 44 ms on config 2 -- so its launches are never split: ft_launch_tile)
+  const FtCtaWork cw = ft_cta_work<G::PER == 1>(a);
+  const int n_cw = cw.R_cta * a.wpp;                          // consumer warps of this CTA
+  const int tile = cw.tile;
+  const uint64_t group_l = cw.group_l;                        // launch-local group
   const uint64_t group = a.glist ? (uint64_t)__ldg(a.glist + group_l) : group_l;
   if (a.gskip && ((__ldg(a.gskip + (group >> 5)) >> (group & 31)) & 1u)) return;   // (whole CTA: before any barrier)
   const int n_sft = (int)d.n_sft;
@@ -543,7 +581,7 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
   if (warp > n_cw) return;
 
   // ---- consumers -------------------------------------------------------------------------------
-  const int r_pt = warp / a.wpp, sub = warp % a.wpp;
+  const int r_pt = cw.part * cw.R_cta + warp / a.wpp, sub = warp % a.wpp;   // the point's place in its group
   uint64_t pt = a.pt_begin + group * (uint64_t)a.R + (uint64_t)r_pt;
   const bool pt_active = pt < a.pt_end;
   if (!pt_active) pt = a.pt_end - 1;  // keep the barrier protocol; results are discarded
@@ -580,6 +618,8 @@ __device__ __forceinline__ void ft_tile_body(const FtDev& d, const FtTileArgs& a
   const uint32_t fb_end = full0 + 8u * (uint32_t)NS, stage_bytes = (uint32_t)kRPS * row_bytes;
   uint32_t ph = 0;
 
+  // (staggering the block phase of the warps of a CTA, so that they do not compute their track entries at the same
+  // time, was measured: +0.6 % on config 4, 0 on configs 2 and 3, -1.6 % on K2B, -10 % on K2H -- not used)
   for (int a0 = 0; a0 < n_sft; a0 += 32) {
     // -- A1/A2: this lane's SFT ---------------------------------------------------------------------
     uint32_t entry = 0;

@@ -244,6 +244,8 @@ int topk_regions(ft_ctx* c, const TopkSpec& sp, std::vector<FtCandDev>* out, int
         }
     }
     const uint32_t n_list = (uint32_t)glist.size();
+    std::vector<uint32_t> glist_sorted(glist);
+    std::sort(glist_sorted.begin(), glist_sorted.end());
     const int64_t rows = (int64_t)n_list * (int64_t)R;
     // one upload: group list | skip bitmask | row_start | rows
     const size_t n_words = ((size_t)n_groups + 31) / 32;
@@ -293,6 +295,7 @@ int topk_regions(ft_ctx* c, const TopkSpec& sp, std::vector<FtCandDev>* out, int
       if ((uint64_t)n_list < n_groups) {
         FtPass pb = p;
         pb.out_f = nullptr; pb.out_i = nullptr; pb.filter = true; pb.glist = nullptr; pb.n_glist = 0; pb.gskip = gskip_dev; pb.out_key = 0;
+        pb.skip_host = glist_sorted.data(); pb.n_skip_host = (uint32_t)glist_sorted.size();
         if ((rc = ft_run_stat(c, pb)) != FT_OK) return rc;
       }
       FT_CUDA(c, cudaMemcpyAsync(cnt.data(), c->sel.cnt, sizeof(uint32_t) * n_regions, cudaMemcpyDeviceToHost, c->stream));
