@@ -214,7 +214,6 @@ typedef struct {
  *   stat, rho_th  as ft_eval.   out_power_dev [device] fp32 [n] or NULL; out_count_dev [device] int32 [n] or NULL.
  * Synchronises the stream.  A track that leaves [0, n_bins) is an error, not a clamp: the call
  * returns FT_ERR_TRACK_RANGE, that template's outputs are NaN / -1 and the others are valid.
- * Spectrograms of more than 2^19 bins per SFT are FT_ERR_UNSUPPORTED here (and in ft_eval_bank).
  */
 int ft_eval_templates(ft_ctx* ctx, const ft_template* templates_dev, int64_t n, double t_ref, int stat,
                       double rho_th, float* out_power_dev, int32_t* out_count_dev);
