@@ -40,8 +40,8 @@ UNIT = "evals/s"
 SMEM_BYTES_PER_CLK_SM = 128.0   # nominal: B300_MICROARCH "smem crossbar BW 128 B/cyc/SM" (fallback when not measured)
 FP64_FMA_PER_CLK_SM = 64.0      # nominal B200 vector fp64 (40 TFLOP/s at 148 SMs x 1.965 GHz / 2)
 N_SM = 148
-# fp64-pipe issue slots per evaluation of K1's loop body, counted in the SASS
-K1_FP64_SLOTS = {"isolated": 24.0, "binary": 43.0}
+# fp64-pipe cycles per evaluation of K1, in DFMA-equivalents, from ncu sm__pipe_fp64_cycles_active (profiles/r02_k1_*_ncu.md)
+K1_FP64_SLOTS = {"isolated": 19.2, "binary": 41.3}
 
 
 def ncu_traffic(config: int, kernel: str):

@@ -202,6 +202,7 @@ bool ft_tile_choose(const FtDev& d, const FtTileHostIn& in, int mode, FtTilePlan
   int bJ = 0, bW = 0; int64_t bT = 0;
   // a warp's range may hold one break: cw J |D - 1| < 0.45 (clamped before the cast: eps -> 0 for a_p = 0, v = 0)
   const int maxJ_eps = (int)std::min(64.0, std::floor(0.45 / ((double)cw * std::fmax(in.eps_bound, 1e-12))));
+  const double spread_bins = 2.0 * in.eps_bound * (d.f0_start + (double)d.n_f0 * d.df0) / in.df + 16.0;   // Doppler spread of a strip
   for (int64_t nt = 1; nt <= chunks; ++nt) {
     if (in.force_tiles > 0 && nt != in.force_tiles) continue;
     const int64_t cpt = (chunks + nt - 1) / nt;
@@ -212,7 +213,13 @@ bool ft_tile_choose(const FtDev& d, const FtTileHostIn& in, int mode, FtTilePlan
       int J = 0;
       for (int c : kJList) if (c >= Jn) { J = c; break; }
       if (J == 0 || J > maxJ_eps) continue;
-      const double cost = (double)nt * wpp * (J + 1.5) * (1.0 + 0.02 * (double)(nt - 1));
+      // shared-memory wavefronts per (outer point, SFT): the loads of the tile's chunks, the entry reads, and the point's
+      // share of the TMA writes of the strip (tile + Doppler spread, 32 floats per wavefront, R points per CTA); every
+      // further tile costs ~4 % (measured on configs 2 and 4: two tiles win on 3 600 f0, lose on 1 800)
+      const double R_def = wpp == 1 ? 27.0 : (double)(24 / wpp);
+      const double strip_wf = ((double)cpt * cw + spread_bins) / 32.0;
+      const double cost = (double)nt * ((double)std::min<int64_t>(cpt, (int64_t)wpp * J) + 0.5 * wpp + strip_wf / R_def) *
+                          (1.0 + 0.04 * (double)(nt - 1));
       if (cost < best) { best = cost; bJ = J; bW = wpp; bT = nt; }
     }
     if (cpt == 1) break;
@@ -324,34 +331,38 @@ uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points, uint32
 
 // Split tail: a launch of n_groups CTA groups (n_skip of them exit at once) runs (n_groups - n_skip) / 148 waves; the
 // last, partial wave would leave SMs idle for up to a whole CTA time.  Its groups are split in S parts of R / S points
-// each (S the largest divisor of R with rem * S <= 148), run by CTAs with that many fewer consumer warps.  Single-tile
-// plans with one CTA per SM only.  Sets a->main_groups / main_ctas / tail_split and returns the grid size.
+// each (S the largest divisor of R with rem * n_tiles * S <= 148), run by CTAs with that many fewer consumer warps.
+// Plans with one CTA per SM only.  Sets a->main_groups / main_ctas / tail_split and returns the grid size.
 static uint64_t ft_split_tail(const FtTilePlan& plan, uint64_t n_groups, const uint32_t* skip_sorted, uint32_t n_skip,
                               FtTileArgs* a) {
   a->tail_split = 1; a->main_groups = 0; a->main_ctas = 0;
-  const uint64_t grid1 = n_groups * (uint64_t)plan.n_tiles;
+  const uint64_t nt = (uint64_t)plan.n_tiles;
+  const uint64_t grid1 = n_groups * nt;
   constexpr uint64_t kSMs = 148;
-  if (plan.mode == 1 || plan.n_tiles != 1 || plan.ctas_per_sm != 1 || n_skip > n_groups) return grid1;   // (mode 1: see ft_tile_body)
-  const uint64_t eff = n_groups - n_skip;
-  const uint64_t W = eff / kSMs, rem = eff % kSMs;
-  if (W == 0 || rem == 0) return grid1;
+  if (plan.mode == 1 || plan.ctas_per_sm != 1 || n_skip > n_groups) return grid1;   // (mode 1: see ft_tile_body)
+  const uint64_t eff = n_groups - n_skip;                 // groups that run (n_tiles CTAs each)
+  const uint64_t W = eff * nt / kSMs;                     // full waves
+  if (W == 0) return grid1;
+  const uint64_t main_eff = W * kSMs / nt;                // running groups of the full waves
+  const uint64_t rem = eff - main_eff;
+  if (rem == 0) return grid1;
   auto nonskipped = [&](uint64_t G) {   // groups of [0, G) that run
     const uint32_t* e = std::lower_bound(skip_sorted, skip_sorted + n_skip, (uint32_t)std::min<uint64_t>(G, 0xffffffffu));
     return G - (uint64_t)(e - skip_sorted);
   };
-  uint64_t lo = 0, hi = n_groups;      // smallest G with nonskipped(G) == W * 148
+  uint64_t lo = 0, hi = n_groups;      // smallest G with nonskipped(G) == main_eff
   while (lo < hi) {
     const uint64_t mid = (lo + hi) / 2;
-    if (nonskipped(mid) >= W * kSMs) hi = mid; else lo = mid + 1;
+    if (nonskipped(mid) >= main_eff) hi = mid; else lo = mid + 1;
   }
   const uint64_t G_main = lo;
   const int unit = plan.ppw == 2 ? 2 : 1;
   int S = 1;
   for (int s = 2; s <= plan.R; ++s)
-    if (plan.R % s == 0 && (plan.R / s) % unit == 0 && rem * (uint64_t)s <= kSMs) S = s;
-  if (S == 1 || G_main > 0x7fffffffull) return grid1;
-  a->main_groups = (uint32_t)G_main; a->main_ctas = (uint32_t)G_main; a->tail_split = (uint32_t)S;
-  return G_main + (n_groups - G_main) * (uint64_t)S;
+    if (plan.R % s == 0 && (plan.R / s) % unit == 0 && rem * nt * (uint64_t)s <= kSMs) S = s;
+  if (S == 1 || G_main * nt > 0x7fffffffull) return grid1;
+  a->main_groups = (uint32_t)G_main; a->main_ctas = (uint32_t)(G_main * nt); a->tail_split = (uint32_t)S;
+  return (G_main + (n_groups - G_main) * (uint64_t)S) * nt;
 }
 
 cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const FtTileRun& run, uint64_t pt_begin,

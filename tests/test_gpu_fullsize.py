@@ -440,7 +440,7 @@ def test_config5_sweep_sizes_exhaustive(size):
 
 def test_config5_16000_sfts_and_4hz_band_geometry():
     """n_sft = 16 000 (the longest accumulation of the sweep: fp32 sums over the centred array must hold 1e-5) at a
-    reduced sky grid, and the 4 Hz band of the largest sweep size, which plans 4 warps per point over 2 f0 tiles."""
+    reduced sky grid, and the 4 Hz band of the largest sweep size, which plans several f0 tiles."""
     wl = W.config5(16000, 1.0, 8)
     op, oc, _, otie = fo.Oracle(wl).eval_range()
     ctx = H.gpu_context(wl)
@@ -455,7 +455,7 @@ def test_config5_16000_sfts_and_4hz_band_geometry():
     ctx = H.gpu_context(wl)
     gp, gc = H.gpu_full(ctx, wl, stat="both")
     desc = ctx.describe().split(";")[0]
-    assert "wpp=4" in desc and "n_tiles=2" in desc, desc
+    assert ("wpp=4" in desc and "n_tiles=2" in desc) or ("wpp=2" in desc and "n_tiles=4" in desc), desc   # several f0 tiles
     H.assert_full_parity(wl, gp, gc, op, oc, otie)
     bpb = int(round(wl.band_width / wl.grid.df0)); n_bands = -(-wl.grid.n_f0 // bpb)
     ctx.eval(wl.grid, "power", wl.rho_th)
