@@ -65,10 +65,29 @@ __device__ __forceinline__ FtPoint ft_decode_point(const FtDev& d, uint64_t pt) 
   return p;
 }
 
+// V = dot / c as q0 = dot * (1/c), V = q0 + (dot - q0 c) (1/c): the residual is exact in the fused multiply-add,
+// and the corrected quotient is the correctly rounded one (Markstein's theorem: 1/c is correctly rounded and q0
+// is within an ulp); ft_selftest(0) compares it with __ddiv_rn bit for bit.
+__device__ __forceinline__ double ft_div_c(double dot) {
+  const double kInvC = 1.0 / FT_C_LIGHT;
+  const double q0 = __dmul_rn(dot, kInvC);
+  return __fma_rn(__fma_rn(-q0, FT_C_LIGHT, dot), kInvC, q0);
+}
+
+
 // D_alpha = (1 + V) - B, the bracket of Eq. (2) at SFT alpha.
 __device__ __forceinline__ double ft_doppler(const FtDev& d, const FtPoint& p, int64_t a, double t) {
   const double vx = d.vel[3 * a + 0], vy = d.vel[3 * a + 1], vz = d.vel[3 * a + 2];
   const double V = __ddiv_rn(__dadd_rn(__dadd_rn(__dmul_rn(vx, p.nx), __dmul_rn(vy, p.ny)), __dmul_rn(vz, p.nz)), FT_C_LIGHT);
+  double B = 0.0;
+  if (p.binary) B = __dmul_rn(p.apOm, p.crow ? p.crow[a] : cos(__dmul_rn(p.Om, __dsub_rn(t, p.t_asc))));
+  return __dsub_rn(__dadd_rn(1.0, V), B);
+}
+
+// The same with V = dot / c by ft_div_c (the same bits, a fraction of the instructions): per-evaluation kernels.
+__device__ __forceinline__ double ft_doppler_rcp(const FtDev& d, const FtPoint& p, int64_t a, double t) {
+  const double vx = d.vel[3 * a + 0], vy = d.vel[3 * a + 1], vz = d.vel[3 * a + 2];
+  const double V = ft_div_c(__dadd_rn(__dadd_rn(__dmul_rn(vx, p.nx), __dmul_rn(vy, p.ny)), __dmul_rn(vz, p.nz)));
   double B = 0.0;
   if (p.binary) B = __dmul_rn(p.apOm, p.crow ? p.crow[a] : cos(__dmul_rn(p.Om, __dsub_rn(t, p.t_asc))));
   return __dsub_rn(__dadd_rn(1.0, V), B);

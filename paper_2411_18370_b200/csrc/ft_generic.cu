@@ -161,15 +161,20 @@ ft_refine_thread_kernel(const __grid_constant__ FtDev d, const uint64_t* __restr
   unsigned ties = 0;
   FtSkyPoint sk;
   if (d.skyw) sk = ft_sky_point(p.nx, p.ny, p.nz);
+  // branch-free body (an out-of-range bin -- impossible for a validated grid -- contributes an exact zero), unrolled
+  // so that the gathers of several SFTs are in flight; the sums are still added in ascending SFT order.  The kernel is
+  // bound by the scattered gathers (246 000 survivors of config 2: 8.0 -> 6.7 ms with this form; staging the per-SFT
+  // tables in shared memory as K1 does measured slower, 7.3 ms).
+#pragma unroll 4
   for (int64_t a = 0; a < d.n_sft; ++a) {
     const double t = d.t_mid[a];
-    const double D = ft_doppler(d, p, a, t);
+    const double D = ft_doppler_rcp(d, p, a, t);
     const double x = ft_track_x(f0, __dmul_rn(p.f1, __dsub_rn(t, d.t_ref)), D, d.f_min, d.inv_df);
     ties += ft_near_tie(x) ? 1u : 0u;
     const int64_t k = __double2ll_rn(x);
-    if (k < 0 || k >= d.n_bins || !(x == x)) continue;
-    const int64_t off = a * d.ld + k;
-    const float pix = __ldg(d.P + off);
+    const bool ok = k >= 0 && k < d.n_bins && x == x;
+    const int64_t off = a * d.ld + (ok ? k : 0);
+    const float pix = ok ? __ldg(d.P + off) : 0.f;
     double wa = (double)((d.wkind == 1) ? __ldg(d.w + a) : __ldg(d.w + off));
     if (d.skyw) {
       wa = __dmul_rn(ft_antenna_u(d.ant + 9 * a, sk), wa);
@@ -177,7 +182,9 @@ ft_refine_thread_kernel(const __grid_constant__ FtDev d, const uint64_t* __restr
       wsq = __dadd_rn(wsq, __dmul_rn(wa, wa));
     }
     power = __dadd_rn(power, __dmul_rn(wa, (double)pix));
-    if (pix > d.rho) { wcount = __dadd_rn(wcount, wa); ++count; }
+    const bool hit = pix > d.rho;
+    wcount = __dadd_rn(wcount, hit ? wa : 0.0);
+    count += hit ? 1 : 0;
   }
   double mu = d.mu_G, sigma = d.sigma_G;
   if (d.skyw) { power = power / wsum; wcount = wcount / wsum; mu = 1.0; sigma = sqrt(wsq) / wsum; }

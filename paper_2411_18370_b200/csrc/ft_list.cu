@@ -33,15 +33,6 @@ __device__ __forceinline__ double ft_f2d(float x) {
   return (double)x;
 }
 
-// V = dot / c as q0 = dot * (1/c), V = q0 + (dot - q0 c) (1/c): the residual is exact in the fused multiply-add,
-// and the corrected quotient is the correctly rounded one (Markstein's theorem: 1/c is correctly rounded and q0
-// is within an ulp); ft_selftest(0) compares it with __ddiv_rn bit for bit.
-__device__ __forceinline__ double ft_div_c(double dot) {
-  const double kInvC = 1.0 / FT_C_LIGHT;
-  const double q0 = __dmul_rn(dot, kInvC);
-  return __fma_rn(__fma_rn(-q0, FT_C_LIGHT, dot), kInvC, q0);
-}
-
 // cos(x) for the orbital phase of K1: k = rint(x / pi) by a magic-number fused multiply-add (no F2I / I2F), r = x - k pi
 // with pi split in three doubles (each product exact in the fused multiply-add), cos(r) on [-pi/2, pi/2] by its Taylor
 // series to r^24 (truncation < 1e-19; twelve fused multiply-adds), sign from the parity of k.  No table, no branch:
