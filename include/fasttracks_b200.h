@@ -219,6 +219,67 @@ int ft_eval_templates(ft_ctx* ctx, const ft_template* templates_dev, int64_t n, 
                       double rho_th, float* out_power_dev, int32_t* out_count_dev);
 
 /*
+ * ft_eval_templates_noalloc — the computation of ft_eval_templates (same kernel K1, same canonical arithmetic,
+ * same results bit for bit) as ONE self-contained call that never enters the CUDA allocator: no handle, no
+ * cudaMalloc / cudaFree / cudaMallocAsync, no library routine that allocates.
+ *
+ * Who needs it.  Every other call of this header works on a handle, and ft_create and the handle's grow-only
+ * buffers allocate device memory (ft_eval_templates itself re-allocates its ordering buffer whenever a longer
+ * list arrives).  Some hosts cannot live with that:
+ *   - a process that has handed the whole device to one memory pool (a framework's caching allocator, an RMM arena,
+ *     a serving runtime with a fixed memory plan): a cudaMalloc made behind the pool's back fails with
+ *     out-of-memory although the pool holds free blocks, or eats into the head-room the plan relies on;
+ *   - a follow-up loop with a latency budget: cudaMalloc and cudaFree stall every stream of the device, not just
+ *     the caller's, so one call that grows a buffer delays unrelated work on the same GPU;
+ *   - code that runs after start-up in a system whose rule is "no allocation after initialisation".
+ * Such a caller allocates the inputs and outputs below through whatever allocator it is allowed to use and calls
+ * this function; the kernel's own work space is a fixed array inside the library.
+ *
+ * The work space.  K1 needs global-memory scratch beyond its inputs and outputs: the f0-ordered evaluation order
+ * (one uint32 per template plus a 4096-entry histogram), the out-of-range flag and the near-tie counter.  Here
+ * they live in a file-scope static __device__ array of (FT_NOALLOC_MAX_TEMPLATES + 4096) * 4 + 256 bytes
+ * (4 MiB + 16.25 KiB).  It is part of the library image: every GPU on which this process uses the library holds
+ * that much from the moment the module is loaded there until the process exits, whether or not this function is
+ * ever called.  n > FT_NOALLOC_MAX_TEMPLATES is rejected with FT_ERR_ARG (split the bank into batches; template
+ * results do not depend on the batching).
+ *
+ * Rules that follow from the shared array:
+ *   - The FIRST call on a device looks the array's device address up (cudaGetSymbolAddress, once per device,
+ *     cached) and thereby makes the CUDA runtime load the library's module on that device.  Make that first call
+ *     during start-up, before any stream capture begins on the device.
+ *   - All calls on a device use the same array, and it keeps what the previous call left there.  The function
+ *     clears what must start at zero (histogram, flag, counter) at the beginning of every call, and the ordering
+ *     is rewritten in full for the n templates of the call, so nothing stale is ever read.
+ *   - Two calls in flight on one GPU at the same time would race on the array.  The function therefore holds a
+ *     per-device lock from its first enqueue until its stream has drained, which serialises host threads of one
+ *     process (separate processes do not interact: each has its own copy of the array).
+ *
+ * Arguments.  The device that is CURRENT when the function is called must be the one that owns every device
+ * pointer and the stream.  All device arrays are caller-owned and only read, except the two outputs.
+ *   P_dev        [device] fp32 [n_sft][ld_bins]: the spectrogram as in ft_create (any alignment, ld_bins >= n_bins).
+ *   t_mid_dev    [device] fp64 [n_sft];  vel_dev [device] fp64 [n_sft][3]  (host arrays in ft_create, device arrays here).
+ *   w_dev, wkind [device] FT_W_PER_SFT: fp32 [n_sft];  FT_W_PER_SFT_BIN: fp32 [n_sft][ld_bins].
+ *   f_min, df    as ft_create.
+ *   templates_dev [device] ft_template [n];  n in [0, FT_NOALLOC_MAX_TEMPLATES];  t_ref, stat (FT_STAT_POWER / _HOUGH /
+ *                _BOTH), rho_th, out_power_dev [device] fp32 [n] or NULL, out_count_dev [device] int32 [n] or NULL:
+ *                as ft_eval_templates.
+ *   near_ties_host [host] or NULL: receives the number of evaluations of THIS call within 1e-9 bin of a rounding tie.
+ *   cuda_stream  a cudaStream_t (NULL = default stream); the work is enqueued there and the function returns after
+ *                that stream has drained.
+ *   err_msg_host, err_msg_cap  [host] or NULL / 0: on a non-zero return, a NUL-terminated description of the error
+ *                (there is no handle to keep one).
+ * Returns FT_OK; FT_ERR_ARG (NULL / non-finite / out-of-range argument, n beyond the maximum, a pointer that is not
+ * device memory of the current device); FT_ERR_CUDA; FT_ERR_TRACK_RANGE (some track leaves [0, n_bins): that
+ * template's outputs are NaN / -1, the others are valid).  Sky-dependent weights (ft_set_antenna) are not available here.
+ */
+#define FT_NOALLOC_MAX_TEMPLATES 1048576
+int ft_eval_templates_noalloc(const float* P_dev, int64_t n_sft, int64_t n_bins, int64_t ld_bins,
+                              const double* t_mid_dev, const double* vel_dev, const float* w_dev, int wkind,
+                              double f_min, double df, const ft_template* templates_dev, int64_t n, double t_ref,
+                              int stat, double rho_th, float* out_power_dev, int32_t* out_count_dev,
+                              uint64_t* near_ties_host, void* cuda_stream, char* err_msg_host, int64_t err_msg_cap);
+
+/*
  * ft_bank_draw — a random template bank drawn uniformly in the xi coordinates of Eq. (A11) (:602-614) over a
  * box of the physical parameters ("draw n templates uniformly in xi, map them to lambda", :312-316, :627):
  *   f0 ~ f0^5, (alpha, sin delta) uniform, a_p ~ a_p^2, Omega = 2 pi / P_orb ~ Omega^3, phi_b = Omega (t_asc - t_ref)

@@ -14,7 +14,7 @@ FT_STAT = {"power": 0, "hough": 1, "both": 2, "whough": 3}
 FT_OPT_KERNEL, FT_OPT_FUSED_TOPK, FT_OPT_POINTS_PER_CTA, FT_OPT_PACKED_COUNT, FT_OPT_F0_TILES = 0, 1, 2, 3, 4
 FT_OPT_SELECT_CAP, FT_OPT_COUNT_FLOOR, FT_OPT_ONE_PASS_BOTH, FT_OPT_WCOUNT_FLOOR, FT_OPT_VETO_FIRST, FT_OPT_TAIL_PACKING = 5, 6, 7, 8, 9, 10
 SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_topk_per_box", "ft_set_antenna", "ft_eval_list",
-           "ft_eval_templates", "ft_bank_draw", "ft_eval_bank", "ft_track", "ft_set_option", "ft_set_option_f64",
+           "ft_eval_templates", "ft_eval_templates_noalloc", "ft_bank_draw", "ft_eval_bank", "ft_track", "ft_set_option", "ft_set_option_f64",
            "ft_get_counters", "ft_measure_peaks", "ft_selftest", "ft_last_error", "ft_describe", "ft_destroy"]
 
 
@@ -96,6 +96,11 @@ def load_library(path: str | None = None):
         lib.ft_eval_templates.restype = C.c_int
         lib.ft_eval_templates.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_int, C.c_double,
                                           C.c_void_p, C.c_void_p]
+        lib.ft_eval_templates_noalloc.restype = C.c_int
+        lib.ft_eval_templates_noalloc.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
+                                                  C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_int64,
+                                                  C.c_double, C.c_int, C.c_double, C.c_void_p, C.c_void_p,
+                                                  C.POINTER(C.c_uint64), C.c_void_p, C.c_char_p, C.c_int64]
         lib.ft_topk_per_box.restype = C.c_int
         lib.ft_topk_per_box.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_double, C.c_int32, C.c_int, C.c_void_p,
                                         C.POINTER(C.c_int32)]
@@ -130,6 +135,48 @@ def load_library(path: str | None = None):
 
 def _hp(a):
     return a.ctypes.data_as(C.c_void_p)
+
+
+FT_NOALLOC_MAX_TEMPLATES = 1 << 20
+
+
+def eval_templates_noalloc(P_dev, t_mid_dev, vel_dev, w_dev, f_min, df, templates_dev, t_ref, stat, rho_th,
+                           out_power=None, out_count=None, n_bins=None, stream=None) -> int:
+    """ft_eval_templates_noalloc: the statistic of an explicit template list without a handle and without any
+    device allocation by the library -- for hosts whose device memory belongs to a pool, or that may not
+    allocate after start-up (see the header).  Every array is a torch device tensor the CALLER allocated:
+    P_dev fp32 [n_sft][ld], t_mid_dev fp64 [n_sft], vel_dev fp64 [n_sft][3], w_dev fp32 [n_sft] or [n_sft][ld],
+    templates_dev n records of 64 B, out_power fp32 [n] / out_count int32 [n] or None.  At most
+    FT_NOALLOC_MAX_TEMPLATES templates per call.  Marshalling only; returns the call's near-tie count."""
+    import torch
+    lib = load_library()
+    assert P_dev.is_cuda and P_dev.dtype == torch.float32 and P_dev.dim() == 2 and P_dev.is_contiguous()
+    n_sft, ld = P_dev.shape
+    assert t_mid_dev.is_cuda and t_mid_dev.dtype == torch.float64 and t_mid_dev.numel() == n_sft and t_mid_dev.is_contiguous()
+    assert vel_dev.is_cuda and vel_dev.dtype == torch.float64 and vel_dev.numel() == 3 * n_sft and vel_dev.is_contiguous()
+    assert w_dev.is_cuda and w_dev.dtype == torch.float32 and w_dev.is_contiguous()
+    assert w_dev.numel() in (n_sft, n_sft * ld)
+    wkind = 1 if w_dev.dim() == 1 else 2
+    assert templates_dev.is_cuda and templates_dev.is_contiguous()
+    nbytes = templates_dev.numel() * templates_dev.element_size()
+    assert nbytes % 64 == 0
+    n = nbytes // 64
+    for o in (out_power, out_count):
+        assert o is None or (o.is_cuda and o.numel() == n and o.is_contiguous())
+    pp = C.c_void_p(out_power.data_ptr()) if out_power is not None else None
+    pc = C.c_void_p(out_count.data_ptr()) if out_count is not None else None
+    st = stream if stream is not None else torch.cuda.current_stream(P_dev.device).cuda_stream
+    ties = C.c_uint64(0)
+    msg = C.create_string_buffer(512)
+    with torch.cuda.device(P_dev.device):   # the call works on the current device
+        rc = lib.ft_eval_templates_noalloc(C.c_void_p(P_dev.data_ptr()), n_sft, ld if n_bins is None else int(n_bins), ld,
+                                           C.c_void_p(t_mid_dev.data_ptr()), C.c_void_p(vel_dev.data_ptr()),
+                                           C.c_void_p(w_dev.data_ptr()), wkind, float(f_min), float(df),
+                                           C.c_void_p(templates_dev.data_ptr()), n, float(t_ref), FT_STAT[stat],
+                                           float(rho_th), pp, pc, C.byref(ties), C.c_void_p(st), msg, 512)
+    if rc != 0:
+        raise FtError(rc, msg.value.decode())
+    return int(ties.value)
 
 
 class Context:

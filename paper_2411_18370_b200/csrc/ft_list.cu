@@ -12,8 +12,17 @@
 // correction (bit-identical to the IEEE quotient: ft_selftest 0).  A track leaving the spectrogram raises
 // *err (reading R9: an error, not a clamp) and the template's outputs are NaN / -1.
 #include <algorithm>
+#include <cstdarg>
+#include <mutex>
 
 #include "ft_ctx.cuh"
+
+// Work space of ft_eval_templates_noalloc (end of this file): K1's scratch for callers that may not allocate.
+// Layout: uint32 perm[n] | uint32 hist[4096] (n <= FT_NOALLOC_MAX_TEMPLATES, so both fit in the first
+// (MAX + 4096) words) | at byte (MAX + 4096) * 4: int32 out-of-range flag, at + 8: uint64 near-tie counter.
+// In host code this name is only a stand-in for the symbol, NOT a device address: the address a kernel may be
+// given comes from cudaGetSymbolAddress (ft_noalloc_scratch_ptr below), looked up once per device.
+static __device__ __align__(256) unsigned char ft_noalloc_scratch[((size_t)FT_NOALLOC_MAX_TEMPLATES + 4096) * 4 + 256];
 
 namespace {
 
@@ -557,6 +566,113 @@ int ft_selftest(ft_ctx* c, int which, int64_t n, uint64_t seed, uint64_t* n_fail
   FT_CUDA(c, cudaMemcpyAsync(&h, nf, 8, cudaMemcpyDeviceToHost, c->stream));
   FT_CUDA(c, cudaStreamSynchronize(c->stream));
   *n_fail_out = h;
+  return FT_OK;
+}
+
+}  // extern "C"
+
+// ---- ft_eval_templates_noalloc: K1 with its scratch in the static array at the top of this file --------------
+namespace {
+
+constexpr int kNoallocMaxDevices = 64;
+constexpr size_t kNoallocTail = ((size_t)FT_NOALLOC_MAX_TEMPLATES + K1_BUCKETS) * sizeof(uint32_t);   // flag | ties
+std::mutex g_noalloc_setup_mu;                          // guards the address table
+std::mutex g_noalloc_call_mu[kNoallocMaxDevices];       // one call at a time per device: the array is shared
+unsigned char* g_noalloc_ptr[kNoallocMaxDevices] = {};  // device address of ft_noalloc_scratch, per device ordinal
+
+int noalloc_fail(char* msg, int64_t cap, int code, const char* fmt, ...) {
+  if (msg && cap > 0) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(msg, (size_t)cap, fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+// The array's address on the current device.  cudaGetSymbolAddress answers for the device that is current, so the
+// table is per device; the first lookup on a device also loads this library's module there.
+cudaError_t ft_noalloc_scratch_ptr(int dev, unsigned char** out) {
+  std::lock_guard<std::mutex> g(g_noalloc_setup_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, ft_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    g_noalloc_ptr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_noalloc_ptr[dev];
+  return cudaSuccess;
+}
+
+// true if p is device (or managed) memory reachable as such from device dev
+bool noalloc_on_device(const void* p, int dev) {
+  cudaPointerAttributes a{};
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return (a.type == cudaMemoryTypeDevice && a.device == dev) || a.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ft_eval_templates_noalloc(const float* P_dev, int64_t n_sft, int64_t n_bins, int64_t ld_bins,
+                              const double* t_mid_dev, const double* vel_dev, const float* w_dev, int wkind,
+                              double f_min, double df, const ft_template* templates_dev, int64_t n, double t_ref,
+                              int stat, double rho_th, float* out_power_dev, int32_t* out_count_dev,
+                              uint64_t* near_ties_host, void* cuda_stream, char* msg, int64_t cap) {
+  if (msg && cap > 0) msg[0] = 0;
+  if (near_ties_host) *near_ties_host = 0;
+  if (!P_dev || !t_mid_dev || !vel_dev || !w_dev)
+    return noalloc_fail(msg, cap, FT_ERR_ARG, "ft_eval_templates_noalloc: NULL spectrogram / table pointer");
+  if (n_sft < 1 || n_bins < 1 || ld_bins < n_bins)
+    return noalloc_fail(msg, cap, FT_ERR_ARG, "ft_eval_templates_noalloc: need n_sft >= 1, n_bins >= 1, ld_bins >= n_bins");
+  if (wkind != FT_W_PER_SFT && wkind != FT_W_PER_SFT_BIN) return noalloc_fail(msg, cap, FT_ERR_ARG, "ft_eval_templates_noalloc: bad wkind");
+  if (!std::isfinite(f_min) || !std::isfinite(df) || !(df > 0.0) || !std::isfinite(t_ref) || !std::isfinite(rho_th))
+    return noalloc_fail(msg, cap, FT_ERR_ARG, "ft_eval_templates_noalloc: non-finite argument or df <= 0");
+  if (stat < 0 || stat > 2) return noalloc_fail(msg, cap, FT_ERR_ARG, "ft_eval_templates_noalloc: stat must be power, hough or both");
+  if (n < 0 || (n > 0 && !templates_dev)) return noalloc_fail(msg, cap, FT_ERR_ARG, "ft_eval_templates_noalloc: NULL list");
+  if (n > (int64_t)FT_NOALLOC_MAX_TEMPLATES)
+    return noalloc_fail(msg, cap, FT_ERR_ARG,
+                        "ft_eval_templates_noalloc: n = %lld exceeds FT_NOALLOC_MAX_TEMPLATES = %d, the size of the built-in "
+                        "work space; evaluate the bank in batches", (long long)n, FT_NOALLOC_MAX_TEMPLATES);
+  if (n == 0) return FT_OK;
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return noalloc_fail(msg, cap, FT_ERR_CUDA, "ft_eval_templates_noalloc: no CUDA device (%s); there is no CPU fallback", cudaGetErrorString(e));
+  if (dev < 0 || dev >= kNoallocMaxDevices) return noalloc_fail(msg, cap, FT_ERR_ARG, "ft_eval_templates_noalloc: device ordinal %d not supported", dev);
+  const void* ptrs[7] = {P_dev, t_mid_dev, vel_dev, w_dev, templates_dev, out_power_dev, out_count_dev};
+  for (const void* p : ptrs)
+    if (p && !noalloc_on_device(p, dev))
+      return noalloc_fail(msg, cap, FT_ERR_ARG, "ft_eval_templates_noalloc: a pointer is not device memory of the current device %d", dev);
+  unsigned char* scratch = nullptr;
+  if ((e = ft_noalloc_scratch_ptr(dev, &scratch)) != cudaSuccess)   // first call on this device: symbol look-up (set-up)
+    return noalloc_fail(msg, cap, FT_ERR_CUDA, "ft_eval_templates_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  FtDev d{};
+  d.P = P_dev; d.w = w_dev; d.t_mid = t_mid_dev; d.vel = vel_dev;
+  d.n_sft = n_sft; d.n_bins = n_bins; d.ld = ld_bins; d.wkind = wkind;
+  d.f_min = f_min; d.inv_df = 1.0 / df; d.rho = (float)rho_th;
+  uint32_t* perm = n >= 4096 ? reinterpret_cast<uint32_t*>(scratch) : nullptr;   // same ordering policy as ft_eval_templates
+  int32_t* flag_dev = reinterpret_cast<int32_t*>(scratch + kNoallocTail);
+  unsigned long long* ties_dev = reinterpret_cast<unsigned long long*>(scratch + kNoallocTail + 8);
+  struct { int32_t flag; int32_t pad; unsigned long long ties; } tail{0, 0, 0};
+  static_assert(sizeof(tail) == 16, "tail layout");
+  {
+    std::lock_guard<std::mutex> busy(g_noalloc_call_mu[dev]);   // held until the stream has drained: calls must not overlap
+    // the array keeps the last call's contents: flag and counter start at zero here, the histogram inside launch_list
+    if ((e = cudaMemsetAsync(scratch + kNoallocTail, 0, 16, s)) != cudaSuccess)
+      return noalloc_fail(msg, cap, FT_ERR_CUDA, "ft_eval_templates_noalloc: cudaMemsetAsync: %s", cudaGetErrorString(e));
+    int launches = 0;
+    e = launch_list<false, false>(d, stat, reinterpret_cast<const FtTemplateDev*>(templates_dev), FtBankBox{}, 0, 0, n, t_ref,
+                                  out_power_dev, out_count_dev, flag_dev, ties_dev, nullptr, nullptr, perm, s, &launches);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&tail, scratch + kNoallocTail, 16, cudaMemcpyDeviceToHost, s);
+    const cudaError_t e2 = cudaStreamSynchronize(s);
+    if (e == cudaSuccess) e = e2;
+  }
+  if (e != cudaSuccess) return noalloc_fail(msg, cap, FT_ERR_CUDA, "ft_eval_templates_noalloc: %s", cudaGetErrorString(e));
+  if (near_ties_host) *near_ties_host = tail.ties;
+  if (tail.flag)
+    return noalloc_fail(msg, cap, FT_ERR_TRACK_RANGE, "ft_eval_templates_noalloc: some tracks leave the spectrogram (their outputs are NaN / -1)");
   return FT_OK;
 }
 
