@@ -575,6 +575,35 @@ def test_standardised_statistic_is_zero_mean_unit_variance_in_noise(golden):
             assert np.allclose(sigma, math.sqrt((w ** 2).sum()), rtol=1e-12)
 
 
+def test_standardised_statistic_with_per_bin_weights_uses_row_means():
+    """Eq. (36) under per-(SFT, bin) weights (reading R21): the box-level weights are the row means
+    m_a = mean_k w[a][k] over the n_bins bins of the spectrogram, so sigma_G = sqrt(sum_a m_a^2) and
+    z = (s - sum_a m_a) / sigma_G for EVERY template, recomputed here in numpy from the weight array alone.
+    Catches: a mean over the leading dimension instead of n_bins, a missing division, the gathered w[a][k_a] used
+    in the moments, sigma_G from sum m instead of sum m^2."""
+    wl = W.config4(n_sft=120, n_sky=4, band_hz=0.2, n_lines=5)
+    assert wl.per_bin_weights
+    # the last two columns become row padding (ld = n_bins + 2): a mean over the leading dimension would differ
+    nb = wl.n_bins - 2
+    wl.w[:, nb:] *= np.float32(7.0)
+    o = fo.Oracle(wl)
+    o.pb.n_bins -= 2
+    power, _, _, _, z, sigma = o.eval_range_z()
+    m = wl.w[:, :nb].astype(np.float64).mean(axis=1)      # [n_sft] row means over the n_bins bins
+    assert not np.allclose(m, wl.w.astype(np.float64).mean(axis=1), rtol=1e-6)
+    mu, sg = m.sum(), math.sqrt((m ** 2).sum())
+    assert np.allclose(sigma, sg, rtol=1e-12, atol=0) and np.ptp(sigma) == 0.0
+    assert np.allclose(z, (power - mu) / sg, rtol=0, atol=1e-9)
+    # the line bins make rows uneven: the gathered weight differs from the row mean, so a slip would show
+    assert abs(power.mean() - mu) < 0.2 * mu and np.ptp(wl.w, axis=1).max() > 0.0
+    # the statistic itself is the gathered-weight sum: brute force for three templates
+    for idx in (0, int(power.size // 2), int(power.size - 1)):
+        k, _, rc = o.track(idx)
+        assert rc == 0
+        a = np.arange(wl.n_sft)
+        assert abs(power[idx] - (wl.w[a, k].astype(np.float64) * wl.P[a, k].astype(np.float64)).sum()) < 1e-12
+
+
 # ---------------------------------------------------------------- boxes (PAPER.md:338-342) and the veto (:496-502)
 def test_topk_per_region_against_python_sorted():
     """Catches: wrong region index, veto applied after instead of before the selection, tie order."""
