@@ -163,7 +163,7 @@ __global__ void k1_scatter_kernel(const __grid_constant__ FtDev d, const FtTempl
   if (j < n) perm[atomicAdd(cursor + k1_bucket<GEN>(d, tl, bx, seed, first, j), 1u)] = (uint32_t)j;
 }
 
-struct K1Acc { double power; int32_t count; unsigned ties; unsigned bad; };
+struct K1Acc { double power; int32_t count; unsigned ties; unsigned bad; double wsum; };
 
 #ifndef FT_K1_INT_CVT
 #define FT_K1_INT_CVT 0   // fp32 -> fp64 by the conversion instruction (0: measured faster, one issue slot) or by integer moves (1)
@@ -180,10 +180,13 @@ __device__ __forceinline__ double k1_f2d(float x) {
 // loop body), 2 every template is (cosine without a branch), 1 mixed (cosine under a per-thread branch).  PERSFT: per-SFT weights (staged as
 // doubles) or per-bin weights (gathered like the pixel).  The loop has no branch: an out-of-range bin is clamped
 // for the load and remembered in acc.bad (the template's outputs are then discarded).
-template <int STAT, int BIN, bool PERSFT>
+// SKY: sky-dependent weights (Eq. 4-5, ft_set_antenna): the weight of SFT a is u_a(n) w_a, u = a^2 + b^2 from the
+// staged antenna coefficients sAnt[9 c ..] and the template's sky factors sk; acc.wsum carries sum_a u_a w_a and the
+// caller divides by it at the end (the order of ft_refine_one).  Implies per-SFT weights.
+template <int STAT, int BIN, bool PERSFT, bool SKY>
 __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp, double Om, double apOm, bool binary,
-                                         const double2* sA, const double2* sB, const double2* sC, int m, int64_t a0,
-                                         uint32_t n_bins, K1Acc& acc) {
+                                         const double2* sA, const double2* sB, const double2* sC, const double* sAnt,
+                                         const FtSkyPoint& sk, int m, int64_t a0, uint32_t n_bins, K1Acc& acc) {
   const float* __restrict__ prow = d.P + a0 * d.ld;
   const float* __restrict__ wrow = d.w + a0 * d.ld;
   const int64_t ld = d.ld;
@@ -215,8 +218,12 @@ __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp
     const uint32_t kc = min(k, n_bins - 1u);
     const float pix = __ldg(prow + kc);
     if (STAT != 1) {
-      const double w = PERSFT ? sC[c].x : k1_f2d(__ldg(wrow + kc));
-      acc.power = fma(w, k1_f2d(pix), acc.power);  // exact product: same as mul then add
+      double w = PERSFT ? sC[c].x : k1_f2d(__ldg(wrow + kc));
+      if (SKY) {
+        w = __dmul_rn(ft_antenna_u(sAnt + 9 * c, sk), w);
+        acc.wsum = __dadd_rn(acc.wsum, w);
+      }
+      acc.power = fma(w, k1_f2d(pix), acc.power);  // (fixed weights: exact product, same as mul then add)
     }
     if (STAT != 0) acc.count += (pix > d.rho) ? 1 : 0;
     prow += ld;
@@ -226,7 +233,7 @@ __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp
 
 // STAT: 0 power, 1 count, 2 both.  GEN: templates drawn in registers from (seed, first + q) instead of read.
 // BEST: per-CTA loudest (value desc, index asc) to best_v / best_i [gridDim.x].
-template <int STAT, bool GEN, bool BEST>
+template <int STAT, bool GEN, bool BEST, bool SKY>
 __global__ void __launch_bounds__(K1_THREADS)
 ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict__ tl, const __grid_constant__ FtBankBox bx,
                uint64_t seed, uint64_t first, int64_t n, double t_ref,
@@ -235,6 +242,7 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
                const uint32_t* __restrict__ perm) {
   // per-SFT tables of the current chunk: (vx, vy), (vz, t - t_ref), (w, t): three LDS.128 per evaluation at most
   __shared__ double2 sA[K1_THREADS], sB[K1_THREADS], sC[K1_THREADS];
+  __shared__ double sAnt[SKY ? 9 * K1_THREADS : 1];   // antenna coefficients A[5], B[4] of the chunk's SFTs
   const int64_t slot = (int64_t)blockIdx.x * K1_THREADS + threadIdx.x;
   const bool active = slot < n;
   const int64_t q = active ? (perm ? (int64_t)perm[slot] : slot) : 0;   // the template this thread evaluates
@@ -246,7 +254,9 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
   const bool all_binary = __syncthreads_and(binary || !active) != 0;
   const uint32_t n_bins = (uint32_t)min(d.n_bins, (int64_t)0x7fffffff);
   const bool per_sft = d.wkind == 1;
-  K1Acc acc{0.0, 0, 0u, 0u};
+  K1Acc acc{0.0, 0, 0u, 0u, 0.0};
+  FtSkyPoint sk{};
+  if (SKY) sk = ft_sky_point(tp.nx, tp.ny, tp.nz);
   for (int64_t a0 = 0; a0 < d.n_sft; a0 += K1_THREADS) {
     const int64_t a = a0 + threadIdx.x;
     __syncthreads();
@@ -255,23 +265,31 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
       sA[threadIdx.x] = make_double2(d.vel[3 * a], d.vel[3 * a + 1]);
       sB[threadIdx.x] = make_double2(d.vel[3 * a + 2], __dsub_rn(t, t_ref));
       sC[threadIdx.x] = make_double2(per_sft ? (double)d.w[a] : 0.0, t);
+      if (SKY) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) sAnt[9 * threadIdx.x + q] = d.ant[9 * a + q];
+      }
     }
     __syncthreads();
     const int m = (int)min((int64_t)K1_THREADS, d.n_sft - a0);
     if (active) {
-      if (all_binary) {
-        if (per_sft) k1_chunk<STAT, 2, true>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
-        else k1_chunk<STAT, 2, false>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+      if (SKY) {   // (sky-dependent weights need per-SFT weights: ft_set_antenna)
+        if (all_binary) k1_chunk<STAT, 2, true, true>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else if (any_binary) k1_chunk<STAT, 1, true, true>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 0, true, true>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+      } else if (all_binary) {
+        if (per_sft) k1_chunk<STAT, 2, true, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 2, false, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
       } else if (any_binary) {
-        if (per_sft) k1_chunk<STAT, 1, true>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
-        else k1_chunk<STAT, 1, false>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+        if (per_sft) k1_chunk<STAT, 1, true, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 1, false, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
       } else {
-        if (per_sft) k1_chunk<STAT, 0, true>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
-        else k1_chunk<STAT, 0, false>(d, tp, Om, apOm, binary, sA, sB, sC, m, a0, n_bins, acc);
+        if (per_sft) k1_chunk<STAT, 0, true, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 0, false, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
       }
     }
   }
-  const double power = acc.power;
+  const double power = SKY ? acc.power / acc.wsum : acc.power;   // Eq. (5): sum_a w_a(n) = 1
   const int32_t count = acc.count;
   const bool bad = acc.bad != 0u;
   if (active) {
@@ -395,9 +413,12 @@ cudaError_t launch_list(const FtDev& d, int stat, const FtTemplateDev* tl, const
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     *launches += 3;
   }
-  if (stat == 0) ft_list_kernel<0, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
-  else if (stat == 1) ft_list_kernel<1, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
-  else ft_list_kernel<2, GEN, BEST><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
+  const bool sky = d.skyw && d.ant && stat != 1;   // (the number count does not see the weights)
+  if (stat == 0 && sky) ft_list_kernel<0, GEN, BEST, true><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
+  else if (stat == 0) ft_list_kernel<0, GEN, BEST, false><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
+  else if (stat == 1) ft_list_kernel<1, GEN, BEST, false><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
+  else if (sky) ft_list_kernel<2, GEN, BEST, true><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
+  else ft_list_kernel<2, GEN, BEST, false><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
   *launches += 1;
   return cudaGetLastError();
 }

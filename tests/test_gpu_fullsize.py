@@ -95,6 +95,105 @@ def test_full_size_sampled_outputs_and_candidates(cfg):
     ctx.close()
 
 
+def test_config2_full_size_packed_number_count():
+    """The packed number-count kernel (K2H, ft_tile8.cu) at the size bench.py times it at (config 2: 20 000 sky x
+    1800 f0 x 5 f1 x 4000 SFTs, eighteen 224-SFT folds of the 8-bit lanes into the 16-bit level): the full count
+    array against the oracle on 4096 sampled templates and on EVERY template of one sub-band, bit for bit; the
+    top-10 by count of every band re-evaluated one by one, and that band's candidates against the oracle's sort."""
+    wl = _full(2)
+    g = wl.grid
+    o = fo.Oracle(wl)
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    ctx = H.gpu_context(wl)
+    _, gc = H.gpu_full(ctx, wl, stat="hough")
+    assert "packed tile kernel" in ctx.describe()
+    rng = np.random.Generator(np.random.PCG64(212))
+    idx = np.unique(rng.integers(0, g.n_templates, 4096).astype(np.uint64))
+    _, oc, _, otie = o.eval_list(idx)
+    ok = otie == 0
+    assert np.array_equal(gc[idx.astype(np.int64)][ok], oc[ok])
+    b = 13
+    n_pt = g.n_templates // g.n_f0
+    cols = np.arange(b * bpb, min(g.n_f0, (b + 1) * bpb), dtype=np.uint64)
+    bidx = (np.arange(n_pt, dtype=np.uint64)[:, None] * np.uint64(g.n_f0) + cols[None, :]).reshape(-1)
+    bp, bc, _, btie = o.eval_list(bidx)
+    okb = btie == 0
+    assert np.array_equal(gc[bidx.astype(np.int64)][okb], bc[okb])
+    assert int((~okb).sum()) <= H.near_tie_bound(wl, bidx.size * wl.n_sft)
+    ctx.eval(g, "hough", wl.rho_th)
+    cands = ctx.topk_per_band(wl.band_width, wl.k, n_bands)
+    assert cands.shape == (n_bands, wl.k) and np.all(cands["idx"] != PAD)
+    flat = cands.reshape(-1)
+    cp, cc, cw, _ = o.eval_list(flat["idx"])
+    assert np.array_equal(flat["count"], cc) and np.array_equal(flat["power"], cp) and np.array_equal(flat["wcount"], cw)
+    for bb in range(n_bands):
+        c = cands[bb]
+        assert np.all((c["idx"] % np.uint64(g.n_f0)).astype(np.int64) // bpb == bb)
+        key = list(zip(-c["count"].astype(np.int64), c["idx"]))
+        assert key == sorted(key)
+    order = np.lexsort((bidx, -bc.astype(np.int64)))[:wl.k]
+    # (a template flagged as a near-tie may legitimately differ by one hit: it matters only within one hit of the k-th count)
+    risky = (~okb) & (bc >= bc[order[-1]] - 1)
+    assert not risky.any(), "re-seed: a near-tie template sits at the selection boundary"
+    assert np.array_equal(cands[b]["idx"], bidx[order]) and np.array_equal(cands[b]["count"], bc[order])
+    ctx.close()
+
+
+def test_config2_full_size_sky_dependent_weights():
+    """The row-weighted tile kernel (K2W, ft_tilew.cu; Eq. 4-5) at the size bench.py times it at, with the paper's
+    post-processing on top (loudest template per box of sky points x sub-band, ranked by z, Eq. 36): sampled
+    outputs of the full array within 1e-5 of the oracle; every candidate re-evaluated by the oracle (the library
+    evaluates a, b through per-SFT and per-sky tables: power, z, sigma_G to 1e-12, count exact); and one whole
+    region (625 outer points x 90 f0 x 4000 SFTs) against the oracle's own sort of z."""
+    wl = _full(2)
+    g = wl.grid
+    ant = W.antenna_geometry(wl)
+    o = fo.Oracle(wl, antenna=ant)
+    bpb = int(round(wl.band_width / g.df0)); n_bands = -(-g.n_f0 // bpb)
+    ctx = H.gpu_context(wl)
+    ctx.set_antenna(*ant)
+    gp, _ = H.gpu_full(ctx, wl, stat="power")
+    assert "row-weighted" in ctx.describe()
+    rng = np.random.Generator(np.random.PCG64(213))
+    idx = np.unique(rng.integers(0, g.n_templates, 2048).astype(np.uint64))
+    op, _, _, otie = o.eval_list(idx)
+    ok = otie == 0
+    rel = np.abs(gp[idx.astype(np.int64)].astype(np.float64) - op) / op
+    assert rel[ok].max() <= H.POWER_RTOL, rel[ok].max()
+    n_pt = g.n_templates // g.n_f0
+    n_pbox = 160
+    pbox = (np.arange(n_pt, dtype=np.int64) * n_pbox // n_pt).astype(np.int32)
+    ctx.eval(g, "power", wl.rho_th)
+    cands = ctx.topk_per_box(pbox, n_pbox, wl.band_width, 1, rank_by_z=True)
+    assert cands.shape == (n_pbox * n_bands, 1) and np.all(cands["idx"] != PAD)
+    flat = cands.reshape(-1)
+    rsel = np.random.Generator(np.random.PCG64(214)).choice(flat.size, 400, replace=False)
+    for c in flat[rsel]:
+        i = int(c["idx"])
+        p1, c1, w1, _, z1, s1 = o.eval_range_z(i, i + 1)
+        assert abs(c["power"] - p1[0]) <= 1e-12 * p1[0] and c["count"] == c1[0]
+        assert abs(c["z"] - z1[0]) <= 1e-9 * max(1.0, abs(z1[0])) and abs(c["sigma"] - s1[0]) <= 1e-12 * s1[0]
+        assert c["box"] == pbox[i // g.n_f0] * n_bands + (i % g.n_f0) // bpb
+    # one whole region: box 57 x band 6, every template by the oracle, plain sort of z
+    pb, b = 57, 6
+    pts = np.flatnonzero(pbox == pb)
+    zs, ps, ids, tie = [], [], [], []
+    for pt in pts:
+        lo = int(pt) * g.n_f0 + b * bpb
+        p1, _, _, t1, z1, _ = o.eval_range_z(lo, lo + bpb)
+        zs.append(z1); ps.append(p1); ids.append(np.arange(lo, lo + bpb, dtype=np.uint64)); tie.append(t1)
+    zs, ps, ids, tie = np.concatenate(zs), np.concatenate(ps), np.concatenate(ids), np.concatenate(tie)
+    relr = np.abs(gp[ids.astype(np.int64)].astype(np.float64) - ps) / ps      # the full fp32 array on the whole region
+    assert relr[tie == 0].max() <= H.POWER_RTOL
+    j = int(np.lexsort((ids, -zs))[0])
+    got = cands[pb * n_bands + b, 0]
+    srt = np.sort(zs)
+    # (a near-tie template may land one bin off: it matters only if its z is within reach of the top)
+    assert not ((tie != 0) & (zs > srt[-1] - 1.0)).any() and srt[-1] - srt[-2] > 1e-9, "re-seed: ambiguous winner"
+    assert int(got["idx"]) == int(ids[j]) and abs(got["z"] - zs[j]) <= 1e-9 * max(1.0, abs(zs[j]))
+    ctx.close()
+
+
 def test_config3_ranked_by_count_full_size():
     wl = _full(3)
     g = wl.grid

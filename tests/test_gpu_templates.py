@@ -146,6 +146,58 @@ def test_bank_draw_and_eval_bank_match_oracle(cfg, binary):
     ctx.close()
 
 
+@pytest.mark.parametrize("cfg,binary", [(2, False), (3, True)])
+def test_unstructured_bank_with_sky_dependent_weights(cfg, binary):
+    """Eq. (4)-(5) on the path the paper uses them on (random banks): after ft_set_antenna,
+    ft_eval_templates and ft_eval_bank weight every template by the antenna pattern of ITS sky point.  Against the
+    oracle's explicit-list evaluation with the same antenna tables: power to 1e-6, counts bit-exact, the loudest
+    template of a drawn batch; and the values differ from the fixed-weight ones (the feature is not vacuous)."""
+    import torch
+    wl = {2: lambda: W.config2(n_sft=501, n_sky=7, band_hz=0.35),
+          3: lambda: W.config3(n_sft=403, n_ap=3, n_porb=3, n_tasc=2, n_inj=0)}[cfg]()
+    ant = W.antenna_geometry(wl)
+    o = fo.Oracle(wl, antenna=ant)
+    ctx = H.gpu_context(wl)
+    fixed_p, fixed_c = _run(ctx, W.random_bank(wl, 5003, seed=6), wl.grid.t_ref)
+    ctx.set_antenna(*ant)
+    for n in (5003, 700):           # with and without the f0 ordering
+        tl = W.random_bank(wl, n, seed=6)
+        if cfg == 3:                # several sky points, so that the weights differ between templates
+            sky = W.config2(n_sft=8, n_sky=n).grid.sky
+            tl["nx"], tl["ny"], tl["nz"] = sky[:, 0], sky[:, 1], sky[:, 2]
+        op, oc, _, otie = fo.eval_templates(o, tl.astype(fo.TEMPLATE_DTYPE), wl.grid.t_ref)
+        gp, gc = _run(ctx, tl, wl.grid.t_ref)
+        ok = otie == 0
+        assert np.array_equal(gc[ok], oc[ok])
+        rel = np.abs(gp.astype(np.float64) - op) / op
+        assert rel[ok].max() <= 1e-6, rel[ok].max()
+        gp1, _ = _run(ctx, tl, wl.grid.t_ref, stat="power")
+        assert np.array_equal(gp1, gp)
+        if n == 5003 and cfg == 2:
+            assert np.array_equal(gc, fixed_c) and np.abs(gp / fixed_p - 1).max() > 1e-3
+    # a drawn bank: every statistic and the winner, which ft_eval_bank re-evaluates in fp64 with the same weights
+    box = _box(wl, binary)
+    n, seed, first = 4500, 23, 77
+    otl = fo.bank_draw(box, seed, first, n)
+    op, oc, owc, otie = fo.eval_templates(o, otl, box["t_ref"])
+    dev = torch.device("cuda:0")
+    gp = torch.full((n,), float("nan"), dtype=torch.float32, device=dev)
+    best, _ = ctx.eval_bank(box, seed, first, n, "power", wl.rho_th, out_power=gp)
+    gp = gp.cpu().numpy()
+    ok = otie == 0
+    assert (np.abs(gp.astype(np.float64) - op) / op)[ok].max() <= 1e-6
+    j = int(np.lexsort((np.arange(n), -op))[0])
+    if ok[j] and (np.sort(op)[-1] - np.sort(op)[-2]) > 1e-6 * op[j]:
+        assert int(best["idx"]) == j
+        assert abs(best["power"] - op[j]) <= 1e-12 * op[j] and best["count"] == oc[j]
+        assert abs(best["wcount"] - owc[j]) <= 1e-12 * owc[j]
+    # back to the weights as given
+    ctx.set_antenna(None)
+    back_p, back_c = _run(ctx, W.random_bank(wl, 5003, seed=6), wl.grid.t_ref)
+    assert np.array_equal(back_p, fixed_p) and np.array_equal(back_c, fixed_c)
+    ctx.close()
+
+
 def test_track_of_a_template_equals_the_oracles():
     wl = W.config3(n_sft=403, n_ap=3, n_porb=3, n_tasc=2, n_inj=0)
     tl = W.random_bank(wl, 20, seed=5)
