@@ -34,7 +34,8 @@
  * BORROWED until ft_destroy (inputs) or until the call's work has completed on the stream
  * (outputs).  "host" pointers are read during the call and copied.  All device work is enqueued
  * on the CUDA stream given to ft_create; calls that write host memory synchronise that stream
- * before returning.  A handle is not thread-safe.  There is no CPU fallback: without a CUDA
+ * before returning.  A handle is not thread-safe; different handles may be driven from different host threads (the
+ * process-wide tables of the library are guarded).  There is no CPU fallback: without a CUDA
  * device ft_create fails with FT_ERR_CUDA.
  */
 #ifndef FASTTRACKS_B200_H

@@ -149,6 +149,10 @@ struct FtCandDev {
   double sigma;    // sigma_G
 };
 
+// Number of SMs of the CURRENT device (cudaDevAttrMultiProcessorCount, looked up once per device; 148 on a B200):
+// grids of helper launches, the threshold sample and the split tail are sized from it.  Thread-safe.  (ft_tile.cu)
+int ft_sm_count();
+
 // ---- host-visible launchers (defined in the .cu files) ---------------------------------------
 struct FtSelectBuffers;  // ft_select.cu
 

@@ -578,9 +578,9 @@ int ft_selftest(ft_ctx* c, int which, int64_t n, uint64_t seed, uint64_t* n_fail
   FT_CUDA(c, ft_grow(c->io_dev, c->io_cap, 8));
   unsigned long long* nf = reinterpret_cast<unsigned long long*>(c->io_dev);
   FT_CUDA(c, cudaMemsetAsync(nf, 0, 8, c->stream));
-  if (which == 0) ft_selftest_div_kernel<<<148 * 8, 256, 0, c->stream>>>(seed, n, nf);
-  else if (which == 1) ft_selftest_cvt_kernel<<<148 * 8, 256, 0, c->stream>>>(n, nf);
-  else ft_selftest_cos_kernel<<<148 * 8, 256, 0, c->stream>>>(seed, n, nf);
+  if (which == 0) ft_selftest_div_kernel<<<ft_sm_count() * 8, 256, 0, c->stream>>>(seed, n, nf);
+  else if (which == 1) ft_selftest_cvt_kernel<<<ft_sm_count() * 8, 256, 0, c->stream>>>(n, nf);
+  else ft_selftest_cos_kernel<<<ft_sm_count() * 8, 256, 0, c->stream>>>(seed, n, nf);
   FT_CUDA(c, cudaGetLastError());
   c->counters.kernel_launches += 1;
   unsigned long long h = 0;

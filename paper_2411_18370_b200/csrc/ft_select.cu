@@ -305,7 +305,7 @@ cudaError_t ft_select_threshold(const float* keys, int64_t n_rows, int64_t n_f0,
 cudaError_t ft_select_append_keys(const float* keys, int64_t n_rows, int64_t n_f0, const FtRowMap& map,
                                   FtSelectDev sel, cudaStream_t s) {
   const int64_t n = n_rows * n_f0;
-  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, (int64_t)ft_sm_count() * 16);
   ft_append_from_keys_kernel<<<grid, 256, 0, s>>>(keys, n_rows, n_f0, map, sel);
   return cudaGetLastError();
 }
@@ -338,7 +338,7 @@ cudaError_t ft_select_trim_refined(const FtCandDev* cand, const uint32_t* off, i
 }
 
 cudaError_t ft_count_to_key(const int32_t* c, float* k, int64_t n, cudaStream_t s) {
-  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, (int64_t)ft_sm_count() * 16);
   ft_count_to_key_kernel<<<grid, 256, 0, s>>>(c, k, n);
   return cudaGetLastError();
 }
@@ -349,19 +349,19 @@ cudaError_t ft_select_tighten(FtSelectDev sel, uint32_t k, FtMargin margin, cuda
 }
 
 cudaError_t ft_fill_f32(float* p, int64_t n, float v, cudaStream_t s) {
-  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, (int64_t)ft_sm_count() * 16);
   ft_fill_f32_kernel<<<grid, 256, 0, s>>>(p, n, v);
   return cudaGetLastError();
 }
 
 cudaError_t ft_keys_affine(float* keys, int64_t n, double mu, double inv_sigma, cudaStream_t s) {
-  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, (int64_t)ft_sm_count() * 16);
   ft_keys_affine_kernel<<<grid, 256, 0, s>>>(keys, n, mu, inv_sigma);
   return cudaGetLastError();
 }
 
 cudaError_t ft_select_mask_keys_local(float* keys, const int32_t* counts, int64_t n, int32_t floor, cudaStream_t s) {
-  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  const unsigned grid = (unsigned)std::min<int64_t>((n + 255) / 256, (int64_t)ft_sm_count() * 16);
   ft_mask_keys_local_kernel<<<grid, 256, 0, s>>>(keys, counts, n, floor);
   return cudaGetLastError();
 }

@@ -17,6 +17,7 @@
 // the same kernel.  The kernel body is ft_tile_body (ft_tile_dev.cuh); this file instantiates it for the
 // plain fp32 gather and holds the host side: tiling choice, strip table, launch.
 #include <algorithm>
+#include <mutex>
 #include <cmath>
 #include <vector>
 
@@ -141,12 +142,28 @@ cudaError_t launch_J(const FtDev& d, const FtTileArgs& a, unsigned grid, unsigne
 
 }  // namespace
 
+int ft_sm_count() {
+  static std::mutex mu;
+  static int count[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+  std::lock_guard<std::mutex> lock(mu);
+  if (count[dev] == 0) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    count[dev] = n;
+  }
+  return count[dev];
+}
+
 // The opt-in to > 48 KB of dynamic shared memory is per function AND per device: remember the devices a
 // function has been configured on (a bit per device; a process may drive several GPUs).
 cudaError_t ft_tile_allow_smem(const void* func) {
   struct Seen { const void* f; unsigned long long mask; };
   static Seen seen[128];
   static int n_seen = 0;
+  static std::mutex mu;                       // handles on different host threads share this table
+  std::lock_guard<std::mutex> lock(mu);
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
@@ -319,26 +336,26 @@ bool ft_tile_finish(const FtDev& d, FtTilePlan* plan, int32_t max_w, std::string
   return true;
 }
 
-// Outer points of the threshold sample: one wave of CTA groups (148), more only when the bank is so large
+// Outer points of the threshold sample: one wave of CTA groups (one per SM), more only when the bank is so large
 // that the fused pass would append more than cap / 8 entries per band (appended ~ k * groups / sample groups).
 uint64_t ft_tile_sample_points(const FtTilePlan& plan, uint64_t n_points, uint32_t k, uint32_t cap) {
   const uint64_t R = (uint64_t)plan.R;
   const uint64_t n_groups = (n_points + R - 1) / R;
-  uint64_t n_sg = std::max<uint64_t>(148, (8ull * k * n_groups + cap - 1) / std::max<uint32_t>(cap, 1u));
+  uint64_t n_sg = std::max<uint64_t>((uint64_t)ft_sm_count(), (8ull * k * n_groups + cap - 1) / std::max<uint32_t>(cap, 1u));
   n_sg = std::min(n_sg, n_groups);
   return std::min(n_sg * R, n_points);
 }
 
-// Split tail: a launch of n_groups CTA groups (n_skip of them exit at once) runs (n_groups - n_skip) / 148 waves; the
+// Split tail: a launch of n_groups CTA groups (n_skip of them exit at once) runs (n_groups - n_skip) / n_SM waves; the
 // last, partial wave would leave SMs idle for up to a whole CTA time.  Its groups are split in S parts of R / S points
-// each (S the largest divisor of R with rem * n_tiles * S <= 148), run by CTAs with that many fewer consumer warps.
+// each (S the largest divisor of R with rem * n_tiles * S <= n_SM), run by CTAs with that many fewer consumer warps.
 // Plans with one CTA per SM only.  Sets a->main_groups / main_ctas / tail_split and returns the grid size.
 static uint64_t ft_split_tail(const FtTilePlan& plan, uint64_t n_groups, const uint32_t* skip_sorted, uint32_t n_skip,
                               FtTileArgs* a) {
   a->tail_split = 1; a->main_groups = 0; a->main_ctas = 0;
   const uint64_t nt = (uint64_t)plan.n_tiles;
   const uint64_t grid1 = n_groups * nt;
-  constexpr uint64_t kSMs = 148;
+  const uint64_t kSMs = (uint64_t)ft_sm_count();
   if (plan.mode == 1 || plan.ctas_per_sm != 1 || n_skip > n_groups) return grid1;   // (mode 1: see ft_tile_body)
   const uint64_t eff = n_groups - n_skip;                 // groups that run (n_tiles CTAs each)
   const uint64_t W = eff * nt / kSMs;                     // full waves
@@ -424,7 +441,7 @@ cudaError_t ft_launch_tile(const FtDev& d, const FtTilePlan& plan, const FtTileR
 }
 
 cudaError_t ft_launch_hitmap(const float* P, float rho, float* H, int64_t n, cudaStream_t s) {
-  ft_hitmap_kernel<<<148 * 8, 256, 0, s>>>(P, rho, H, n);
+  ft_hitmap_kernel<<<ft_sm_count() * 8, 256, 0, s>>>(P, rho, H, n);
   return cudaGetLastError();
 }
 

@@ -57,6 +57,6 @@ cudaError_t ft_tile8_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned
 
 cudaError_t ft_launch_hitmap8(const float* P, float rho, uint8_t* H8, int64_t n_sft, int64_t n_bins, int64_t ld,
                               int64_t ld8, cudaStream_t s) {
-  ft_hitmap8_kernel<<<148 * 8, 256, 0, s>>>(P, rho, H8, n_sft, n_bins, ld, ld8);
+  ft_hitmap8_kernel<<<ft_sm_count() * 8, 256, 0, s>>>(P, rho, H8, n_sft, n_bins, ld, ld8);
   return cudaGetLastError();
 }

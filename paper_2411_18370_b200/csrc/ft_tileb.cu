@@ -52,6 +52,6 @@ cudaError_t ft_tileb_launch(int J, const FtDev& d, const FtTileArgs& a, unsigned
 }
 
 cudaError_t ft_launch_qb(const float* Q, const float* P, float rho, float* QB, int64_t n, cudaStream_t s) {
-  ft_qb_kernel<<<148 * 8, 256, 0, s>>>(Q, P, rho, QB, n);
+  ft_qb_kernel<<<ft_sm_count() * 8, 256, 0, s>>>(Q, P, rho, QB, n);
   return cudaGetLastError();
 }
