@@ -15,6 +15,8 @@ import ctypes as C
 import os
 import subprocess
 
+import math
+
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -235,6 +237,58 @@ def mismatch(s_signal, s_template, mu_G):
     """Eq. (24) PAPER.md:190: m(lambda'; lambda) = (s(lambda) - s(lambda')) / (s(lambda) - mu_G)."""
     return (np.asarray(s_signal, dtype=np.float64) - np.asarray(s_template, dtype=np.float64)) / \
         (np.asarray(s_signal, dtype=np.float64) - mu_G)
+
+
+def n_templates(box: dict, T_sft: float, T_obs: float, v_over_c: float) -> float:
+    """Eq. (29) for the all-sky binary search, i.e. Eq. (A10) PAPER.md:589-598 with the density of Eq. (A9)
+    rho = k f0^5 a_p^2 Omega^3, k = T_SFT^6 T_obs (v/c)^2: the number of templates N(Delta lambda) that cover the
+    lambda-box `box` (keys BANK_FIELDS; sky as (alpha, sin delta), Omega = 2 pi / P_orb, phi_b over its full range
+    [0, 2 pi)).  Written out factor by factor in the order of Eq. (A10); f1 is not a resolved dimension there."""
+    k = T_sft ** 6 * T_obs * v_over_c ** 2
+    I_f0 = (box["f0_hi"] ** 6 - box["f0_lo"] ** 6) / 6.0                       # int df0 f0^5
+    I_sky = (box["ra_hi"] - box["ra_lo"]) * (box["sd_hi"] - box["sd_lo"])      # int dalpha dsin(delta)
+    I_ap = (box["ap_hi"] ** 3 - box["ap_lo"] ** 3) / 3.0                       # int da_p a_p^2
+    Om_lo, Om_hi = 2.0 * math.pi / box["porb_hi"], 2.0 * math.pi / box["porb_lo"]
+    I_Om = (Om_hi ** 4 - Om_lo ** 4) / 4.0                                     # int dOmega Omega^3
+    I_phi = 2.0 * math.pi                                                      # int dphi_b
+    return k * I_f0 * I_sky * I_ap * I_Om * I_phi
+
+
+def mismatch_sampler(wl, box: dict, n_inj: int, oversampling: float, seed: int, amp: float, T_obs: float,
+                     v_over_c: float = 1e-4, n_bank=None):
+    """The sampling of p(m | o), step by step, for n_inj signals:
+      1. a noise data stream (the workload's spectrogram) containing a CW signal drawn from the search's priors --
+         signal j is template j of the xi-uniform stream `seed` over `box` (the density of Eq. A9), injected with
+         amplitude `amp` along its own track (the bins of Eq. 2 at every SFT);
+      2. o N(Delta lambda) templates (Eq. 29 / A10; rounded up, at least 1) drawn uniformly in xi over the box --
+         the stream `seed + 1 + j`;
+      3. the statistic of every one of them (Eq. 3) and m = (s(lambda) - max s(lambda')) / (s(lambda) - mu_G), Eq. (24),
+         with mu_G = sum_a w_a (Eq. 13 on the P = s/2 scale).
+    Returns dict(m [n_inj], s_signal, s_best, best [n_inj] positions in the bank stream, n_bank, N).  Per-SFT weights."""
+    assert not wl.per_bin_weights
+    N = n_templates(box, wl.T_sft, T_obs, v_over_c)
+    if n_bank is None:
+        n_bank = max(1, int(math.ceil(oversampling * N)))
+    mu_G = float(np.sum(wl.w.astype(np.float64)))
+    import copy
+    m = np.empty(n_inj); s_sig = np.empty(n_inj); s_best = np.empty(n_inj); best = np.empty(n_inj, dtype=np.int64)
+    for j in range(n_inj):
+        sig = bank_draw(box, seed, j, 1)
+        clean = Oracle(wl)
+        k, _, rc = clean.track_template(sig[0], box["t_ref"])
+        if rc != 0:
+            raise ValueError("oracle: the signal's track leaves the spectrogram")
+        wj = copy.copy(wl)
+        wj.P = wl.P.copy()
+        wj.P[np.arange(wl.n_sft), k] += np.float32(amp)
+        oj = Oracle(wj)
+        s_sig[j] = eval_templates(oj, sig, box["t_ref"])[0][0]
+        bank = bank_draw(box, seed + 1 + j, 0, n_bank)
+        sp = eval_templates(oj, bank, box["t_ref"])[0]
+        best[j] = int(np.lexsort((np.arange(n_bank), -sp))[0])
+        s_best[j] = sp[best[j]]
+        m[j] = mismatch(s_sig[j], s_best[j], mu_G)
+    return dict(m=m, s_signal=s_sig, s_best=s_best, best=best, n_bank=n_bank, N=N)
 
 
 BANK_FIELDS = ("f0_lo", "f0_hi", "f1_lo", "f1_hi", "ra_lo", "ra_hi", "sd_lo", "sd_hi", "ap_lo", "ap_hi",

@@ -634,6 +634,74 @@ def test_mismatch_definition_eq24():
     assert abs(fo.mismatch(3.0, 2.5, 1.0) - 0.25) < 1e-15
 
 
+def test_number_of_templates_eq_a10_against_quadrature_and_bank_density():
+    """N(Delta lambda) (Eq. 29 with the density of Eq. A9, closed form Eq. A10) against (a) numerical quadrature of
+    rho = k f0^5 a_p^2 Omega^3 over the box, one axis at a time (Simpson), and (b) the bank itself: a xi-uniform bank
+    puts the fraction N(sub-box) / N(box) of its templates into a sub-box.  Catches: a wrong exponent or factor 1/(p+1),
+    P_orb used where Omega is meant, a missing 2 pi of phi_b, sky as delta instead of sin delta."""
+    from scipy.integrate import simpson
+    box = dict(f0_lo=100.0, f0_hi=100.125, f1_lo=0.0, f1_hi=0.0, ra_lo=0.3, ra_hi=1.1, sd_lo=-0.2, sd_hi=0.5,
+               ap_lo=2.0, ap_hi=7.0, porb_lo=12 * 86400.0, porb_hi=40 * 86400.0, t_ref=0.0)
+    T_sft, T_obs, voc = 900.0, 180 * 86400.0, 1e-4
+    k = T_sft ** 6 * T_obs * voc ** 2
+
+    def quad(lo, hi, p):
+        x = np.linspace(lo, hi, 20001)
+        return simpson(x ** p, x=x)
+    num = (k * quad(box["f0_lo"], box["f0_hi"], 5) * (box["ra_hi"] - box["ra_lo"]) * (box["sd_hi"] - box["sd_lo"])
+           * quad(box["ap_lo"], box["ap_hi"], 2) * quad(2 * math.pi / box["porb_hi"], 2 * math.pi / box["porb_lo"], 3) * 2 * math.pi)
+    N = fo.n_templates(box, T_sft, T_obs, voc)
+    assert abs(N - num) < 1e-9 * num
+    # k = T_SFT^6 T_obs (v/c)^2: N scales as the sixth power of T_SFT and linearly in T_obs
+    assert abs(fo.n_templates(box, 2 * T_sft, 3 * T_obs, voc) / N - 64 * 3) < 1e-9
+    # (b) the sub-box a_p < 5, P_orb < 20 d (i.e. Omega above 2 pi / 20 d), alpha < 0.6
+    sub = dict(box, ap_hi=5.0, porb_hi=20 * 86400.0, ra_hi=0.6)
+    frac = fo.n_templates(sub, T_sft, T_obs, voc) / N
+    n = 200000
+    tl = fo.bank_draw(box, 21, 0, n)
+    ra = np.arctan2(tl["ny"], tl["nx"])
+    inside = (tl["a_p"] < 5.0) & (tl["P_orb"] < 20 * 86400.0) & (ra < 0.6)
+    assert abs(inside.mean() - frac) < 5 * math.sqrt(frac * (1 - frac) / n), (inside.mean(), frac)
+
+
+def test_mismatch_sampler_noiseless_limits():
+    """PAPER.md:320-324 on a NOISELESS spectrogram (P = 0 plus the signal), where the answer is known: s(lambda) =
+    amp * sum w, mu_G = sum w, the best template recovers the fraction of SFTs on which its track coincides with the
+    signal's, so m = 1 - (weighted fraction of coinciding SFTs) in [0, 1], recomputed here from the tracks alone; and
+    a bank that contains the signal itself (zero-width box) gives m = 0 exactly.  Catches: the wrong sign or
+    denominator of Eq. (24), the signal injected along another template's track, the maximum taken over the wrong bank."""
+    wl = W.config3(n_sft=240, n_ap=2, n_porb=2, n_tasc=2, n_inj=0)
+    wl.P[:] = 0.0
+    g = wl.grid
+    n = g.sky[0]
+    ra = float(np.arctan2(n[1], n[0]) % (2 * math.pi)); sd = float(n[2])
+    f_mid = g.f0_start + 0.5 * g.n_f0 * g.df0
+    box = dict(f0_lo=f_mid, f0_hi=f_mid + 4 * g.df0, f1_lo=0.0, f1_hi=0.0, ra_lo=ra, ra_hi=ra + 1e-3, sd_lo=sd, sd_hi=sd + 1e-3,
+               ap_lo=4.0, ap_hi=4.2, porb_lo=20 * 86400.0, porb_hi=20.5 * 86400.0, t_ref=g.t_ref)
+    T_obs = float(wl.t_mid.max() - wl.t_mid.min())
+    r = fo.mismatch_sampler(wl, box, n_inj=3, oversampling=0.0, seed=5, amp=2.0, T_obs=T_obs, n_bank=300)
+    w = wl.w.astype(np.float64)
+    o = fo.Oracle(wl)
+    for j in range(3):
+        sig = fo.bank_draw(box, 5, j, 1)
+        ks, _, _ = o.track_template(sig[0], box["t_ref"])
+        assert abs(r["s_signal"][j] - 2.0 * w.sum()) < 1e-12
+        bank = fo.bank_draw(box, 5 + 1 + j, 0, 300)
+        frac = np.array([w[(o.track_template(t, box["t_ref"])[0] == ks)].sum() for t in bank]) / w.sum()
+        # mu_G = sum w enters Eq. (24) although the data hold no noise: m = (2 - 2 frac) / (2 - 1)
+        assert abs(r["m"][j] - (2.0 - 2.0 * frac.max()) / (2.0 - 1.0)) < 1e-12
+        assert int(r["best"][j]) == int(np.argmax(frac)) or np.sum(frac == frac.max()) > 1
+    point = dict(box, f0_hi=box["f0_lo"], ra_hi=ra, sd_hi=sd, ap_hi=4.0, porb_hi=20 * 86400.0)
+    # (phi_b still varies inside a zero-width box: pin the orbit phase by making the bank the signal's own stream)
+    sig = fo.bank_draw(point, 9, 0, 1)
+    wl2 = W.config3(n_sft=240, n_ap=2, n_porb=2, n_tasc=2, n_inj=0)
+    wl2.P[:] = 0.0
+    ks, _, _ = fo.Oracle(wl2).track_template(sig[0], g.t_ref)
+    wl2.P[np.arange(wl2.n_sft), ks] += np.float32(2.0)
+    sp = fo.eval_templates(fo.Oracle(wl2), sig, g.t_ref)[0]
+    assert fo.mismatch(sp[0], sp[0], w.sum()) == 0.0
+
+
 # ---------------------------------------------------------------- Eq. (A11): xi-uniform random banks
 BOX = dict(f0_lo=100.0, f0_hi=200.0, f1_lo=-1e-9, f1_hi=0.0, ra_lo=0.0, ra_hi=2 * math.pi, sd_lo=-1.0, sd_hi=1.0,
            ap_lo=1.0, ap_hi=10.0, porb_lo=10 * 86400.0, porb_hi=60 * 86400.0, t_ref=1000.0)
