@@ -251,3 +251,37 @@ def test_mismatch_sampler_workload():
         ms.append(m_gpu)
     assert ms[1] <= ms[0]
     ctx.close()
+
+
+def test_mismatch_sampler_against_the_oracles_sampler():
+    """SURVEY §8(f) row 4 as a workload (paper_2411_18370_b200/sampler.py): N(Delta lambda) by
+    Eq. (A10), o N templates per injected signal through ft_eval_bank, m by Eq. (24) -- against the oracle's own
+    step-by-step sampler on the same streams: the same bank sizes, the same loudest template, s_best to fp64
+    rounding, every m within 1e-5 (s(lambda) of the signal is the library's fp32 output); m < 1, and m is
+    non-increasing in the oversampling for every signal (the banks of one stream are nested), hence its median
+    (PAPER.md:326)."""
+    from paper_2411_18370_b200 import sampler as S
+    wl = W.config3(n_sft=403, n_ap=3, n_porb=3, n_tasc=2, n_inj=0)
+    g = wl.grid
+    n = g.sky[0]
+    ra = float(np.arctan2(n[1], n[0]) % (2 * np.pi)); sd = float(n[2])
+    f_mid = g.f0_start + 0.5 * g.n_f0 * g.df0
+    box = dict(f0_lo=f_mid, f0_hi=f_mid + 0.01, f1_lo=0.0, f1_hi=0.0, ra_lo=ra, ra_hi=ra + 0.02, sd_lo=sd - 0.01, sd_hi=sd + 0.01,
+               ap_lo=4.0, ap_hi=6.0, porb_lo=20 * 86400.0, porb_hi=25 * 86400.0, t_ref=g.t_ref)
+    T_obs = float(wl.t_mid.max() - wl.t_mid.min()) + wl.T_sft
+    N = S.n_templates(box, wl.T_sft, T_obs)
+    assert abs(N - fo.n_templates(box, wl.T_sft, T_obs, 1e-4)) <= 1e-12 * N and 20 < N < 5000, N
+    prev = None
+    for o in (0.25, 2.0, 16.0):
+        got = S.mismatch_samples(wl, box, n_inj=8, oversampling=o, seed=31, amp=3.0, T_obs=T_obs)
+        ref = fo.mismatch_sampler(wl, box, 8, o, 31, 3.0, T_obs)
+        assert got["n_bank"] == ref["n_bank"] == int(np.ceil(o * N)) and got["bank_templates"] == 8 * got["n_bank"]
+        assert np.array_equal(got["best"], ref["best"])
+        assert np.allclose(got["s_best"], ref["s_best"], rtol=1e-12, atol=0)
+        assert np.allclose(got["s_signal"], ref["s_signal"], rtol=1e-6, atol=0)
+        assert np.abs(got["m"] - ref["m"]).max() <= 1e-5
+        assert np.all(got["m"] < 1.0) and np.all(got["m"] > -0.5)
+        if prev is not None:
+            assert np.all(got["m"] <= prev + 1e-12) and np.median(got["m"]) <= np.median(prev)
+        prev = got["m"]
+    assert np.median(prev) < 0.9      # sixteen-fold oversampling recovers a good part of the signal
