@@ -270,6 +270,24 @@ int fto_eval_templates(const fto_problem* pb, const fto_template* tl, int64_t n,
   return status;
 }
 
+/* The same with the standardised statistic z (Eq. 36) and sigma_G of every template of the list: the quantities the
+ * paper's per-box procedure ranks a random bank by. */
+int fto_eval_templates_z(const fto_problem* pb, const fto_template* tl, int64_t n, double t_ref,
+                         double* power, int32_t* count, double* wcount, uint8_t* near_tie, double* z, double* sigma) {
+  int status = FTO_OK;
+#pragma omp parallel for schedule(static)
+  for (int64_t j = 0; j < n; ++j) {
+    const int rc = fto_one_params(pb, tl + j, t_ref, power ? power + j : NULL, count ? count + j : NULL,
+                                  wcount ? wcount + j : NULL, near_tie ? near_tie + j : NULL, NULL, NULL,
+                                  z ? z + j : NULL, sigma ? sigma + j : NULL);
+    if (rc != FTO_OK) {
+#pragma omp atomic write
+      status = rc;
+    }
+  }
+  return status;
+}
+
 /* Track (bins, positions) of ONE explicit template. */
 int fto_track_template(const fto_problem* pb, const fto_template* tp, double t_ref, int64_t* k_out, double* x_out) {
   return fto_one_params(pb, tp, t_ref, NULL, NULL, NULL, NULL, k_out, x_out, NULL, NULL);

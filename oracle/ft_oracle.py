@@ -192,6 +192,30 @@ def eval_templates(oracle: "Oracle", templates, t_ref: float):
     return o
 
 
+def eval_templates_z(oracle: "Oracle", templates, t_ref: float):
+    """eval_templates plus (z, sigma_G) of Eq. (36) for every template: (power, count, wcount, near_tie, z, sigma)."""
+    tl = np.ascontiguousarray(templates, dtype=TEMPLATE_DTYPE)
+    o = oracle._outs(tl.size) + (np.empty(tl.size, np.float64), np.empty(tl.size, np.float64))
+    oracle.lib.fto_eval_templates_z.restype = C.c_int
+    rc = oracle.lib.fto_eval_templates_z(C.byref(oracle.pb), tl.ctypes.data_as(C.c_void_p), C.c_int64(tl.size),
+                                         C.c_double(float(t_ref)), *[a.ctypes.data_as(C.c_void_p) for a in o])
+    if rc != 0:
+        raise ValueError(f"oracle: a track left the spectrogram (rc={rc})")
+    return o
+
+
+def loudest_of_bank(power, wcount, z, wcount_floor: float = 0.0, rank_by_z: bool = False):
+    """The paper's per-box step on a random bank (PAPER.md:476 "retrieve the loudest template per box", :496-502
+    "loudest normalized power ... subject to a minimal weighted number count", Eq. 36 :346): among the templates
+    whose weighted number count is >= wcount_floor, the one with the largest z (rank_by_z) or power; ties to the
+    lower position.  Returns its position, or -1 if the veto leaves none."""
+    key = np.asarray(z if rank_by_z else power, dtype=np.float64)
+    keep = np.flatnonzero(np.asarray(wcount) >= wcount_floor)
+    if keep.size == 0:
+        return -1
+    return int(keep[np.lexsort((keep, -key[keep]))[0]])
+
+
 def topk_per_band(values, n_f0: int, bins_per_band: int, k: int, idx_begin: int = 0):
     """Plain definition of the per-band top-k over a FULL statistic array.
 

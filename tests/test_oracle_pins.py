@@ -628,6 +628,33 @@ def test_topk_per_region_against_python_sorted():
     assert all(np.array_equal(x[0], y[0]) for x, y in zip(a, b))
 
 
+def test_explicit_templates_z_equals_grid_z_and_bank_loudest_under_veto():
+    """fto_eval_templates_z: a list that enumerates the grid gives eval_range_z's z and sigma_G exactly (fixed and
+    sky-dependent weights, where sigma_G differs between sky points); loudest_of_bank against Python's sorted().
+    Catches: z from another template's weights, the veto applied after the maximum, the tie order."""
+    wl = W.config2(n_sft=96, n_sky=5, band_hz=0.05)
+    g = wl.grid
+    recs = [(g.f0_start + i * g.df0, g.f1_start + j * g.df1, s[0], s[1], s[2], 0.0, 86400.0, g.t_ref)
+            for s in g.sky for j in range(g.n_f1) for i in range(g.n_f0)]
+    tl = np.array(recs, dtype=fo.TEMPLATE_DTYPE)
+    for ant in (None, W.antenna_geometry(wl)):
+        o = fo.Oracle(wl, antenna=ant)
+        a = o.eval_range_z()
+        b = fo.eval_templates_z(o, tl, g.t_ref)
+        for x, y in zip(a, b):
+            assert np.array_equal(x, y)
+        if ant is not None:
+            assert np.ptp(b[5]) > 1e-3 * b[5].mean()
+    power, _, wcount, _, z, _ = b
+    floor = float(np.quantile(wcount, 0.7))
+    for by_z in (False, True):
+        key = z if by_z else power
+        ref = sorted((-(key[i]), i) for i in range(key.size) if wcount[i] >= floor)[0][1]
+        assert fo.loudest_of_bank(power, wcount, z, floor, by_z) == ref
+    assert fo.loudest_of_bank(power, wcount, z, 2.0 * wcount.max()) == -1
+    assert fo.loudest_of_bank([1.0, 3.0, 3.0], [1, 1, 1], [0, 0, 0]) == 1
+
+
 def test_mismatch_definition_eq24():
     """Eq. (24): m = 0 at the matched template, m = 1 for a template that recovers only the noise mean."""
     assert fo.mismatch(3.0, 3.0, 1.0) == 0.0 and fo.mismatch(3.0, 1.0, 1.0) == 1.0
