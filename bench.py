@@ -266,6 +266,7 @@ def bank_run(args, dev, flush, wl, binary, measured):
     by one ft_eval_bank call; best of two timed repetitions after a warm-up."""
     r = Runner(wl, dev, args)
     g = wl.grid
+    binary = bool(binary and float(np.max(g.a_p)) > 0.0)   # (--only-bank binary on an isolated configuration: isolated bank)
     box = dict(f0_lo=g.f0_start, f0_hi=g.f0_start + (g.n_f0 - 1) * g.df0, f1_lo=g.f1_start, f1_hi=g.f1_start + (g.n_f1 - 1) * g.df1,
                ra_lo=0.0, ra_hi=2 * np.pi, sd_lo=-1.0, sd_hi=1.0,
                ap_lo=float(np.min(g.a_p)) if binary else 0.0, ap_hi=float(np.max(g.a_p)) if binary else 0.0,
@@ -290,8 +291,28 @@ def bank_run(args, dev, flush, wl, binary, measured):
            "value": evals / (best_ms * 1e-3), "unit": UNIT, "kernel_ms": best_ms,
            "bound": "alu (fp64 pipe)", "fp64_pipe_slots_per_eval": instr,
            "roofline_frac": evals * instr / (best_ms * 1e-3) / fp64_peak,
+           "roofline_frac_of_nominal": evals * instr / (best_ms * 1e-3) / (FP64_FMA_PER_CLK_SM * N_SM * 1.965e9),
            "peak": fp64_peak, "peak_unit": "fp64 instr/s",
            "peak_source": "ft_measure_peaks DFMA rate (of measured)" if measured else "nominal 64 DFMA/clk/SM (of nominal)"}
+    if not binary and not wl.per_bin_weights:
+        # the paper's per-box step on a random bank, end to end (Eq. 36): sky-dependent weights
+        # (Eq. 4-5) per template, both statistics, weighted-count floor mu + 3 sigma, loudest by z -- ft_eval_bank_veto
+        r.ctx.set_antenna(*W.antenna_geometry(wl))
+        p_hit = float(np.exp(-wl.rho_th))
+        n_eff = wl.n_sft      # (sum w = 1 per sky point; sum w^2 ~ 1 / n_sft: the floor of a uniform-weight bank)
+        wfloor = p_hit + 3.0 * np.sqrt(p_hit * (1.0 - p_hit) / n_eff)
+        veto_ms = None
+        for rep in range(3):
+            flush.fill_(rep)
+            best, _ = r.ctx.eval_bank_veto(box, 7, 0, n, wl.rho_th, wfloor, True)
+            ms = r.ctx.counters()["last_kernel_ms"]
+            if rep > 0:
+                veto_ms = ms if veto_ms is None else min(veto_ms, ms)
+        res["per_box_procedure"] = {"call": "ft_set_antenna + ft_eval_bank_veto (both statistics, weighted-count floor, loudest by z)",
+                                    "value": evals / (veto_ms * 1e-3), "unit": UNIT, "kernel_ms": veto_ms,
+                                    "wcount_floor": wfloor, "winner_found": bool(best["idx"] != np.uint64(2 ** 64 - 1)),
+                                    "winner_z": float(best["z"])}
+        r.ctx.set_antenna(None)
     r.close()
     return res
 

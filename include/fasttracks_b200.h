@@ -312,6 +312,25 @@ int ft_eval_bank(ft_ctx* ctx, const ft_bank_box* box, uint64_t seed, uint64_t fi
                  ft_template* best_template_host);
 
 /*
+ * ft_eval_bank_veto — the paper's per-box step on a random bank, end to end (:476 "retrieve the loudest template per
+ * box"; :496-502 "the loudest normalized power ... subject to a minimal weighted number count"; Eq. 36 :346): draw
+ * and evaluate templates first .. first + n - 1 of the xi-uniform bank as ft_eval_bank does, with BOTH statistics
+ * from one gather, and return the template with the largest z (rank_by_z != 0) or normalized power among those whose
+ * weighted number count sum_a w_a [P > rho_th] is >= wcount_floor (0 = no veto); ties to the lower position.
+ * With sky-dependent weights (ft_set_antenna) every template carries the weights, mu_G = 1 and sigma_G of its own
+ * sky position, so the order by z differs from the order by power.
+ *   out_power_dev / out_count_dev  [device] fp32 / int32 [n] or NULL: every statistic, as ft_eval_bank.
+ *   best_host [host] ft_cand_box or NULL: the winner re-evaluated in fp64 (power, wcount, count, z, sigma; idx =
+ *             position in the stream; box = -1).  idx = UINT64_MAX if the veto leaves no template (FT_OK).
+ *   best_template_host [host] ft_template or NULL (untouched when there is no winner).
+ * The veto and the ranking use the kernel's fp64 sums (for fixed weights the same bits as the plain definition; with
+ * sky-dependent weights within ~1e-15 of it).  Synchronises the stream.
+ */
+int ft_eval_bank_veto(ft_ctx* ctx, const ft_bank_box* box, uint64_t seed, uint64_t first, int64_t n, double rho_th,
+                      double wcount_floor, int rank_by_z, float* out_power_dev, int32_t* out_count_dev,
+                      ft_cand_box* best_host, ft_template* best_template_host);
+
+/*
  * ft_track — the track of ONE explicit template: bin k_a (Eq. 2 rounded to the bin grid, :248) for every SFT.
  *   template_host [host]; k_out_host [host] int64 [n_sft].  For building injections (a "data stream containing a
  *   CW signal", :322) without leaving the library.  Synchronises.  FT_ERR_TRACK_RANGE if a bin is outside.

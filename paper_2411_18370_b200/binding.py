@@ -14,7 +14,7 @@ FT_STAT = {"power": 0, "hough": 1, "both": 2, "whough": 3}
 FT_OPT_KERNEL, FT_OPT_FUSED_TOPK, FT_OPT_POINTS_PER_CTA, FT_OPT_PACKED_COUNT, FT_OPT_F0_TILES = 0, 1, 2, 3, 4
 FT_OPT_SELECT_CAP, FT_OPT_COUNT_FLOOR, FT_OPT_ONE_PASS_BOTH, FT_OPT_WCOUNT_FLOOR, FT_OPT_VETO_FIRST, FT_OPT_TAIL_PACKING = 5, 6, 7, 8, 9, 10
 SYMBOLS = ["ft_create", "ft_eval", "ft_topk_per_band", "ft_topk_per_box", "ft_set_antenna", "ft_eval_list",
-           "ft_eval_templates", "ft_eval_templates_noalloc", "ft_bank_draw", "ft_eval_bank", "ft_track", "ft_set_option", "ft_set_option_f64",
+           "ft_eval_templates", "ft_eval_templates_noalloc", "ft_bank_draw", "ft_eval_bank", "ft_eval_bank_veto", "ft_track", "ft_set_option", "ft_set_option_f64",
            "ft_get_counters", "ft_measure_peaks", "ft_selftest", "ft_last_error", "ft_describe", "ft_destroy"]
 
 
@@ -111,6 +111,9 @@ def load_library(path: str | None = None):
         lib.ft_eval_bank.restype = C.c_int
         lib.ft_eval_bank.argtypes = [C.c_void_p, C.POINTER(FtBankBox), C.c_uint64, C.c_uint64, C.c_int64, C.c_int,
                                      C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.ft_eval_bank_veto.restype = C.c_int
+        lib.ft_eval_bank_veto.argtypes = [C.c_void_p, C.POINTER(FtBankBox), C.c_uint64, C.c_uint64, C.c_int64, C.c_double,
+                                          C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.ft_track.restype = C.c_int
         lib.ft_track.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         lib.ft_set_option_f64.restype = C.c_int
@@ -287,6 +290,21 @@ class Context:
         bx = self._box(box)
         self._check(self.lib.ft_eval_bank(self.h, C.byref(bx), int(seed), int(first), int(n), FT_STAT[stat], float(rho_th),
                                           pp, pc, _hp(best), _hp(tp)))
+        return best[0], tp[0]
+
+    def eval_bank_veto(self, box: dict, seed: int, first: int, n: int, rho_th: float, wcount_floor: float = 0.0,
+                       rank_by_z: bool = False, out_power=None, out_count=None):
+        """ft_eval_bank_veto: the loudest template (by z or power) among those passing the weighted-count floor;
+        returns (ft_cand_box record, template record); record idx = 2^64 - 1 if none passes."""
+        for o in (out_power, out_count):
+            assert o is None or (o.is_cuda and o.numel() == n and o.is_contiguous())
+        pp = C.c_void_p(out_power.data_ptr()) if out_power is not None else None
+        pc = C.c_void_p(out_count.data_ptr()) if out_count is not None else None
+        best = np.zeros(1, dtype=CAND_BOX_DTYPE)
+        tp = np.zeros(1, dtype=TEMPLATE_DTYPE)
+        bx = self._box(box)
+        self._check(self.lib.ft_eval_bank_veto(self.h, C.byref(bx), int(seed), int(first), int(n), float(rho_th),
+                                               float(wcount_floor), int(bool(rank_by_z)), pp, pc, _hp(best), _hp(tp)))
         return best[0], tp[0]
 
     def track(self, template, t_ref: float):

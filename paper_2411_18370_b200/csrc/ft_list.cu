@@ -163,7 +163,7 @@ __global__ void k1_scatter_kernel(const __grid_constant__ FtDev d, const FtTempl
   if (j < n) perm[atomicAdd(cursor + k1_bucket<GEN>(d, tl, bx, seed, first, j), 1u)] = (uint32_t)j;
 }
 
-struct K1Acc { double power; int32_t count; unsigned ties; unsigned bad; double wsum; };
+struct K1Acc { double power; int32_t count; unsigned ties; unsigned bad; double wsum; double wcount; double wsq; };
 
 #ifndef FT_K1_INT_CVT
 #define FT_K1_INT_CVT 0   // fp32 -> fp64 by the conversion instruction (0: measured faster, one issue slot) or by integer moves (1)
@@ -183,7 +183,9 @@ __device__ __forceinline__ double k1_f2d(float x) {
 // SKY: sky-dependent weights (Eq. 4-5, ft_set_antenna): the weight of SFT a is u_a(n) w_a, u = a^2 + b^2 from the
 // staged antenna coefficients sAnt[9 c ..] and the template's sky factors sk; acc.wsum carries sum_a u_a w_a and the
 // caller divides by it at the end (the order of ft_refine_one).  Implies per-SFT weights.
-template <int STAT, int BIN, bool PERSFT, bool SKY>
+// EXT (ft_eval_bank_veto; STAT == 2): also the weighted number count sum_a w_a [P > rho] (acc.wcount) and, with SKY,
+// sum_a (u_a w_a)^2 (acc.wsq) for sigma_G of Eq. (36).
+template <int STAT, int BIN, bool PERSFT, bool SKY, bool EXT = false>
 __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp, double Om, double apOm, bool binary,
                                          const double2* sA, const double2* sB, const double2* sC, const double* sAnt,
                                          const FtSkyPoint& sk, int m, int64_t a0, uint32_t n_bins, K1Acc& acc) {
@@ -222,8 +224,10 @@ __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp
       if (SKY) {
         w = __dmul_rn(ft_antenna_u(sAnt + 9 * c, sk), w);
         acc.wsum = __dadd_rn(acc.wsum, w);
+        if (EXT) acc.wsq = __fma_rn(w, w, acc.wsq);
       }
       acc.power = fma(w, k1_f2d(pix), acc.power);  // (fixed weights: exact product, same as mul then add)
+      if (EXT) acc.wcount = __dadd_rn(acc.wcount, (pix > d.rho) ? w : 0.0);
     }
     if (STAT != 0) acc.count += (pix > d.rho) ? 1 : 0;
     prow += ld;
@@ -233,13 +237,13 @@ __device__ __forceinline__ void k1_chunk(const FtDev& d, const FtTemplateDev& tp
 
 // STAT: 0 power, 1 count, 2 both.  GEN: templates drawn in registers from (seed, first + q) instead of read.
 // BEST: per-CTA loudest (value desc, index asc) to best_v / best_i [gridDim.x].
-template <int STAT, bool GEN, bool BEST, bool SKY>
+template <int STAT, bool GEN, bool BEST, bool SKY, bool EXT = false>
 __global__ void __launch_bounds__(K1_THREADS)
 ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict__ tl, const __grid_constant__ FtBankBox bx,
                uint64_t seed, uint64_t first, int64_t n, double t_ref,
                float* __restrict__ out_power, int32_t* __restrict__ out_count, int32_t* __restrict__ err,
                unsigned long long* __restrict__ near_ties, double* __restrict__ best_v, int64_t* __restrict__ best_i,
-               const uint32_t* __restrict__ perm) {
+               const uint32_t* __restrict__ perm, double wfloor = 0.0, int by_z = 0) {
   // per-SFT tables of the current chunk: (vx, vy), (vz, t - t_ref), (w, t): three LDS.128 per evaluation at most
   __shared__ double2 sA[K1_THREADS], sB[K1_THREADS], sC[K1_THREADS];
   __shared__ double sAnt[SKY ? 9 * K1_THREADS : 1];   // antenna coefficients A[5], B[4] of the chunk's SFTs
@@ -254,7 +258,7 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
   const bool all_binary = __syncthreads_and(binary || !active) != 0;
   const uint32_t n_bins = (uint32_t)min(d.n_bins, (int64_t)0x7fffffff);
   const bool per_sft = d.wkind == 1;
-  K1Acc acc{0.0, 0, 0u, 0u, 0.0};
+  K1Acc acc{0.0, 0, 0u, 0u, 0.0, 0.0, 0.0};
   FtSkyPoint sk{};
   if (SKY) sk = ft_sky_point(tp.nx, tp.ny, tp.nz);
   for (int64_t a0 = 0; a0 < d.n_sft; a0 += K1_THREADS) {
@@ -274,18 +278,18 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
     const int m = (int)min((int64_t)K1_THREADS, d.n_sft - a0);
     if (active) {
       if (SKY) {   // (sky-dependent weights need per-SFT weights: ft_set_antenna)
-        if (all_binary) k1_chunk<STAT, 2, true, true>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
-        else if (any_binary) k1_chunk<STAT, 1, true, true>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
-        else k1_chunk<STAT, 0, true, true>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        if (all_binary) k1_chunk<STAT, 2, true, true, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else if (any_binary) k1_chunk<STAT, 1, true, true, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 0, true, true, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
       } else if (all_binary) {
-        if (per_sft) k1_chunk<STAT, 2, true, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
-        else k1_chunk<STAT, 2, false, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        if (per_sft) k1_chunk<STAT, 2, true, false, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 2, false, false, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
       } else if (any_binary) {
-        if (per_sft) k1_chunk<STAT, 1, true, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
-        else k1_chunk<STAT, 1, false, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        if (per_sft) k1_chunk<STAT, 1, true, false, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 1, false, false, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
       } else {
-        if (per_sft) k1_chunk<STAT, 0, true, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
-        else k1_chunk<STAT, 0, false, false>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        if (per_sft) k1_chunk<STAT, 0, true, false, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
+        else k1_chunk<STAT, 0, false, false, EXT>(d, tp, Om, apOm, binary, sA, sB, sC, sAnt, sk, m, a0, n_bins, acc);
       }
     }
   }
@@ -303,6 +307,12 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
     __shared__ double bv[K1_THREADS / 32];
     __shared__ long long bi[K1_THREADS / 32];
     double v = (active && !bad) ? (STAT == 1 ? (double)count : power) : -INFINITY;
+    if (EXT) {   // the per-box step of the paper on a random bank: veto on the weighted number count, rank by z (Eq. 36)
+      const double wc = SKY ? acc.wcount / acc.wsum : acc.wcount;
+      const double mu = SKY ? 1.0 : d.mu_G, sigma = SKY ? sqrt(acc.wsq) / acc.wsum : d.sigma_G;
+      if (by_z) v = (power - mu) / sigma;
+      if (!(active && !bad) || wc < wfloor) v = -INFINITY;
+    }
     long long i = active ? (long long)q : 0x7fffffffffffffffll;   // (the template's index, not the slot)
     for (int o = 16; o > 0; o >>= 1) {
       const double v2 = __shfl_xor_sync(0xffffffffu, v, o);
@@ -314,6 +324,7 @@ ft_list_kernel(const __grid_constant__ FtDev d, const FtTemplateDev* __restrict_
     if (threadIdx.x == 0) {
       for (int wv = 1; wv < K1_THREADS / 32; ++wv)
         if (bv[wv] > v || (bv[wv] == v && bi[wv] < i)) { v = bv[wv]; i = bi[wv]; }
+      if (EXT && v == -INFINITY) i = 0x7fffffffffffffffll;   // nobody of this CTA passed the veto
       best_v[blockIdx.x] = v; best_i[blockIdx.x] = i;
     }
   }
@@ -399,7 +410,7 @@ template <bool GEN, bool BEST>
 cudaError_t launch_list(const FtDev& d, int stat, const FtTemplateDev* tl, const FtBankBox& bx, uint64_t seed, uint64_t first,
                         int64_t n, double t_ref, float* out_power, int32_t* out_count, int32_t* err,
                         unsigned long long* near_ties, double* best_v, int64_t* best_i, uint32_t* perm, cudaStream_t s,
-                        int* launches) {
+                        int* launches, bool ext = false, double wfloor = 0.0, int by_z = 0) {
   *launches = 0;
   if (n <= 0) return cudaSuccess;
   const unsigned grid = (unsigned)((n + K1_THREADS - 1) / K1_THREADS);
@@ -414,6 +425,14 @@ cudaError_t launch_list(const FtDev& d, int stat, const FtTemplateDev* tl, const
     *launches += 3;
   }
   const bool sky = d.skyw && d.ant && stat != 1;   // (the number count does not see the weights)
+  if constexpr (GEN && BEST) {
+    if (ext) {   // ft_eval_bank_veto: both statistics + weighted count (+ sigma_G), veto and z in the winner search
+      if (sky) ft_list_kernel<2, true, true, true, true><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm, wfloor, by_z);
+      else ft_list_kernel<2, true, true, false, true><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm, wfloor, by_z);
+      *launches += 1;
+      return cudaGetLastError();
+    }
+  }
   if (stat == 0 && sky) ft_list_kernel<0, GEN, BEST, true><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
   else if (stat == 0) ft_list_kernel<0, GEN, BEST, false><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
   else if (stat == 1) ft_list_kernel<1, GEN, BEST, false><<<grid, K1_THREADS, 0, s>>>(d, tl, bx, seed, first, n, t_ref, out_power, out_count, err, near_ties, best_v, best_i, perm);
@@ -490,12 +509,14 @@ int ft_bank_draw(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t firs
   return FT_OK;
 }
 
-int ft_eval_bank(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t first, int64_t n, int stat, double rho_th,
-                 float* out_power_dev, int32_t* out_count_dev, ft_cand* best_host, ft_template* best_template_host) {
+// ft_eval_bank (ext = false) and ft_eval_bank_veto (ext = true: both statistics, veto floor, rank by z; best_box_host)
+static int eval_bank_impl(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t first, int64_t n, int stat, double rho_th,
+                          float* out_power_dev, int32_t* out_count_dev, ft_cand* best_host, ft_template* best_template_host,
+                          bool ext, double wfloor, int by_z, ft_cand_box* best_box_host) {
   if (!c || !box) return FT_ERR_ARG;
   if (n < 1) return ft_fail(c, FT_ERR_ARG, "ft_eval_bank: n >= 1");
-  if (stat != FT_STAT_POWER && stat != FT_STAT_HOUGH) return ft_fail(c, FT_ERR_ARG, "ft_eval_bank: stat must be power or hough");
-  if (!std::isfinite(rho_th)) return ft_fail(c, FT_ERR_ARG, "ft_eval_bank: non-finite argument");
+  if (!ext && stat != FT_STAT_POWER && stat != FT_STAT_HOUGH) return ft_fail(c, FT_ERR_ARG, "ft_eval_bank: stat must be power or hough");
+  if (!std::isfinite(rho_th) || !std::isfinite(wfloor)) return ft_fail(c, FT_ERR_ARG, "ft_eval_bank: non-finite argument");
   if (int rc = check_box(c, box)) return rc;
   if (!c->d.P) return ft_fail(c, FT_ERR_STATE, "ft_eval_bank: handle not created");
   if (int rc = ft_enter(c)) return rc;
@@ -517,7 +538,8 @@ int ft_eval_bank(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t firs
   int launches = 0;
   ft_tick(c);
   const cudaError_t e = launch_list<true, true>(d, stat, nullptr, bx, seed, first, n, box->t_ref, out_power_dev, out_count_dev,
-                                                c->flag_dev, c->near_ties_dev, best_v, best_i, perm, c->stream, &launches);
+                                                c->flag_dev, c->near_ties_dev, best_v, best_i, perm, c->stream, &launches,
+                                                ext, wfloor, by_z);
   ft_tock(c, launches);
   if (e != cudaSuccess) return ft_fail(c, FT_ERR_CUDA, std::string("ft_eval_bank: ") + cudaGetErrorString(e));
   ft_best_reduce_kernel<<<1, 1024, 0, c->stream>>>(best_v, best_i, n_blocks);
@@ -528,8 +550,13 @@ int ft_eval_bank(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t firs
   FT_CUDA(c, cudaMemcpyAsync(&win, best_i, sizeof win, cudaMemcpyDeviceToHost, c->stream));
   FT_CUDA(c, cudaMemcpyAsync(&flag, c->flag_dev, sizeof flag, cudaMemcpyDeviceToHost, c->stream));
   FT_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (ext && (win < 0 || win >= n)) {   // the veto left no template (or every track left the spectrogram: flag below)
+    if (best_box_host) { *best_box_host = ft_cand_box{}; best_box_host->idx = UINT64_MAX; best_box_host->box = -1; }
+    if (flag) return ft_fail(c, FT_ERR_TRACK_RANGE, "ft_eval_bank_veto: some tracks leave the spectrogram (their outputs are NaN / -1; they never win)");
+    return FT_OK;
+  }
   if (win < 0 || win >= n) return ft_fail(c, FT_ERR_TRACK_RANGE, "ft_eval_bank: every track leaves the spectrogram");
-  if (best_host || best_template_host) {
+  if (best_host || best_template_host || best_box_host) {
     // the winner again, in the refinement arithmetic (power, weighted count, count), from its regenerated parameters
     ft_bank_draw_kernel<<<1, 32, 0, c->stream>>>(bx, seed, first + (uint64_t)win, 1, tp_dev);
     FT_CUDA(c, cudaGetLastError());
@@ -541,10 +568,24 @@ int ft_eval_bank(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t firs
     FT_CUDA(c, cudaMemcpyAsync(&tp, tp_dev, sizeof tp, cudaMemcpyDeviceToHost, c->stream));
     FT_CUDA(c, cudaStreamSynchronize(c->stream));
     if (best_host) *best_host = ft_cand{cd.power, cd.wcount, (uint64_t)win, cd.count, -1};
+    if (best_box_host) *best_box_host = ft_cand_box{cd.power, cd.wcount, (uint64_t)win, cd.count, -1, cd.z, cd.sigma};
     if (best_template_host) std::memcpy(best_template_host, &tp, sizeof tp);
   }
   if (flag) return ft_fail(c, FT_ERR_TRACK_RANGE, "ft_eval_bank: some tracks leave the spectrogram (their outputs are NaN / -1; they never win)");
   return FT_OK;
+}
+
+int ft_eval_bank(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t first, int64_t n, int stat, double rho_th,
+                 float* out_power_dev, int32_t* out_count_dev, ft_cand* best_host, ft_template* best_template_host) {
+  return eval_bank_impl(c, box, seed, first, n, stat, rho_th, out_power_dev, out_count_dev, best_host, best_template_host,
+                        false, 0.0, 0, nullptr);
+}
+
+int ft_eval_bank_veto(ft_ctx* c, const ft_bank_box* box, uint64_t seed, uint64_t first, int64_t n, double rho_th,
+                      double wcount_floor, int rank_by_z, float* out_power_dev, int32_t* out_count_dev,
+                      ft_cand_box* best_host, ft_template* best_template_host) {
+  return eval_bank_impl(c, box, seed, first, n, FT_STAT_BOTH, rho_th, out_power_dev, out_count_dev, nullptr, best_template_host,
+                        true, wcount_floor, rank_by_z ? 1 : 0, best_host);
 }
 
 int ft_track(ft_ctx* c, const ft_template* tp_host, double t_ref, int64_t* k_out_host) {

@@ -285,3 +285,54 @@ def test_mismatch_sampler_against_the_oracles_sampler():
             assert np.all(got["m"] <= prev + 1e-12) and np.median(got["m"]) <= np.median(prev)
         prev = got["m"]
     assert np.median(prev) < 0.9      # sixteen-fold oversampling recovers a good part of the signal
+
+
+@pytest.mark.parametrize("cfg,binary,antenna", [(2, False, False), (2, False, True), (3, True, True), (4, False, False)])
+def test_loudest_of_a_random_bank_under_the_veto_by_z(cfg, binary, antenna):
+    """ft_eval_bank_veto = the paper's per-box procedure on the unstructured path (Eq. 36):
+    random bank, both statistics from one gather, weighted-count floor, loudest by z.  Against the oracle's
+    eval_templates_z + loudest_of_bank on ITS draw of the same stream: the same winner (when no near-tie template
+    and no fp64-rounding-level tie could change it), its refined power / wcount / z / sigma_G, and the full arrays."""
+    import torch
+    wl = {2: lambda: W.config2(n_sft=501, n_sky=7, band_hz=0.35),
+          3: lambda: W.config3(n_sft=403, n_ap=3, n_porb=3, n_tasc=2, n_inj=0),
+          4: lambda: W.config4(n_sft=300, n_sky=5, band_hz=0.4, n_lines=6)}[cfg]()
+    ant = W.antenna_geometry(wl) if antenna else None
+    o = fo.Oracle(wl, antenna=ant)
+    box = _box(wl, binary)
+    n, seed, first = 6000, 29, 11
+    otl = fo.bank_draw(box, seed, first, n)
+    op, oc, owc, otie, oz, osig = fo.eval_templates_z(o, otl, box["t_ref"])
+    ctx = H.gpu_context(wl)
+    if antenna:
+        ctx.set_antenna(*ant)
+    dev = torch.device("cuda:0")
+    gp = torch.full((n,), float("nan"), dtype=torch.float32, device=dev)
+    gc = torch.full((n,), -7, dtype=torch.int32, device=dev)
+    floors = (0.0, float(np.quantile(owc, 0.9)), float(np.quantile(owc, 0.999)), 10.0 * float(owc.max()))
+    for floor in floors:
+        for by_z in (False, True):
+            best, btp = ctx.eval_bank_veto(box, seed, first, n, wl.rho_th, floor, by_z, out_power=gp, out_count=gc)
+            j = fo.loudest_of_bank(op, owc, oz, floor, by_z)
+            if j < 0:
+                assert best["idx"] == np.uint64(2 ** 64 - 1)
+                continue
+            key = oz if by_z else op
+            passing = owc >= floor
+            # unambiguous: the winner is clear of the runner-up and of the floor beyond fp64 rounding, no near-tie in reach
+            runner = np.sort(key[passing])[-2] if passing.sum() > 1 else -np.inf
+            clear = (key[j] - runner > 1e-9 * abs(key[j])) and not np.any((otie != 0) & (key >= key[j] - 0.2 * abs(key[j]))) \
+                and np.min(np.abs(owc - floor)) > 1e-12
+            if clear:
+                assert int(best["idx"]) == j, (floor, by_z)
+                tol = 1e-12 if antenna else 0.0
+                assert abs(best["power"] - op[j]) <= tol * op[j] and best["count"] == oc[j]
+                assert abs(best["wcount"] - owc[j]) <= max(tol, 1e-15) * owc[j]
+                assert abs(best["z"] - oz[j]) <= 1e-9 * max(1.0, abs(oz[j])) and abs(best["sigma"] - osig[j]) <= 1e-12 * osig[j]
+                assert abs(btp["f0"] - otl["f0"][j]) <= 1e-13 * otl["f0"][j]
+    ok = otie == 0
+    assert np.array_equal(gc.cpu().numpy()[ok], oc[ok])
+    assert (np.abs(gp.cpu().numpy().astype(np.float64) - op) / op)[ok].max() <= 1e-6
+    if antenna and cfg == 2:   # the order by z is not the order by power when sigma_G varies over the sky
+        assert not np.array_equal(np.argsort(-oz)[:50], np.argsort(-op)[:50])
+    ctx.close()
