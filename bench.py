@@ -491,8 +491,12 @@ def run_gpu(args):
                           "ms_per_step": res["kernel_ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                           "dtype": "f64", "data": "synthetic", "config": {"workload": res["workload"]}, "k1": res}))
         return
-    r = Runner(wl, dev, args, stat=args.stat or None)
+    r = Runner(wl, dev, args, stat=("both" if args.veto_sigma > 0 else args.stat) or None)
     measured = r.ctx.measure_peaks() if not args.no_peaks else None
+    if args.veto_sigma > 0:   # the veto of PAPER.md:496-502 (the command of profiles/r03_refine_thread_ncu.md)
+        from paper_2411_18370_b200 import binding as B
+        p_hit = float(np.exp(-wl.rho_th)); w64 = np.asarray(wl.w, dtype=np.float64)
+        r.ctx.set_option_f64(B.FT_OPT_WCOUNT_FLOOR, p_hit * w64.sum() + args.veto_sigma * np.sqrt(p_hit * (1.0 - p_hit) * (w64 ** 2).sum()))
     if args.antenna:   # sky-dependent weights (Eq. 4-5): the row-weighted tile kernel
         r.ctx.set_antenna(*W.antenna_geometry(wl))
     base_step = r.full_arrays_step() if args.full_arrays else r.step
@@ -574,7 +578,7 @@ def run_gpu(args):
             "counters": {k: c1[k] for k in ("near_ties", "appended", "refined", "refine_fallbacks")},
             "kernel_geometry": r.ctx.describe(),
         }
-        if world == 1 and not args.no_extra and args.config == 2 and not args.n_sky and not args.n_sft and not args.stat and not args.full_arrays and not args.antenna:
+        if world == 1 and not args.no_extra and args.config == 2 and not args.n_sky and not args.n_sft and not args.stat and not args.full_arrays and not args.antenna and not args.veto_sigma:
             out["extra"] = extra_runs(args, dev, flush, measured, peaks, None)
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"], _ = oracle_sample(wl, seconds=args.cpu_seconds)
@@ -626,6 +630,8 @@ def main(argv=None):
     ap.add_argument("--only-bank", default="", choices=["", "isolated", "binary"],
                     help="run K1 alone: a xi-uniform random bank on the configuration's spectrogram")
     ap.add_argument("--antenna", action="store_true", help="sky-dependent weights w_a(n) (ft_set_antenna with the workload's detector geometry)")
+    ap.add_argument("--veto-sigma", type=float, default=0.0,
+                    help="> 0: power top-k under the weighted number-count floor mu + X sigma (PAPER.md:496-502); implies --stat both")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="headline configuration only")
     ap.add_argument("--no-peaks", action="store_true", help="skip ft_measure_peaks (roofline against nominal peaks)")

@@ -147,7 +147,17 @@ ft_refine_kernel(const __grid_constant__ FtDev d, const uint64_t* __restrict__ i
 // Long candidate lists (the survivors of a number-count veto, ft_topk.cu): ONE THREAD per candidate walks the SFTs
 // in ascending order, so the sums have the oracle's rounding sequence without the 32-fold redundancy of the
 // warp-per-candidate form (which is the faster one for the few hundred candidates of a plain top-k).
-__global__ void __launch_bounds__(128)
+#ifndef FT_RT_MINB
+#define FT_RT_MINB 8     // CTAs of 128 threads per SM the register budget is held to (8 -> 64 registers)
+#endif
+#ifndef FT_RT_UNROLL
+#define FT_RT_UNROLL 8
+#endif
+#define FT_STR2(x) #x
+#define FT_STR(x) FT_STR2(x)
+// SKY: sky-dependent weights (their nine sky factors stay out of the register budget of the fixed-weight variant).
+template <bool SKY>
+__global__ void __launch_bounds__(128, SKY ? 4 : FT_RT_MINB)
 ft_refine_thread_kernel(const __grid_constant__ FtDev d, const uint64_t* __restrict__ idx_list, int64_t n,
                         FtCandDev* __restrict__ out, unsigned long long* __restrict__ near_ties) {
   const int64_t cand = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -160,12 +170,15 @@ ft_refine_thread_kernel(const __grid_constant__ FtDev d, const uint64_t* __restr
   int32_t count = 0;
   unsigned ties = 0;
   FtSkyPoint sk;
-  if (d.skyw) sk = ft_sky_point(p.nx, p.ny, p.nz);
+  if (SKY) sk = ft_sky_point(p.nx, p.ny, p.nz);
   // branch-free body (an out-of-range bin -- impossible for a validated grid -- contributes an exact zero), unrolled
-  // so that the gathers of several SFTs are in flight; the sums are still added in ascending SFT order.  The kernel is
-  // bound by the scattered gathers (246 000 survivors of config 2: 8.0 -> 6.7 ms with this form; staging the per-SFT
-  // tables in shared memory as K1 does measured slower, 7.3 ms).
-#pragma unroll 4
+  // so that the gathers of several SFTs are in flight; the sums are still added in ascending SFT order.
+  // Round 3 (ncu: profiles/r03_refine_thread_ncu.md): the kernel was latency-bound at 94 registers = 5 CTAs per SM
+  // (long-scoreboard stalls 65 % of the issue slots, 2.6 waves); the sky factors moved into a template variant
+  // (64 registers, 8 CTAs per SM): 6.7 -> 4.4 ms for the 246 000 survivors of config 2 (step 95.8 -> 93.5 ms).  Staging
+  // the per-SFT tables per 128-SFT chunk in shared memory measured the same at 64 registers (it spills) and 1 ms
+  // slower at 80; unroll 4 and 8 measure the same.
+  _Pragma(FT_STR(unroll FT_RT_UNROLL))
   for (int64_t a = 0; a < d.n_sft; ++a) {
     const double t = d.t_mid[a];
     const double D = ft_doppler_rcp(d, p, a, t);
@@ -176,7 +189,7 @@ ft_refine_thread_kernel(const __grid_constant__ FtDev d, const uint64_t* __restr
     const int64_t off = a * d.ld + (ok ? k : 0);
     const float pix = ok ? __ldg(d.P + off) : 0.f;
     double wa = (double)((d.wkind == 1) ? __ldg(d.w + a) : __ldg(d.w + off));
-    if (d.skyw) {
+    if (SKY) {
       wa = __dmul_rn(ft_antenna_u(d.ant + 9 * a, sk), wa);
       wsum = __dadd_rn(wsum, wa);
       wsq = __dadd_rn(wsq, __dmul_rn(wa, wa));
@@ -187,7 +200,7 @@ ft_refine_thread_kernel(const __grid_constant__ FtDev d, const uint64_t* __restr
     count += hit ? 1 : 0;
   }
   double mu = d.mu_G, sigma = d.sigma_G;
-  if (d.skyw) { power = power / wsum; wcount = wcount / wsum; mu = 1.0; sigma = sqrt(wsq) / wsum; }
+  if (SKY) { power = power / wsum; wcount = wcount / wsum; mu = 1.0; sigma = sqrt(wsq) / wsum; }
   FtCandDev c;
   c.power = power; c.wcount = wcount; c.idx = idx; c.count = count; c.band = -1;   // (bad cannot happen: the grid was validated at bind)
   c.sigma = sigma; c.z = (power - mu) / sigma;
@@ -260,7 +273,8 @@ cudaError_t ft_launch_refine(const FtDev& d, const uint64_t* idx_dev, const uint
                              FtCandDev* out, unsigned long long* near_ties, cudaStream_t s) {
   if (n_max <= 0) return cudaSuccess;
   if (!n_dev && n_max >= 8192) {   // a long list of known length: one thread per candidate
-    ft_refine_thread_kernel<<<(unsigned)((n_max + 127) / 128), 128, 0, s>>>(d, idx_dev, n_max, out, near_ties);
+    if (d.skyw) ft_refine_thread_kernel<true><<<(unsigned)((n_max + 127) / 128), 128, 0, s>>>(d, idx_dev, n_max, out, near_ties);
+    else ft_refine_thread_kernel<false><<<(unsigned)((n_max + 127) / 128), 128, 0, s>>>(d, idx_dev, n_max, out, near_ties);
     return cudaGetLastError();
   }
   const int64_t warps_per_block = 4;
